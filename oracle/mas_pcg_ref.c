@@ -1,0 +1,270 @@
+/*
+ * mas_pcg_ref.c -- ORACLE.  Test infrastructure, not product code.
+ *
+ * A plain, slow, single-threaded C99 statement of what the MAS PCG hot path computes: the
+ * point-Jacobi (PC1) preconditioned conjugate-gradient solve of the implicit SPD 7-point
+ * finite-difference operator on MAS's non-uniform, logically rectangular spherical mesh
+ * (Sec. 2.2 "non-uniform logically-rectangular ... finite difference", "PCG ...
+ * PC1 uses the inverse diagonal of the matrix (point-Jacobi)"; Sec. 4.1 "sparse
+ * matrix-vector products (essentially stencil operations), basic array operations, and dot
+ * products"; eq. (1) for the operator's form  (1/rho) div(nu rho grad v)).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may load this library.  It shares no source, header, table or helper with the CUDA path
+ * (paper_1811_02605_b200/csrc) and includes none of its files.
+ *
+ * The paper never writes the discrete operator.  The reading used here is
+ * DESIGN.md R1: finite-volume flux form on cell centres, which is what makes the matrix
+ * symmetric on a non-uniform mesh ("our symmetric matrices").
+ *
+ *   cell (i,j,k) has volume            V   = r_c[i]^2 dr_c[i] sin_c[j] dth_c[j] dph_c[k]
+ *   radial face i (between i-1 and i)  G_r = nu_f r_f[i]^2 sin_c[j] dth_c[j] dph_c[k] / dr_f[i]
+ *   theta  face j (between j-1 and j)  G_t = nu_f dr_c[i] sin_f[j] dph_c[k] / dth_f[j]
+ *   phi    face k (between k and k+1)  G_p = nu   dr_c[i] dth_c[j] / (sin_c[j] dph_f[k])
+ *
+ *   (A_sym u)_c = V_c u_c + dt * sum over the 6 faces f of c of  G_f (u_c - u_neighbour(f))
+ *
+ * which is V times the finite-difference form of  u - dt div(nu grad u)  in spherical
+ * coordinates (area/distance per face; the r's cancel on theta faces).  Boundaries:
+ *   radial Dirichlet: homogeneous value ON the boundary face, neighbour value 0, distance
+ *                     dr_f[0] = r_c[0]-r_f[0]  (Q4);  radial Neumann: G = 0 on that face;
+ *   polar axis: sin_f = 0 exactly, so G_t = 0 (Q5);  phi: periodic index wrap.
+ *   nu on a face = arithmetic mean of the two cell values; a boundary face takes its cell's (Q3).
+ *
+ * The system solved (R2): the caller's A_phys x = b with A_phys = diag(V)^-1 A_sym;
+ * internally A_sym x = b_s, b_s = V.b; residuals, norms and the stopping test live in the
+ * symmetric system.  Parity status: pinned by tests/test_oracle_*.py (dense LU, manufactured
+ * solution, symmetry/SPD, Krylov optimality, closed forms, continuum consistency).  What is
+ * tied to the paper's own run (its mesh, nu, RHS, its 70/550 iteration counts) is
+ * "parity unpinned": the data are not available.
+ *
+ * Sums are plain index-order loops with a long double accumulator (Q22).  No blocking, no
+ * fusion, no reordering.  Layout: [nr][nt][np], phi fastest.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+enum { REF_BC_DIRICHLET = 0, REF_BC_NEUMANN = 1 };
+enum { REF_OK = 0, REF_MAXIT = 1, REF_EINVAL = -1, REF_ENOMEM = -2, REF_EBREAKDOWN = -4 };
+
+typedef struct ref_op {
+    int nr, nt, np;
+    double dt;
+    /* face conductances without their phi factor, tabulated once from the 1-D metric arrays */
+    double *gr;   /* [(nr+1)][nt]  nu_f r_f^2 sin_c dth_c / dr_f ; 0 on Neumann boundary faces */
+    double *gt;   /* [nr][(nt+1)]  nu_f dr_c sin_f / dth_f      ; 0 on the polar faces          */
+    double *gp;   /* [nr][nt]      nu   dr_c dth_c / sin_c                                    */
+    double *v2;   /* [nr][nt]      r_c^2 dr_c sin_c dth_c                                      */
+    double *dph_c, *dph_f; /* [np] */
+} ref_op;
+
+static double nu_at(int kind, const double *nu, int nt, int i, int j)
+{
+    return kind == 0 ? nu[0] : nu[(size_t)i * nt + j];
+}
+
+void mas_ref_destroy(ref_op *op)
+{
+    if (!op) return;
+    free(op->gr); free(op->gt); free(op->gp); free(op->v2); free(op->dph_c); free(op->dph_f);
+    free(op);
+}
+
+/* Build the operator of DESIGN.md R1 from the 1-D metric arrays (all HOST pointers). */
+ref_op *mas_ref_create(int nr, int nt, int np,
+                       const double *r_c, const double *dr_c, const double *r_f, const double *dr_f,
+                       const double *sin_c, const double *dth_c, const double *sin_f, const double *dth_f,
+                       const double *dph_c, const double *dph_f,
+                       double dt, int nu_kind, const double *nu, int bc_inner, int bc_outer)
+{
+    if (nr < 1 || nt < 1 || np < 1 || dt < 0.0) return NULL;
+    ref_op *op = (ref_op *)calloc(1, sizeof(ref_op));
+    if (!op) return NULL;
+    op->nr = nr; op->nt = nt; op->np = np; op->dt = dt;
+    op->gr = (double *)calloc((size_t)(nr + 1) * nt, sizeof(double));
+    op->gt = (double *)calloc((size_t)nr * (nt + 1), sizeof(double));
+    op->gp = (double *)calloc((size_t)nr * nt, sizeof(double));
+    op->v2 = (double *)calloc((size_t)nr * nt, sizeof(double));
+    op->dph_c = (double *)malloc(sizeof(double) * np);
+    op->dph_f = (double *)malloc(sizeof(double) * np);
+    if (!op->gr || !op->gt || !op->gp || !op->v2 || !op->dph_c || !op->dph_f) { mas_ref_destroy(op); return NULL; }
+    memcpy(op->dph_c, dph_c, sizeof(double) * np);
+    memcpy(op->dph_f, dph_f, sizeof(double) * np);
+
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j < nt; j++) {
+            op->v2[(size_t)i * nt + j] = r_c[i] * r_c[i] * dr_c[i] * sin_c[j] * dth_c[j];
+            op->gp[(size_t)i * nt + j] = nu_at(nu_kind, nu, nt, i, j) * dr_c[i] * dth_c[j] / sin_c[j];
+        }
+    /* radial faces i = 0..nr */
+    for (int i = 0; i <= nr; i++)
+        for (int j = 0; j < nt; j++) {
+            double nuf;
+            if (i == 0)        nuf = nu_at(nu_kind, nu, nt, 0, j);
+            else if (i == nr)  nuf = nu_at(nu_kind, nu, nt, nr - 1, j);
+            else               nuf = 0.5 * (nu_at(nu_kind, nu, nt, i - 1, j) + nu_at(nu_kind, nu, nt, i, j));
+            double g = nuf * r_f[i] * r_f[i] * sin_c[j] * dth_c[j] / dr_f[i];
+            if (i == 0 && bc_inner == REF_BC_NEUMANN) g = 0.0;
+            if (i == nr && bc_outer == REF_BC_NEUMANN) g = 0.0;
+            op->gr[(size_t)i * nt + j] = g;
+        }
+    /* theta faces j = 0..nt ; the polar faces j = 0 and j = nt have zero area */
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j <= nt; j++) {
+            double g = 0.0;
+            if (j > 0 && j < nt) {
+                double nuf = 0.5 * (nu_at(nu_kind, nu, nt, i, j - 1) + nu_at(nu_kind, nu, nt, i, j));
+                g = nuf * dr_c[i] * sin_f[j] / dth_f[j];
+            }
+            op->gt[(size_t)i * (nt + 1) + j] = g;
+        }
+    return op;
+}
+
+void mas_ref_set_dt(ref_op *op, double dt) { op->dt = dt; }
+
+/* the six face conductances of cell (i,j,k), phi factors included */
+static void faces(const ref_op *op, int i, int j, int k, double g[6])
+{
+    const int nt = op->nt, np = op->np;
+    const int km = (k + np - 1) % np;
+    g[0] = op->gr[(size_t)i * nt + j] * op->dph_c[k];             /* face to i-1 (or inner boundary) */
+    g[1] = op->gr[(size_t)(i + 1) * nt + j] * op->dph_c[k];       /* face to i+1 (or outer boundary) */
+    g[2] = op->gt[(size_t)i * (nt + 1) + j] * op->dph_c[k];       /* face to j-1 (or pole: 0)        */
+    g[3] = op->gt[(size_t)i * (nt + 1) + j + 1] * op->dph_c[k];   /* face to j+1 (or pole: 0)        */
+    g[4] = op->gp[(size_t)i * nt + j] / op->dph_f[km];            /* face to k-1 (periodic)          */
+    g[5] = op->gp[(size_t)i * nt + j] / op->dph_f[k];             /* face to k+1 (periodic)          */
+}
+
+static double volume(const ref_op *op, int i, int j, int k)
+{
+    return op->v2[(size_t)i * op->nt + j] * op->dph_c[k];
+}
+
+void mas_ref_volume(const ref_op *op, double *V)
+{
+    for (int i = 0; i < op->nr; i++)
+        for (int j = 0; j < op->nt; j++)
+            for (int k = 0; k < op->np; k++)
+                V[((size_t)i * op->nt + j) * op->np + k] = volume(op, i, j, k);
+}
+
+/* d = diag(A_sym) = V + dt * (sum of the six face conductances) */
+void mas_ref_diag(const ref_op *op, double *d)
+{
+    double g[6];
+    for (int i = 0; i < op->nr; i++)
+        for (int j = 0; j < op->nt; j++)
+            for (int k = 0; k < op->np; k++) {
+                faces(op, i, j, k, g);
+                d[((size_t)i * op->nt + j) * op->np + k] =
+                    volume(op, i, j, k) + op->dt * (g[0] + g[1] + g[2] + g[3] + g[4] + g[5]);
+            }
+}
+
+/* y = A_sym u, flux-difference form; a missing neighbour across a Dirichlet face has value 0 */
+void mas_ref_apply(const ref_op *op, const double *u, double *y)
+{
+    const int nr = op->nr, nt = op->nt, np = op->np;
+    double g[6];
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j < nt; j++)
+            for (int k = 0; k < np; k++) {
+                const size_t c = ((size_t)i * nt + j) * np + k;
+                const int kp = (k + 1) % np, km = (k + np - 1) % np;
+                faces(op, i, j, k, g);
+                const double uc = u[c];
+                const double u_im = i > 0      ? u[c - (size_t)nt * np] : 0.0;
+                const double u_ip = i < nr - 1 ? u[c + (size_t)nt * np] : 0.0;
+                const double u_jm = j > 0      ? u[c - np] : 0.0;   /* g[2] = 0 at the pole */
+                const double u_jp = j < nt - 1 ? u[c + np] : 0.0;   /* g[3] = 0 at the pole */
+                const double u_km = u[c - k + km];
+                const double u_kp = u[c - k + kp];
+                double flux = g[0] * (uc - u_im) + g[1] * (uc - u_ip)
+                            + g[2] * (uc - u_jm) + g[3] * (uc - u_jp)
+                            + g[4] * (uc - u_km) + g[5] * (uc - u_kp);
+                y[c] = volume(op, i, j, k) * uc + op->dt * flux;
+            }
+}
+
+/* s1-style stiffness: max over cells of (d - V)/V at the operator's current dt (Q12, Q13) */
+double mas_ref_stiffness_max(const ref_op *op)
+{
+    double g[6], m = 0.0;
+    for (int i = 0; i < op->nr; i++)
+        for (int j = 0; j < op->nt; j++)
+            for (int k = 0; k < op->np; k++) {
+                faces(op, i, j, k, g);
+                double s = op->dt * (g[0] + g[1] + g[2] + g[3] + g[4] + g[5]) / volume(op, i, j, k);
+                if (s > m) m = s;
+            }
+    return m;
+}
+
+static double dot(size_t n, const double *a, const double *b)
+{
+    long double s = 0.0L;
+    for (size_t c = 0; c < n; c++) s += (long double)a[c] * (long double)b[c];
+    return (double)s;
+}
+
+/*
+ * Textbook PCG with M = diag(A_sym) ("PCG ... PC1 ... point-Jacobi", Saad [22]),
+ * in the order and notation of DESIGN.md R3 / SURVEY.md 8(c) C3.
+ *   b_phys : physical right-hand side (b_s = V.b is formed here)
+ *   x      : in = x0, out = last iterate
+ *   hist   : NULL or >= maxit+1 doubles; hist[k] = ||r_k||_2 / ||b_s||_2
+ * returns REF_OK / REF_MAXIT / negative error; *iters = k.
+ */
+int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, int maxit,
+                int *iters, double *hist)
+{
+    if (!op || !b_phys || !x || !iters || rtol < 0.0 || maxit < 0) return REF_EINVAL;
+    const size_t n = (size_t)op->nr * op->nt * op->np;
+    double *d = (double *)malloc(n * sizeof(double)), *r = (double *)malloc(n * sizeof(double));
+    double *z = (double *)malloc(n * sizeof(double)), *p = (double *)malloc(n * sizeof(double));
+    double *q = (double *)malloc(n * sizeof(double));
+    int status = REF_ENOMEM, k = 0;
+    if (!d || !r || !z || !p || !q) goto done;
+
+    mas_ref_diag(op, d);
+    mas_ref_volume(op, z);                       /* z used as scratch for V */
+    for (size_t c = 0; c < n; c++) r[c] = z[c] * b_phys[c];     /* b_s = V.b */
+    const double bb = dot(n, r, r);
+    if (bb == 0.0) {                             /* zero right-hand side: x = 0 */
+        memset(x, 0, n * sizeof(double));
+        if (hist) hist[0] = 0.0;
+        *iters = 0; status = REF_OK; goto done;
+    }
+    mas_ref_apply(op, x, q);
+    for (size_t c = 0; c < n; c++) r[c] -= q[c];                /* r = b_s - A x0 */
+    for (size_t c = 0; c < n; c++) z[c] = r[c] / d[c];
+    memcpy(p, z, n * sizeof(double));
+    double rho = dot(n, r, z), rr = dot(n, r, r);
+    double h = sqrt(rr / bb);
+    if (hist) hist[0] = h;
+    status = REF_OK;
+    while (k < maxit && h > rtol && rho != 0.0) {
+        mas_ref_apply(op, p, q);
+        const double sigma = dot(n, p, q);
+        if (!(sigma > 0.0) || !isfinite(sigma)) { status = REF_EBREAKDOWN; break; }
+        const double alpha = rho / sigma;
+        for (size_t c = 0; c < n; c++) x[c] += alpha * p[c];
+        for (size_t c = 0; c < n; c++) r[c] -= alpha * q[c];
+        for (size_t c = 0; c < n; c++) z[c] = r[c] / d[c];
+        const double rho1 = dot(n, r, z);
+        rr = dot(n, r, r);
+        k += 1;
+        h = sqrt(rr / bb);
+        if (hist) hist[k] = h;
+        const double beta = rho1 / rho;
+        rho = rho1;
+        for (size_t c = 0; c < n; c++) p[c] = z[c] + beta * p[c];
+    }
+    if (status == REF_OK) status = (h <= rtol || rho == 0.0) ? REF_OK : REF_MAXIT;
+    *iters = k;
+done:
+    free(d); free(r); free(z); free(p); free(q);
+    return status;
+}
