@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's metric on BASELINE.json's config, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c4]
+
+Metric: fp64 PCG iterations/s (and achieved HBM GB/s, % of peak) on the 256x256x512 grid
+(BASELINE.json configs[3]: stretched r mesh, nu(r), s = 1e4, RHS uniform(-1,1) seed 3, 500 fixed
+iterations).  A "step" is one whole solve: init + 500 iterations of {K1 fused matvec, K2 fused
+vector kernel} inside one CUDA-graph WHILE loop, inputs resident in HBM.  `e2e` is the same solve
+through mas_pcg_solve_host with pinned HOST buffers (H2D of b and x0, D2H of x inside the timed
+region).  N > 1: replicas only (the path does not shard), one independent
+solve per rank, value = all ranks' iterations / max-over-ranks time.
+
+--impl reference times the ORACLE (oracle/mas_pcg_ref.c, as it stands, one host thread) on a
+bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64_pcg_iterations_per_s_256x256x512"
+UNIT = "iterations/s"
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+REF_ITERS_PER_STEP = 4             # oracle iterations per step of --impl reference (bounded sample)
+CPU_BASELINE_ITERS = 12            # oracle iterations timed for cpu_baseline (about 10-30 s)
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--variant", type=int, default=None)
+    ap.add_argument("--tile", type=int, default=None)
+    ap.add_argument("--loop-mode", type=int, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload(name, rank=0):
+    """(problem, dt, b, rtol, maxit, description).  Seeds are offset by the rank for replicas."""
+    from mas_inputs import configs
+    import numpy as np
+    prob = configs.make(name)
+    prob.seed += 1000 * rank
+    s = prob.stiffness[-1]
+    dt = prob.dt_for(s)
+    if name in ("c1", "c4"):
+        b = configs.rhs_uniform(prob)
+    elif name == "c2":
+        b = configs.field_manufactured(prob)      # used as a right-hand side here (bench only)
+    else:
+        b = configs.rhs_blob(prob)
+    nr, nt, np_ = prob.mesh.shape
+    rtol, maxit = (0.0, 500) if name == "c4" else (prob.rtol, prob.maxit)
+    desc = (f"{name}: {nr}x{nt}x{np_} fp64, stiffness s={s:g}, rtol={rtol:g}, maxit={maxit}, "
+            f"{'500 fixed PCG iterations' if name == 'c4' else 'solve to rtol'}")
+    return prob, dt, np.ascontiguousarray(b), rtol, maxit, desc
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.th.join(timeout=2)
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(kernel_key):
+    """Per-launch DRAM bytes of the dominant kernel from the committed ncu --set full summary."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
+            return json.load(f).get(kernel_key)
+    except Exception:
+        return None
+
+
+def time_oracle(prob, dt, b, iters):
+    """The oracle as it stands, one host thread: seconds for `iters` PCG iterations from x0 = 0."""
+    from oracle import ref
+    op = ref.RefOperator(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)
+    t0 = time.perf_counter()
+    st, k, _, _ = op.pcg(b, None, 0.0, iters)
+    t = time.perf_counter() - t0
+    op.close()
+    return t, k
+
+
+def run_reference(args, rank, world):
+    """Base-contract reference arm = the oracle on host cores; rank 0 only."""
+    if rank != 0:
+        return
+    prob, dt, b, rtol, maxit, desc = workload(args.workload)
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(prob, dt, b, 1)
+    t_total, its = 0.0, 0
+    for _ in range(args.steps):
+        t, k = time_oracle(prob, dt, b, REF_ITERS_PER_STEP)
+        t_total += t
+        its += k
+    value = its / t_total
+    sample = (f"{args.steps} steps x {REF_ITERS_PER_STEP} PCG iterations from x0=0 (operator setup and "
+              f"initial residual included), single thread, gcc -O2")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": desc, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1811_02605_b200 import MasPcg
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    prob, dt, b_np, rtol, maxit, desc = workload(args.workload, rank)
+    n = prob.mesh.ncells
+    gpu = MasPcg(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)
+    if args.variant is not None:
+        gpu.set_option("variant", args.variant)
+    if args.tile is not None:
+        gpu.set_option("tile", args.tile)
+    if args.loop_mode is not None:
+        gpu.set_option("loop_mode", args.loop_mode)
+    b_host = torch.from_numpy(b_np).pin_memory()
+    x_host = torch.zeros(prob.mesh.shape, dtype=torch.float64).pin_memory()
+    b = b_host.cuda()
+    x = torch.zeros_like(b)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        x.zero_()                                   # x0 = 0 (a 268 MB memset, outside the solver's kernels)
+        return gpu.solve(b, x, rtol, maxit, want_hist=False)
+
+    # ---------------- device-resident timing (value) ----------------
+    for _ in range(max(args.warmup, 3)):
+        st, k, _ = step()
+    barrier()
+    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else 0)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    iters_done, launches = 0, 0
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        st, k, _ = step()
+        iters_done += k
+        s = gpu.stats()
+        launches += s["loop_launches"] + s["other_launches"]
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    stats = gpu.stats()
+
+    # ---------------- end to end through the C ABI with host buffers ----------------
+    gpu.solve_host(b_host, x_host.zero_(), rtol, maxit, want_hist=False)          # warm (allocates staging)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_iters = 0
+    for _ in range(args.steps):
+        x_host.zero_()
+        st2, k2, _ = gpu.solve_host(b_host, x_host, rtol, maxit, want_hist=False)
+        e2e_iters += k2
+    barrier()
+    e2e_s = time.perf_counter() - t0
+
+    # ---------------- per-kernel durations (CUDA events around each launch) ----------------
+    x.zero_()
+    prof = gpu.profile(b, x, 40)
+    barrier()
+
+    t_all = torch.tensor([ms, e2e_s * 1e3, float(iters_done), float(e2e_iters), float(launches)],
+                         dtype=torch.float64, device="cuda")
+    if world > 1:
+        tmax = t_all.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t_all.clone()
+        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms, e2e_ms = float(tmax[0]), float(tmax[1])
+        iters_all, e2e_iters_all, launches_all = float(tsum[2]), float(tsum[3]), float(tsum[4])
+    else:
+        e2e_ms, iters_all, e2e_iters_all, launches_all = e2e_s * 1e3, float(iters_done), float(e2e_iters), float(launches)
+
+    if rank == 0:
+        value = iters_all / (ms * 1e-3)
+        bpc = stats["bytes_per_cell_iter"]
+        peak, peak_src = hbm_peak()
+        k1_bytes, k2_bytes = 4 * 8 * n, 6 * 8 * n         # K1: r,p -> p,q ; K2: x,p,r,q -> x,r
+        k1_gbs = k1_bytes / (prof["k1_ms"] * 1e-3) / 1e9
+        k2_gbs = k2_bytes / (prof["k2_ms"] * 1e-3) / 1e9
+        dom = "k1_fused_matvec" if prof["k1_ms"] >= prof["k2_ms"] else "k2_fused_vector"
+        dom_gbs = k1_gbs if dom.startswith("k1") else k2_gbs
+        it_ms = ms / (iters_all / world) if iters_all else float("nan")
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                       "l2": "inputs larger than L2 (5 live vectors x %.0f MB vs 126 MB)" % (8 * n / 1e6),
+                       "loop_mode": "cuda-graph while" if stats["loop_mode"] == 1 else "host chunks",
+                       "bytes_per_cell_iter": bpc, "status": st, "iters_per_step": k},
+            "clocks": clocks,
+            "e2e": {"value": e2e_iters_all / (e2e_ms * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": 2 * 8 * n, "d2h_bytes_per_step": 8 * n},
+            "gpu_launches": int(launches_all),
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": dom_gbs, "peak": peak, "unit": "GB/s",
+                         "frac": dom_gbs / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
+                         "frac_of_nominal_8000": dom_gbs / 8000.0},
+            "kernels": {"k1_fused_matvec": {"ms": prof["k1_ms"], "min_ms": prof["k1_min_ms"],
+                                            "alg_bytes": k1_bytes, "gbs": k1_gbs},
+                        "k2_fused_vector": {"ms": prof["k2_ms"], "min_ms": prof["k2_min_ms"],
+                                            "alg_bytes": k2_bytes, "gbs": k2_gbs}},
+            "iteration": {"ms": it_ms, "model_gbs": bpc * n / (it_ms * 1e-3) / 1e9,
+                          "frac_of_peak": bpc * n / (it_ms * 1e-3) / 1e9 / peak,
+                          "frac_of_nominal_8000": bpc * n / (it_ms * 1e-3) / 1e9 / 8000.0},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            nit = CPU_BASELINE_ITERS if args.workload in ("c4", "c5") else 40
+            t_a, _ = time_oracle(prob, dt, b_np, 2)
+            t_b, _ = time_oracle(prob, dt, b_np, 2 + nit)
+            line["cpu_baseline"] = {
+                "value": nit / max(t_b - t_a, 1e-9), "unit": UNIT, "cores": 1, "kind": "oracle",
+                "sample": f"{nit} steady-state PCG iterations of the same workload (time of {2 + nit} "
+                          f"iterations minus time of 2), one thread of {os.cpu_count()} host cores, gcc -O2"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,137 @@
+// common.cuh -- device-side types and the deterministic two-stage reduction shared by every kernel
+// of the MAS PCG path (sm_100a).  Product code; shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mas {
+
+// Operator as the kernels see it: 2-D (r,theta) coefficient planes + 1-D phi factors, built once
+// from the 1-D metric arrays (PAPER.md:65 non-uniform logically
+// rectangular mesh).  "row" = i*nt + j indexes a phi-row of np cells and every [nr][nt] plane.
+struct OpDev {
+    int nr, nt, np, nv;          // nv = np/2 (double2 vectors per row)
+    int nrows;                   // nr*nt
+    int uniform_phi;             // 1: dph_c, dph_f constant  => Dinv plane is valid
+    long long n;                 // cells
+    // dt-scaled planes, rewritten by set_dt
+    const double *E;             // [nrows]      V2 + dt*(CRf[i]+CRf[i+1]+CT[j]+CT[j+1])   (diag, per unit vp)
+    const double *F;             // [nrows]      dt*CP                                      (phi coupling)
+    const double *AR;            // [(nr+1)*nt]  dt*CR, zero on both radial boundary faces  (off-diagonal)
+    const double *AT;            // [nr*(nt+1)]  dt*CT, zero on both polar faces
+    const double *Dinv;          // [nrows]      1/(vp*E + F*wp) when uniform_phi
+    // dt-independent
+    const double *V2;            // [nrows]      r_c^2 dr_c sin_c dth_c
+    const double *vp;            // [np] dph_c
+    const double *wp;            // [np] ip[k] + ip[k-1]
+    const double *ip;            // [np] 1/dph_f[k]   (face k+1/2)
+};
+
+// Per-solve arguments, written by the host before the graph launch; kernels read them through a
+// device pointer so that one instantiated CUDA graph serves every solve.
+struct SolveArgs {
+    const double *b;
+    double *x;
+    double rtol;
+    int maxit;
+    int pad;
+};
+
+// Iteration scalars; live on the device for the whole loop (the host never sees them per
+// iteration -- contrast PAPER.md:134-143 where each OpenACC reduction returns to the host).
+struct State {
+    double rho, sigma, alpha, beta, bb, rr;
+    int k;                       // iterations done
+    int active;                  // 1 while the loop should continue
+    int status;                  // MAS_OK / MAS_MAXIT / MAS_EBREAKDOWN
+    int launches;                // loop kernels that actually did work (for mas_pcg_stats)
+    unsigned ticket[4];          // last-block-done counters, one per kernel role
+};
+
+struct Work {                    // handle-owned vectors
+    double *r, *p0, *p1, *q;     // p ping-pongs: iteration k reads p[k&1], writes p[(k+1)&1]
+    double *partials;            // [4][MAX_PARTIALS]
+    double *hist;                // [hist_cap]
+    State *st;
+    const SolveArgs *args;
+};
+
+constexpr int MAX_PARTIALS = 8192;   // upper bound on gridDim.x of any reducing kernel
+constexpr int ST_OK = 0, ST_MAXIT = 1, ST_BREAKDOWN = -4;
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;   // xor butterfly: every lane performs the same commutative pair sums => same bits
+}
+
+// Fixed-shape block sum (warp butterflies, then warp 0 over the per-warp values).  Result valid
+// in thread 0.  `sh` = >= 32 doubles of shared memory.  Deterministic: no atomics on data.
+template <int NT>
+__device__ __forceinline__ double block_sum(double v, double *sh)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    v = warp_sum(v);
+    if (lane == 0) sh[w] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (w == 0) {
+        t = lane < (NT + 31) / 32 ? sh[lane] : 0.0;
+        t = warp_sum(t);
+    }
+    __syncthreads();
+    return t;
+}
+
+// Stage 2: every block stores its NP partial sums at a FIXED slot
+// (its blockIdx), then the block that arrives last sums all slots in a FIXED order.  Which
+// block is last varies from run to run; the summation order does not => bit-reproducible.
+// Returns true in ALL threads of the last block; totals valid in thread 0 only.
+template <int NT, int NP>
+__device__ __forceinline__ bool grid_sum(double (&v)[NP], double *partials, unsigned *ticket, double *sh)
+{
+    __shared__ int s_last;
+    const int G = gridDim.x;
+#pragma unroll
+    for (int q = 0; q < NP; q++) {
+        double t = block_sum<NT>(v[q], sh);
+        if (threadIdx.x == 0) partials[q * MAX_PARTIALS + blockIdx.x] = t;
+    }
+    if (threadIdx.x == 0) {
+        __threadfence();
+        unsigned t = atomicAdd(ticket, 1u);
+        s_last = (t == (unsigned)(G - 1));
+    }
+    __syncthreads();
+    if (!s_last) return false;
+    __threadfence();
+#pragma unroll
+    for (int q = 0; q < NP; q++) {
+        double a = 0.0;
+        for (int i = threadIdx.x; i < G; i += NT) a += __ldcg(&partials[q * MAX_PARTIALS + i]);
+        v[q] = block_sum<NT>(a, sh);
+    }
+    if (threadIdx.x == 0) *ticket = 0u;     // re-arm for the next launch
+    return true;
+}
+
+// Thread -> (row, vector) mapping without per-element division: a block of NT threads covers
+// RB = NT/nvc rows of nvc = min(nv, NT) vectors at a time; longer rows are walked in steps of nvc.
+struct RowMap {
+    int rl, kv0, nvc, rb;
+    bool idle;
+};
+template <int NT>
+__device__ __forceinline__ RowMap row_map(int nv)
+{
+    RowMap m;
+    m.nvc = nv < NT ? nv : NT;
+    m.rb = NT / m.nvc;
+    m.rl = threadIdx.x / m.nvc;
+    m.kv0 = threadIdx.x - m.rl * m.nvc;
+    m.idle = m.rl >= m.rb;
+    return m;
+}
+
+}  // namespace mas

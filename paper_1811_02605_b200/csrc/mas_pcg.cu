@@ -1,0 +1,613 @@
+// mas_pcg.cu -- C ABI (include/mas_pcg.h) of the B200-native MAS PCG path: handle, coefficient
+// planes, workspaces, the CUDA-graph WHILE loop and its host-chunk fallback.  Every step of the
+// numerical path runs in the kernels of kernels_base.cuh / kernels_march.cuh; this file only
+// marshals.  There is no CPU fallback.
+#include "../../include/mas_pcg.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "kernels_base.cuh"
+#include "kernels_march.cuh"
+
+using namespace mas;
+
+namespace {
+
+constexpr int NT_BASE = 256;
+constexpr int HOST_CHUNK = 16;       // iterations per poll in host-chunk mode
+
+struct KLaunch {                     // one kernel launch, usable directly or as a graph node
+    const void *func = nullptr;
+    dim3 grid{1, 1, 1}, block{1, 1, 1};
+    size_t smem = 0;
+    void *args[12] = {};
+    int nargs = 0;
+};
+
+template <typename T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t n = 0;
+    cudaError_t alloc(size_t count)
+    {
+        release();
+        n = count;
+        return cudaMalloc((void **)&p, (count ? count : 1) * sizeof(T));
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        n = 0;
+    }
+};
+
+}  // namespace
+
+struct mas_pcg {
+    int nr = 0, nt = 0, np = 0;
+    size_t n = 0;
+    int device = 0, num_sms = 0;
+    double dt = 0.0;
+    int uniform_phi = 0;
+    // device planes
+    DevBuf<double> V2, SD, CP, CRoff, CT, E, F, AR, AT, Dinv, vp, wp, ip;
+    double vp0 = 0, wp0 = 0;
+    // workspaces
+    DevBuf<double> r, p0, p1, q, partials, hist, bdev, xdev;
+    DevBuf<State> st;
+    DevBuf<SolveArgs> args;
+    // pinned staging
+    SolveArgs *h_args = nullptr;
+    State *h_st = nullptr;
+    double *h_hist = nullptr;
+    size_t hist_cap = 0;
+    // loop
+    int loop_mode = 1;               // requested: 1 graph-while, 0 host chunks
+    int loop_mode_used = 1;
+    int variant = 1;                 // K1 variant (0 = baseline, 1 = 2.5-D marching tiles)
+    int tile = 0;                    // marching tile configuration id
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    bool graph_dirty = true;
+    long long stats[8] = {};
+    OpDev op{};
+    Work work{};
+};
+
+namespace {
+
+int fail(mas_pcg *h, int code)
+{
+    mas_pcg_destroy(h);
+    return code;
+}
+
+#define CK(call)                                   \
+    do {                                           \
+        if ((call) != cudaSuccess) {               \
+            cudaGetLastError();                    \
+            return MAS_ECUDA;                      \
+        }                                          \
+    } while (0)
+
+double nu_at(const mas_nu_t *nu, int nt, int i, int j) { return nu->kind == 0 ? nu->v[0] : nu->v[(size_t)i * nt + j]; }
+
+bool positive(const double *a, int lo, int hi)
+{
+    for (int i = lo; i < hi; i++)
+        if (!(a[i] > 0.0) || !isfinite(a[i])) return false;
+    return true;
+}
+
+int upload(DevBuf<double> &d, const std::vector<double> &h)
+{
+    if (d.alloc(h.size()) != cudaSuccess) return MAS_ENOMEM;
+    CK(cudaMemcpy(d.p, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice));
+    return MAS_OK;
+}
+
+void fill_op(mas_pcg *h)
+{
+    OpDev &o = h->op;
+    o.nr = h->nr; o.nt = h->nt; o.np = h->np; o.nv = h->np / 2;
+    o.nrows = h->nr * h->nt;
+    o.uniform_phi = h->uniform_phi;
+    o.n = (long long)h->n;
+    o.E = h->E.p; o.F = h->F.p; o.AR = h->AR.p; o.AT = h->AT.p; o.Dinv = h->Dinv.p;
+    o.V2 = h->V2.p; o.vp = h->vp.p; o.wp = h->wp.p; o.ip = h->ip.p;
+    Work &w = h->work;
+    w.r = h->r.p; w.p0 = h->p0.p; w.p1 = h->p1.p; w.q = h->q.p;
+    w.partials = h->partials.p; w.hist = h->hist.p; w.st = h->st.p; w.args = h->args.p;
+}
+
+int scale_planes(mas_pcg *h, double dt, cudaStream_t s)
+{
+    PlaneSet ps;
+    ps.V2 = h->V2.p; ps.SD = h->SD.p; ps.CP = h->CP.p; ps.CRoff = h->CRoff.p; ps.CT = h->CT.p;
+    ps.E = h->E.p; ps.F = h->F.p; ps.AR = h->AR.p; ps.AT = h->AT.p; ps.Dinv = h->Dinv.p;
+    ps.nr = h->nr; ps.nt = h->nt; ps.vp0 = h->vp0; ps.wp0 = h->wp0;
+    const int total = (h->nr + 1) * (h->nt + 1);
+    k_scale_planes<<<(total + 255) / 256, 256, 0, s>>>(ps, dt);
+    CK(cudaGetLastError());
+    h->dt = dt;
+    return MAS_OK;
+}
+
+}  // namespace
+
+extern "C" const char *mas_pcg_strerror(int status)
+{
+    switch (status) {
+        case MAS_OK: return "converged";
+        case MAS_MAXIT: return "iteration cap reached before rtol";
+        case MAS_EINVAL: return "invalid argument";
+        case MAS_ENOMEM: return "out of memory";
+        case MAS_ECUDA: return "CUDA runtime error (no device, or a launch failed)";
+        case MAS_EBREAKDOWN: return "PCG breakdown: p.Ap <= 0 or non-finite";
+        default: return "unknown status";
+    }
+}
+
+extern "C" void mas_pcg_destroy(mas_pcg_t *h)
+{
+    if (!h) return;
+    if (h->exec) cudaGraphExecDestroy(h->exec);
+    if (h->graph) cudaGraphDestroy(h->graph);
+    DevBuf<double> *bufs[] = {&h->V2, &h->SD, &h->CP, &h->CRoff, &h->CT, &h->E, &h->F, &h->AR, &h->AT, &h->Dinv,
+                              &h->vp, &h->wp, &h->ip, &h->r, &h->p0, &h->p1, &h->q, &h->partials, &h->hist,
+                              &h->bdev, &h->xdev};
+    for (DevBuf<double> *b : bufs) b->release();
+    h->st.release();
+    h->args.release();
+    if (h->h_args) cudaFreeHost(h->h_args);
+    if (h->h_st) cudaFreeHost(h->h_st);
+    if (h->h_hist) cudaFreeHost(h->h_hist);
+    cudaGetLastError();
+    delete h;
+}
+
+extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double dt, const mas_nu_t *nu,
+                              const mas_bc_t *bc, mas_pcg_t **out)
+{
+    if (out) *out = nullptr;
+    if (!g || !m || !nu || !bc || !out) return MAS_EINVAL;
+    const int nr = g->nr, nt = g->nt, np = g->np;
+    if (nr < 1 || nt < 1 || np < 2 || (np & 1)) return MAS_EINVAL;
+    if ((long long)nr * nt * np >= (1LL << 31)) return MAS_EINVAL;          // 32-bit cell indices per row map
+    if (!(dt >= 0.0) || !isfinite(dt)) return MAS_EINVAL;
+    if (!m->r_c || !m->dr_c || !m->r_f || !m->dr_f || !m->sin_c || !m->dth_c || !m->sin_f || !m->dth_f ||
+        !m->dph_c || !m->dph_f || !nu->v)
+        return MAS_EINVAL;
+    if ((bc->r_inner != MAS_BC_DIRICHLET && bc->r_inner != MAS_BC_NEUMANN) ||
+        (bc->r_outer != MAS_BC_DIRICHLET && bc->r_outer != MAS_BC_NEUMANN))
+        return MAS_EINVAL;
+    if (nu->kind != 0 && nu->kind != 1) return MAS_EINVAL;
+    if (!positive(m->r_c, 0, nr) || !positive(m->dr_c, 0, nr) || !positive(m->r_f, 0, nr + 1) ||
+        !positive(m->dr_f, 0, nr + 1) || !positive(m->sin_c, 0, nt) || !positive(m->dth_c, 0, nt) ||
+        !positive(m->dth_f, 1, nt) || !positive(m->sin_f, 1, nt) || !positive(m->dph_c, 0, np) ||
+        !positive(m->dph_f, 0, np))
+        return MAS_EINVAL;
+    for (int i = 0; i < nr; i++)
+        if (!(m->r_f[i] < m->r_f[i + 1])) return MAS_EINVAL;               // monotone mesh
+    if (!positive(nu->v, 0, nu->kind == 0 ? 1 : nr * nt)) return MAS_EINVAL;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return MAS_ECUDA;                                                  // no CPU fallback
+    }
+    mas_pcg *h = new (std::nothrow) mas_pcg();
+    if (!h) return MAS_ENOMEM;
+    h->nr = nr; h->nt = nt; h->np = np;
+    h->n = (size_t)nr * nt * np;
+    if (cudaGetDevice(&h->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess)
+        return fail(h, MAS_ECUDA);
+
+    // ---- coefficient planes (R1; the paper prints no discrete operator) ----
+    const int nrows = nr * nt;
+    std::vector<double> V2(nrows), CP(nrows), SD(nrows), CRf((size_t)(nr + 1) * nt), CRoff((size_t)(nr + 1) * nt),
+        CT((size_t)nr * (nt + 1)), vp(np), ip(np), wp(np);
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j < nt; j++) {
+            const double area_rt = m->sin_c[j] * m->dth_c[j];
+            V2[i * nt + j] = m->r_c[i] * m->r_c[i] * m->dr_c[i] * area_rt;
+            CP[i * nt + j] = nu_at(nu, nt, i, j) * m->dr_c[i] * m->dth_c[j] / m->sin_c[j];
+        }
+    for (int i = 0; i <= nr; i++)
+        for (int j = 0; j < nt; j++) {
+            const int il = i > 0 ? i - 1 : 0, ih = i < nr ? i : nr - 1;
+            const double nuf = 0.5 * (nu_at(nu, nt, il, j) + nu_at(nu, nt, ih, j));
+            double c = nuf * (m->r_f[i] * m->r_f[i]) * (m->sin_c[j] * m->dth_c[j]) / m->dr_f[i];
+            const bool boundary = (i == 0 || i == nr);
+            if (i == 0 && bc->r_inner == MAS_BC_NEUMANN) c = 0.0;
+            if (i == nr && bc->r_outer == MAS_BC_NEUMANN) c = 0.0;
+            CRf[(size_t)i * nt + j] = c;                        // enters the diagonal (Dirichlet face)
+            CRoff[(size_t)i * nt + j] = boundary ? 0.0 : c;     // no off-diagonal partner on a boundary
+        }
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j <= nt; j++) {
+            double c = 0.0;                                     // polar faces: zero area
+            if (j > 0 && j < nt)
+                c = 0.5 * (nu_at(nu, nt, i, j - 1) + nu_at(nu, nt, i, j)) * m->dr_c[i] * m->sin_f[j] / m->dth_f[j];
+            CT[(size_t)i * (nt + 1) + j] = c;
+        }
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j < nt; j++)
+            SD[i * nt + j] = CRf[(size_t)i * nt + j] + CRf[(size_t)(i + 1) * nt + j] + CT[(size_t)i * (nt + 1) + j] +
+                             CT[(size_t)i * (nt + 1) + j + 1];
+    h->uniform_phi = 1;
+    for (int k = 0; k < np; k++) {
+        vp[k] = m->dph_c[k];
+        ip[k] = 1.0 / m->dph_f[k];
+        if (m->dph_c[k] != m->dph_c[0] || m->dph_f[k] != m->dph_f[0]) h->uniform_phi = 0;
+    }
+    for (int k = 0; k < np; k++) wp[k] = ip[k] + ip[(k + np - 1) % np];
+    h->vp0 = vp[0];
+    h->wp0 = wp[0];
+
+    int rc;
+    if ((rc = upload(h->V2, V2)) || (rc = upload(h->CP, CP)) || (rc = upload(h->SD, SD)) ||
+        (rc = upload(h->CRoff, CRoff)) || (rc = upload(h->CT, CT)) || (rc = upload(h->vp, vp)) ||
+        (rc = upload(h->wp, wp)) || (rc = upload(h->ip, ip)))
+        return fail(h, rc);
+    if (h->E.alloc(nrows) || h->F.alloc(nrows) || h->Dinv.alloc(nrows) || h->AR.alloc((size_t)(nr + 1) * nt) ||
+        h->AT.alloc((size_t)nr * (nt + 1)) || h->r.alloc(h->n) || h->p0.alloc(h->n) || h->p1.alloc(h->n) ||
+        h->q.alloc(h->n) || h->partials.alloc(4 * (size_t)MAX_PARTIALS) || h->st.alloc(1) || h->args.alloc(1)) {
+        cudaGetLastError();
+        return fail(h, MAS_ENOMEM);
+    }
+    h->hist_cap = 1 << 13;
+    if (h->hist.alloc(h->hist_cap) != cudaSuccess) return fail(h, MAS_ENOMEM);
+    if (cudaMallocHost((void **)&h->h_args, sizeof(SolveArgs)) != cudaSuccess ||
+        cudaMallocHost((void **)&h->h_st, sizeof(State)) != cudaSuccess ||
+        cudaMallocHost((void **)&h->h_hist, h->hist_cap * sizeof(double)) != cudaSuccess)
+        return fail(h, MAS_ENOMEM);
+    if (cudaMemset(h->st.p, 0, sizeof(State)) != cudaSuccess) return fail(h, MAS_ECUDA);
+    if (cudaMemset(h->p0.p, 0, h->n * sizeof(double)) != cudaSuccess ||
+        cudaMemset(h->p1.p, 0, h->n * sizeof(double)) != cudaSuccess)
+        return fail(h, MAS_ECUDA);
+    fill_op(h);
+    if ((rc = scale_planes(h, dt, nullptr)) != MAS_OK) return fail(h, rc);
+    if (cudaDeviceSynchronize() != cudaSuccess) return fail(h, MAS_ECUDA);
+    *out = h;
+    return MAS_OK;
+}
+
+// =============================================================================================
+// launch descriptions
+// =============================================================================================
+namespace {
+
+struct LoopCtx {                     // storage that kernel argument pointers refer to
+    OpDev op;
+    Work work;
+    cudaGraphConditionalHandle cond;
+    int use_cond;
+    const double *xin;
+    const SolveArgs *args;
+    double *y;
+    MarchParams mp;
+};
+
+int base_grid(const mas_pcg *h, const void *func, int nt_block)
+{
+    const int nv = h->np / 2;
+    const int nvc = nv < nt_block ? nv : nt_block;
+    const int rb = nt_block / nvc;
+    const long long groups = ((long long)h->nr * h->nt + rb - 1) / rb;
+    int occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, func, nt_block, 0) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        occ = 1;
+    }
+    long long gsz = (long long)h->num_sms * occ;
+    if (gsz > groups) gsz = groups;
+    if (gsz > MAX_PARTIALS) gsz = MAX_PARTIALS;
+    if (gsz < 1) gsz = 1;
+    return (int)gsz;
+}
+
+KLaunch make_apply(const mas_pcg *h, LoopCtx &c)
+{
+    KLaunch k;
+    k.func = (const void *)k_apply<NT_BASE>;
+    k.block = dim3(NT_BASE);
+    k.grid = dim3(base_grid(h, k.func, NT_BASE));
+    k.args[0] = &c.op; k.args[1] = &c.xin; k.args[2] = &c.args; k.args[3] = &c.y;
+    k.nargs = 4;
+    return k;
+}
+
+KLaunch make_init(const mas_pcg *h, LoopCtx &c)
+{
+    KLaunch k;
+    k.func = h->uniform_phi ? (const void *)k_init<NT_BASE, true> : (const void *)k_init<NT_BASE, false>;
+    k.block = dim3(NT_BASE);
+    k.grid = dim3(base_grid(h, k.func, NT_BASE));
+    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
+    k.nargs = 4;
+    return k;
+}
+
+KLaunch make_k2(const mas_pcg *h, LoopCtx &c)
+{
+    KLaunch k;
+    k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true> : (const void *)k2_vec<NT_BASE, false>;
+    k.block = dim3(NT_BASE);
+    k.grid = dim3(base_grid(h, k.func, NT_BASE));
+    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
+    k.nargs = 4;
+    return k;
+}
+
+KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
+{
+    KLaunch k;
+    if (h->variant == 0) {
+        k.func = h->uniform_phi ? (const void *)k1_v0<NT_BASE, true> : (const void *)k1_v0<NT_BASE, false>;
+        k.block = dim3(NT_BASE);
+        k.grid = dim3(base_grid(h, k.func, NT_BASE));
+        k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
+        k.nargs = 4;
+        return k;
+    }
+    march_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, &c.mp, &k.func, &k.grid, &k.block,
+                    &k.smem);
+    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.mp; k.args[3] = &c.cond; k.args[4] = &c.use_cond;
+    k.nargs = 5;
+    return k;
+}
+
+cudaError_t launch(const KLaunch &k, cudaStream_t s)
+{
+    return cudaLaunchKernel(k.func, k.grid, k.block, const_cast<void **>(k.args), k.smem, s);
+}
+
+cudaError_t add_node(cudaGraphNode_t *node, cudaGraph_t g, const cudaGraphNode_t *dep, const KLaunch &k)
+{
+    cudaKernelNodeParams p;
+    memset(&p, 0, sizeof(p));
+    p.func = const_cast<void *>(k.func);
+    p.gridDim = k.grid;
+    p.blockDim = k.block;
+    p.sharedMemBytes = (unsigned)k.smem;
+    p.kernelParams = const_cast<void **>(k.args);
+    p.extra = nullptr;
+    return cudaGraphAddKernelNode(node, g, dep, dep ? 1 : 0, &p);
+}
+
+void drop_graph(mas_pcg *h)
+{
+    if (h->exec) cudaGraphExecDestroy(h->exec);
+    if (h->graph) cudaGraphDestroy(h->graph);
+    h->exec = nullptr;
+    h->graph = nullptr;
+    h->graph_dirty = true;
+}
+
+// graph = [A x0 -> q] -> [init] -> WHILE(cond){ K1 -> K2 }   (call stack 2)
+int build_graph(mas_pcg *h)
+{
+    drop_graph(h);
+    LoopCtx c;
+    c.op = h->op; c.work = h->work; c.use_cond = 1; c.xin = nullptr; c.args = h->args.p; c.y = h->q.p;
+    cudaGraph_t g = nullptr;
+    if (cudaGraphCreate(&g, 0) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+    h->graph = g;
+    if (cudaGraphConditionalHandleCreate(&c.cond, g, 1, cudaGraphCondAssignDefault) != cudaSuccess) {
+        cudaGetLastError();
+        return MAS_ECUDA;
+    }
+    cudaGraphNode_t n_apply, n_init, n_while, n_k1, n_k2;
+    const KLaunch ka = make_apply(h, c), ki = make_init(h, c);
+    if (add_node(&n_apply, g, nullptr, ka) != cudaSuccess || add_node(&n_init, g, &n_apply, ki) != cudaSuccess) {
+        cudaGetLastError();
+        return MAS_ECUDA;
+    }
+    cudaGraphNodeParams wp = {cudaGraphNodeTypeConditional};
+    wp.conditional.handle = c.cond;
+    wp.conditional.type = cudaGraphCondTypeWhile;
+    wp.conditional.size = 1;
+    if (cudaGraphAddNode(&n_while, g, &n_init, 1, &wp) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+    cudaGraph_t body = wp.conditional.phGraph_out[0];
+    const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
+    if (add_node(&n_k1, body, nullptr, k1) != cudaSuccess || add_node(&n_k2, body, &n_k1, k2) != cudaSuccess) {
+        cudaGetLastError();
+        return MAS_ECUDA;
+    }
+    if (cudaGraphInstantiate(&h->exec, g, 0) != cudaSuccess) {
+        cudaGetLastError();
+        h->exec = nullptr;
+        return MAS_ECUDA;
+    }
+    h->graph_dirty = false;
+    return MAS_OK;
+}
+
+int ensure_hist(mas_pcg *h, int maxit)
+{
+    const size_t need = (size_t)maxit + 1;
+    if (need <= h->hist_cap) return MAS_OK;
+    size_t cap = h->hist_cap;
+    while (cap < need) cap *= 2;
+    if (h->hist.alloc(cap) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    if (h->h_hist) cudaFreeHost(h->h_hist);
+    h->h_hist = nullptr;
+    if (cudaMallocHost((void **)&h->h_hist, cap * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    h->hist_cap = cap;
+    fill_op(h);
+    drop_graph(h);              // kernel nodes hold the old hist pointer
+    return MAS_OK;
+}
+
+bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
+
+}  // namespace
+
+extern "C" int mas_pcg_set_dt(mas_pcg_t *h, double dt, void *stream)
+{
+    if (!h || !(dt >= 0.0) || !isfinite(dt)) return MAS_EINVAL;
+    return scale_planes(h, dt, (cudaStream_t)stream);
+}
+
+extern "C" int mas_pcg_apply(mas_pcg_t *h, const double *x_dev, double *y_dev, void *stream)
+{
+    if (!h || !x_dev || !y_dev || x_dev == y_dev || !aligned16(x_dev) || !aligned16(y_dev)) return MAS_EINVAL;
+    LoopCtx c;
+    c.op = h->op; c.xin = x_dev; c.args = h->args.p; c.y = y_dev;
+    CK(launch(make_apply(h, c), (cudaStream_t)stream));
+    return MAS_OK;
+}
+
+extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
+{
+    if (!h || !name) return MAS_EINVAL;
+    if (!strcmp(name, "loop_mode")) {
+        if (value != 0 && value != 1) return MAS_EINVAL;
+        h->loop_mode = value;
+    } else if (!strcmp(name, "variant")) {
+        if (value < 0 || value > 1) return MAS_EINVAL;
+        h->variant = value;
+    } else if (!strcmp(name, "tile")) {
+        if (value < 0 || value >= march_num_tiles()) return MAS_EINVAL;
+        h->tile = value;
+    } else {
+        return MAS_EINVAL;
+    }
+    h->graph_dirty = true;
+    return MAS_OK;
+}
+
+extern "C" int mas_pcg_stats(const mas_pcg_t *h, long long *out)
+{
+    if (!h || !out) return MAS_EINVAL;
+    memcpy(out, h->stats, sizeof(h->stats));
+    return MAS_OK;
+}
+
+extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, double rtol, int maxit, void *stream,
+                             int *iters_out, double *reshist_host)
+{
+    if (!h || !b_dev || !x_dev || b_dev == x_dev || !(rtol >= 0.0) || maxit < 0 || !aligned16(b_dev) ||
+        !aligned16(x_dev))
+        return MAS_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    int rc = ensure_hist(h, maxit);
+    if (rc != MAS_OK) return rc;
+
+    h->h_args->b = b_dev; h->h_args->x = x_dev; h->h_args->rtol = rtol; h->h_args->maxit = maxit; h->h_args->pad = 0;
+    CK(cudaMemcpyAsync(h->args.p, h->h_args, sizeof(SolveArgs), cudaMemcpyHostToDevice, s));
+
+    int mode = h->loop_mode;
+    if (mode == 1 && (h->graph_dirty || !h->exec)) {
+        if (build_graph(h) != MAS_OK) {       // driver without conditional nodes: fall back, and say so in stats
+            drop_graph(h);
+            mode = 0;
+        }
+    }
+    long long launched_outside = 2, launched_loop = 0;
+    if (mode == 1) {
+        CK(cudaGraphLaunch(h->exec, s));
+    } else {
+        LoopCtx c;
+        c.op = h->op; c.work = h->work; c.use_cond = 0; c.xin = nullptr; c.args = h->args.p; c.y = h->q.p;
+        memset(&c.cond, 0, sizeof(c.cond));
+        CK(launch(make_apply(h, c), s));
+        CK(launch(make_init(h, c), s));
+        const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
+        for (int done = 0; done < maxit;) {
+            CK(cudaMemcpyAsync(h->h_st, h->st.p, sizeof(State), cudaMemcpyDeviceToHost, s));
+            CK(cudaStreamSynchronize(s));
+            if (!h->h_st->active) break;
+            const int chunk = maxit - done < HOST_CHUNK ? maxit - done : HOST_CHUNK;
+            for (int it = 0; it < chunk; it++) {
+                CK(launch(k1, s));
+                CK(launch(k2, s));
+            }
+            launched_loop += 2LL * chunk;
+            done += chunk;
+        }
+    }
+    CK(cudaMemcpyAsync(h->h_st, h->st.p, sizeof(State), cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(h->h_hist, h->hist.p, ((size_t)maxit + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));          // the one host sync of a graph-mode solve
+    const State &st = *h->h_st;
+    if (st.bb == 0.0) {                    // zero right-hand side: x = 0
+        CK(cudaMemsetAsync(x_dev, 0, h->n * sizeof(double), s));
+        CK(cudaStreamSynchronize(s));
+    }
+    if (iters_out) *iters_out = st.k;
+    if (reshist_host) memcpy(reshist_host, h->h_hist, ((size_t)st.k + 1) * sizeof(double));
+    h->loop_mode_used = mode;
+    h->stats[0] = mode == 1 ? (long long)st.launches : launched_loop;
+    h->stats[1] = launched_outside;
+    h->stats[2] = mode;
+    h->stats[3] = 80;                      // K1: r,p -> p,q (4N) ; K2: x,p,r,q -> x,r (6N) ; 8 B each
+    return st.status;
+}
+
+extern "C" int mas_pcg_solve_host(mas_pcg_t *h, const double *b_host, double *x_host, double rtol, int maxit,
+                                  void *stream, int *iters_out, double *reshist_host)
+{
+    if (!h || !b_host || !x_host) return MAS_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!h->bdev.p && h->bdev.alloc(h->n) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    if (!h->xdev.p && h->xdev.alloc(h->n) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    const size_t bytes = h->n * sizeof(double);
+    CK(cudaMemcpyAsync(h->bdev.p, b_host, bytes, cudaMemcpyHostToDevice, s));
+    CK(cudaMemcpyAsync(h->xdev.p, x_host, bytes, cudaMemcpyHostToDevice, s));
+    const int rc = mas_pcg_solve(h, h->bdev.p, h->xdev.p, rtol, maxit, stream, iters_out, reshist_host);
+    if (rc < 0) return rc;
+    CK(cudaMemcpyAsync(x_host, h->xdev.p, bytes, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+    return rc;
+}
+
+extern "C" int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev, int nit, void *stream, double *ms_out)
+{
+    if (!h || !b_dev || !x_dev || b_dev == x_dev || !ms_out || nit < 1 || nit > 256 || !aligned16(b_dev) ||
+        !aligned16(x_dev))
+        return MAS_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    h->h_args->b = b_dev; h->h_args->x = x_dev; h->h_args->rtol = 0.0; h->h_args->maxit = nit; h->h_args->pad = 0;
+    int rc = ensure_hist(h, nit);
+    if (rc != MAS_OK) return rc;
+    CK(cudaMemcpyAsync(h->args.p, h->h_args, sizeof(SolveArgs), cudaMemcpyHostToDevice, s));
+    LoopCtx c;
+    c.op = h->op; c.work = h->work; c.use_cond = 0; c.xin = nullptr; c.args = h->args.p; c.y = h->q.p;
+    memset(&c.cond, 0, sizeof(c.cond));
+    std::vector<cudaEvent_t> ev(2 * (size_t)nit + 1);
+    for (cudaEvent_t &e : ev) CK(cudaEventCreate(&e));
+    CK(launch(make_apply(h, c), s));
+    CK(launch(make_init(h, c), s));
+    const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
+    CK(cudaEventRecord(ev[0], s));
+    for (int it = 0; it < nit; it++) {
+        CK(launch(k1, s));
+        CK(cudaEventRecord(ev[2 * it + 1], s));
+        CK(launch(k2, s));
+        CK(cudaEventRecord(ev[2 * it + 2], s));
+    }
+    CK(cudaStreamSynchronize(s));
+    double sum1 = 0, sum2 = 0, min1 = 1e30, min2 = 1e30;
+    for (int it = 0; it < nit; it++) {
+        float a = 0, b = 0;
+        CK(cudaEventElapsedTime(&a, ev[2 * it], ev[2 * it + 1]));
+        CK(cudaEventElapsedTime(&b, ev[2 * it + 1], ev[2 * it + 2]));
+        sum1 += a; sum2 += b;
+        if (a < min1) min1 = a;
+        if (b < min2) min2 = b;
+    }
+    for (cudaEvent_t &e : ev) cudaEventDestroy(e);
+    ms_out[0] = sum1 / nit; ms_out[1] = sum2 / nit; ms_out[2] = min1; ms_out[3] = min2;
+    return MAS_OK;
+}

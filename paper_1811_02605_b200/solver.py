@@ -1,0 +1,68 @@
+"""MasPcg: torch-tensor front end of the C ABI (argument marshalling only)."""
+from __future__ import annotations
+
+import torch
+
+from . import binding as B
+
+
+def _stream_ptr(stream=None) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _dev_ptr(t: torch.Tensor, n: int) -> int:
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n):
+        raise ValueError("need a contiguous CUDA float64 tensor with nr*nt*np elements")
+    return t.data_ptr()
+
+
+class MasPcg:
+    """One operator (mesh, nu, boundary kinds, dt) on the current CUDA device."""
+
+    def __init__(self, mesh, dt, nu_kind, nu, bc=(0, 0)):
+        if not torch.cuda.is_available():
+            raise RuntimeError("MasPcg needs a CUDA device (there is no CPU fallback)")
+        self.shape = (mesh.nr, mesh.nt, mesh.np_)
+        self.n = mesh.nr * mesh.nt * mesh.np_
+        self._h = B.mas_pcg_create(self.shape, mesh.metric_arrays(), dt, nu_kind, nu, bc)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            B.mas_pcg_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def set_dt(self, dt, stream=None):
+        B.mas_pcg_set_dt(self._h, dt, _stream_ptr(stream))
+
+    def set_option(self, name, value):
+        B.mas_pcg_set_option(self._h, name, value)
+
+    def apply(self, x: torch.Tensor, y: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+        """y = A_sym x"""
+        if y is None:
+            y = torch.empty_like(x)
+        B.mas_pcg_apply(self._h, _dev_ptr(x, self.n), _dev_ptr(y, self.n), _stream_ptr(stream))
+        return y
+
+    def solve(self, b: torch.Tensor, x: torch.Tensor, rtol: float, maxit: int, stream=None, want_hist=True):
+        """Solves A_phys x = b in place in x (x holds x0 on entry).  Returns (status, iters, hist)."""
+        return B.mas_pcg_solve(self._h, _dev_ptr(b, self.n), _dev_ptr(x, self.n), rtol, maxit,
+                               _stream_ptr(stream), want_hist)
+
+    def solve_host(self, b_host: torch.Tensor, x_host: torch.Tensor, rtol: float, maxit: int, stream=None,
+                   want_hist=True):
+        """Same with HOST (ideally pinned) float64 tensors; H2D/D2H copies happen inside the C call."""
+        for t in (b_host, x_host):
+            if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != self.n:
+                raise ValueError("need contiguous host float64 tensors with nr*nt*np elements")
+        return B.mas_pcg_solve_host(self._h, b_host.data_ptr(), x_host.data_ptr(), rtol, maxit,
+                                    _stream_ptr(stream), want_hist)
+
+    def profile(self, b: torch.Tensor, x: torch.Tensor, nit: int, stream=None):
+        return B.mas_pcg_profile(self._h, _dev_ptr(b, self.n), _dev_ptr(x, self.n), nit, _stream_ptr(stream))
+
+    def stats(self):
+        return B.mas_pcg_stats(self._h)

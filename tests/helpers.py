@@ -1,0 +1,58 @@
+"""Shared test plumbing: build the oracle operator and the CUDA operator from the same inputs,
+and the parity gates of BASELINE.json north_star (tolerances stated here, derived in DESIGN.md)."""
+from __future__ import annotations
+
+import numpy as np
+
+from mas_inputs import configs, grids
+from oracle import ref
+
+# --- the gates (BASELINE.json north_star; readings Q9, Q10 of SURVEY.md 8(c)) ---
+HIST_RTOL = 1e-10      # per-iteration relative residual: |h_gpu - h_ref| / h_ref, first 50 iterations
+HIST_ITERS = 50
+HIST_FLOOR = 1e-15     # entries at the fp64 rounding floor (h ~ eps) carry no digits: absolute slack there
+X_RTOL = 1e-9          # final x, relative L2, compared at EQUAL iteration counts
+APPLY_RTOL = 1e-13     # single matvec, relative to max |A u| (pure rounding-order difference)
+
+
+def oracle_s1(mesh, nu_kind, nu, bc=(0, 0)) -> float:
+    op = ref.RefOperator(mesh, 1.0, nu_kind, nu, bc)
+    s1 = op.stiffness_max()
+    op.close()
+    return s1
+
+
+def both_ops(mesh, dt, nu_kind, nu, bc=(0, 0)):
+    from paper_1811_02605_b200 import MasPcg
+    return ref.RefOperator(mesh, dt, nu_kind, nu, bc), MasPcg(mesh, dt, nu_kind, nu, bc)
+
+
+def general_case(nr=9, nt=11, np_=70, seed=21, s=300.0, bc=(0, 0)):
+    """Odd r/theta sizes, phi spanning a ragged second tile, non-uniform phi, nu(r, theta)."""
+    mesh = grids.wobbly_phi_mesh(grids.radial_faces_pack(nr, 4.0), nt, np_, seed)
+    rng = np.random.default_rng(seed + 1)
+    nu = 0.5 + rng.uniform(0.0, 1.0, (nr, nt))
+    dt = s / oracle_s1(mesh, 1, nu, bc)
+    return mesh, dt, 1, nu
+
+
+def check_parity(gpu, oref, b, x0, rtol, maxit, *, label=""):
+    """Runs both solvers on the same inputs and applies the three gates.  Returns (k_ref, k_gpu)."""
+    import torch
+    st_r, k_r, x_r, h_r = oref.pcg(b, x0, rtol, maxit)
+    bd = torch.from_numpy(np.ascontiguousarray(b)).cuda()
+    xd = torch.zeros_like(bd) if x0 is None else torch.from_numpy(np.ascontiguousarray(x0)).cuda()
+    st_g, k_g, h_g = gpu.solve(bd, xd, rtol, maxit)
+    assert st_g == st_r, f"{label}: status gpu {st_g} vs oracle {st_r}"
+    assert abs(k_g - k_r) <= 1, f"{label}: iterations gpu {k_g} vs oracle {k_r}"
+    m = min(HIST_ITERS, k_r, k_g) + 1
+    rel = np.maximum(np.abs(h_g[:m] - h_r[:m]) - HIST_FLOOR, 0.0) / h_r[:m]
+    assert rel.max() <= HIST_RTOL, f"{label}: history gap {rel.max():.3e} at it {rel.argmax()}"
+    if k_g != k_r:      # Q10: compare x at equal iteration counts
+        xd = torch.zeros_like(bd) if x0 is None else torch.from_numpy(np.ascontiguousarray(x0)).cuda()
+        _, k_g2, _ = gpu.solve(bd, xd, 0.0, k_r)
+        assert k_g2 == k_r
+    xg = xd.cpu().numpy().reshape(x_r.shape)
+    err = np.linalg.norm(xg - x_r) / np.linalg.norm(x_r)
+    assert err <= X_RTOL, f"{label}: x gap {err:.3e}"
+    return k_r, k_g

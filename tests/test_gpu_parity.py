@@ -1,0 +1,221 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the oracle, element by
+element, on the same seeded inputs.  Run on the B200 box:  pytest tests -m gpu"""
+import numpy as np
+import pytest
+
+from mas_inputs import configs, grids
+from oracle import ref
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+
+
+def _t(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+# ------------------------------------------------------------------ matvec alone (build step 4)
+@pytest.mark.parametrize("bc", [(0, 0), (1, 1), (0, 1)])
+@pytest.mark.parametrize("shape", [(9, 11, 70), (1, 1, 2), (3, 2, 64), (5, 17, 130)])
+def test_apply_matches_oracle_general_mesh(shape, bc):
+    mesh, dt, nu_kind, nu = H.general_case(*shape, bc=bc)
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu, bc)
+    u = np.random.default_rng(1).standard_normal(mesh.shape)
+    y_ref = oref.apply(u)
+    y = gpu.apply(_t(u)).cpu().numpy().reshape(mesh.shape)
+    assert np.abs(y - y_ref).max() <= H.APPLY_RTOL * np.abs(y_ref).max()
+
+
+def test_apply_matches_oracle_uniform_phi_config1():
+    prob = configs.make("c1")
+    oref, gpu = H.both_ops(prob.mesh, prob.dt_for(2.0), prob.nu_kind, prob.nu)
+    u = configs.rhs_uniform(prob)
+    y_ref = oref.apply(u)
+    y = gpu.apply(_t(u)).cpu().numpy().reshape(prob.mesh.shape)
+    assert np.abs(y - y_ref).max() <= H.APPLY_RTOL * np.abs(y_ref).max()
+
+
+def test_gpu_operator_symmetric_and_constant_closed_form():
+    """P3 / P5 on the GPU operator itself."""
+    import torch
+    mesh, dt, nu_kind, nu = H.general_case(12, 13, 96, bc=(1, 1))
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu, (1, 1))
+    rng = np.random.default_rng(4)
+    x, y = _t(rng.standard_normal(mesh.shape)), _t(rng.standard_normal(mesh.shape))
+    Ax, Ay = gpu.apply(x), gpu.apply(y)
+    assert abs(float(torch.vdot(x.ravel(), Ay.ravel()) - torch.vdot(y.ravel(), Ax.ravel()))) \
+        <= 1e-13 * float(x.norm() * Ay.norm())
+    assert float(torch.vdot(x.ravel(), Ax.ravel())) > 0
+    one = torch.ones_like(x)
+    V = oref.volume()
+    assert np.allclose(gpu.apply(one).cpu().numpy().reshape(mesh.shape), V, rtol=1e-13, atol=0)
+
+
+# ------------------------------------------------------------------ full solves: every K1 variant / loop mode
+VARIANTS = [(0, 0), (1, 0), (1, 1), (1, 2), (1, 3), (1, 4)]
+
+
+@pytest.mark.parametrize("loop_mode", [1, 0])
+@pytest.mark.parametrize("variant,tile", VARIANTS)
+def test_solve_parity_general_mesh_all_variants(variant, tile, loop_mode):
+    mesh, dt, nu_kind, nu = H.general_case(21, 19, 134, s=500.0)   # 3 phi tiles (ragged), ragged theta
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    gpu.set_option("variant", variant)
+    gpu.set_option("tile", tile)
+    gpu.set_option("loop_mode", loop_mode)
+    rng = np.random.default_rng(3)
+    b = rng.uniform(-1, 1, mesh.shape)
+    x0 = rng.standard_normal(mesh.shape)
+    H.check_parity(gpu, oref, b, x0, 1e-10, 2000, label=f"v{variant} t{tile} m{loop_mode}")
+    assert gpu.stats()["loop_mode"] == loop_mode
+
+
+@pytest.mark.parametrize("variant,tile", VARIANTS)
+def test_solve_parity_uniform_phi_all_variants(variant, tile):
+    prob = configs.make("c3", shape=(40, 37, 192))
+    s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
+    oref, gpu = H.both_ops(prob.mesh, 1e3 / s1, prob.nu_kind, prob.nu)
+    gpu.set_option("variant", variant)
+    gpu.set_option("tile", tile)
+    H.check_parity(gpu, oref, configs.rhs_blob(prob), None, 1e-9, 3000, label=f"v{variant} t{tile}")
+
+
+@pytest.mark.parametrize("bc", [(1, 1), (1, 0)])
+def test_solve_parity_neumann(bc):
+    mesh, dt, nu_kind, nu = H.general_case(10, 9, 66, s=50.0, bc=bc)
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu, bc)
+    b = np.random.default_rng(8).uniform(-1, 1, mesh.shape)
+    H.check_parity(gpu, oref, b, None, 1e-10, 2000, label=f"bc{bc}")
+
+
+# ------------------------------------------------------------------ BASELINE.json configs
+def test_config1_parity_and_rerun_bit_identity():
+    import torch
+    prob = configs.make("c1")
+    oref, gpu = H.both_ops(prob.mesh, prob.dt_for(2.0), prob.nu_kind, prob.nu)
+    b = configs.rhs_uniform(prob)
+    k_r, k_g = H.check_parity(gpu, oref, b, None, prob.rtol, prob.maxit, label="c1")
+    # north_star (3): a rerun gives the same bits
+    bd = _t(b)
+    runs = []
+    for _ in range(3):
+        xd = torch.zeros_like(bd)
+        st, k, h = gpu.solve(bd, xd, prob.rtol, prob.maxit)
+        runs.append((k, h.tobytes(), xd.cpu().numpy().tobytes()))
+    assert runs[0] == runs[1] == runs[2]
+
+
+@pytest.mark.parametrize("s", configs.STIFFNESS["c2"])
+def test_config2_parity_and_manufactured_solution(s):
+    import torch
+    prob = configs.make("c2")
+    oref, gpu = H.both_ops(prob.mesh, prob.dt_for(s), prob.nu_kind, prob.nu)
+    u = configs.field_manufactured(prob)
+    b = oref.apply_phys(u)                       # the same b for both sides
+    H.check_parity(gpu, oref, b, None, 1e-10, prob.maxit, label=f"c2 s={s}")
+    # P1 on the GPU path: recover u to 1e-10 at rtol 1e-14 (Q11)
+    bd, xd = _t(b), torch.zeros(prob.mesh.shape, dtype=torch.float64, device="cuda")
+    st, k, h = gpu.solve(bd, xd, 1e-14, 5000)
+    assert st == 0
+    xg = xd.cpu().numpy()
+    assert np.linalg.norm(xg - u) / np.linalg.norm(u) <= 1e-10
+
+
+def test_config3_parity_full_size():
+    prob = configs.make("c3")
+    oref, gpu = H.both_ops(prob.mesh, prob.dt_for(1e4), prob.nu_kind, prob.nu)
+    H.check_parity(gpu, oref, configs.rhs_blob(prob), None, prob.rtol, prob.maxit, label="c3")
+
+
+def test_config4_full_size_first_50_iterations_and_fixed_count():
+    """256x256x512 in the launch configuration bench.py times: history over the first 50 iterations
+    and x after 50 against the oracle; then the 500-fixed-iteration run returns MAS_MAXIT, k = 500."""
+    import torch
+    prob = configs.make("c4")
+    oref, gpu = H.both_ops(prob.mesh, prob.dt_for(1e4), prob.nu_kind, prob.nu)
+    b = configs.rhs_uniform(prob)
+    H.check_parity(gpu, oref, b, None, 0.0, 50, label="c4/50")
+    bd = _t(b)
+    xd = torch.zeros_like(bd)
+    st, k, h = gpu.solve(bd, xd, 0.0, prob.maxit)
+    assert st == 1 and k == prob.maxit and np.isfinite(h).all() and h.size == prob.maxit + 1
+    assert gpu.stats()["loop_launches"] == 2 * prob.maxit
+    # property that holds at any size: the true residual of the returned x matches the recurrence
+    V = _t(oref.volume())
+    r_true = V * bd - gpu.apply(xd)
+    h_true = float(r_true.norm() / (V * bd).norm())
+    assert h_true == pytest.approx(h[-1], rel=1e-3)
+
+
+def test_config5_chain_first_3_solves():
+    """Time-step proxy: dt varies per step, warm start; both sides get the SAME right-hand sides
+    (built from the oracle's x_k) so that the histories are comparable to 1e-10."""
+    prob = configs.make("c5", shape=(48, 64, 128))
+    s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
+    dt0 = 100.0 / s1
+    oref, gpu = H.both_ops(prob.mesh, dt0, prob.nu_kind, prob.nu)
+    chain = configs.Chain(prob, 3)
+    rhs = chain.state0 + chain.noise()
+    x_prev = None
+    for step in range(3):
+        dt = dt0 * chain.dt_factor[step]
+        oref.set_dt(dt)
+        gpu.set_dt(dt)
+        H.check_parity(gpu, oref, rhs, x_prev, prob.rtol, prob.maxit, label=f"c5 step {step}")
+        _, _, x_prev, _ = oref.pcg(rhs, x_prev, prob.rtol, prob.maxit)
+        rhs = x_prev + chain.noise()
+
+
+# ------------------------------------------------------------------ edge and degenerate cases
+def test_zero_rhs_maxit_zero_dt_zero():
+    import torch
+    mesh, dt, nu_kind, nu = H.general_case(6, 5, 8)
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    z = torch.zeros(mesh.shape, dtype=torch.float64, device="cuda")
+    x = torch.ones_like(z)
+    st, k, h = gpu.solve(z, x, 1e-10, 10)                  # zero RHS: x = 0, no iterations
+    assert (st, k) == (0, 0) and h[0] == 0.0 and not x.any()
+    b = _t(np.random.default_rng(0).uniform(-1, 1, mesh.shape))
+    x = torch.zeros_like(b)
+    st, k, h = gpu.solve(b, x, 1e-10, 0)                   # maxit = 0
+    assert (st, k) == (1, 0) and h.size == 1 and h[0] == pytest.approx(1.0) and not x.any()
+    gpu.set_dt(0.0)                                        # P7: A = diag(V): one iteration, x = b
+    st, k, h = gpu.solve(b, x, 1e-12, 10)
+    assert (st, k) == (0, 1)
+    assert torch.allclose(x, b, rtol=1e-15, atol=0)
+
+
+def test_smallest_mesh_and_single_row():
+    for shape in [(1, 1, 2), (1, 7, 4), (7, 1, 2)]:
+        mesh, dt, nu_kind, nu = H.general_case(*shape, s=20.0)
+        oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+        b = np.random.default_rng(2).uniform(-1, 1, mesh.shape)
+        H.check_parity(gpu, oref, b, None, 1e-12, 200, label=str(shape))
+
+
+def test_solve_host_matches_device_solve_bitwise():
+    import torch
+    prob = configs.make("c1")
+    from paper_1811_02605_b200 import MasPcg
+    gpu = MasPcg(prob.mesh, prob.dt_for(2.0), prob.nu_kind, prob.nu)
+    b = torch.from_numpy(configs.rhs_uniform(prob)).pin_memory()
+    xh = torch.zeros(prob.mesh.shape, dtype=torch.float64).pin_memory()
+    st, k, h = gpu.solve_host(b, xh, prob.rtol, prob.maxit)
+    xd = torch.zeros(prob.mesh.shape, dtype=torch.float64, device="cuda")
+    st2, k2, h2 = gpu.solve(b.cuda(), xd, prob.rtol, prob.maxit)
+    assert (st, k) == (st2, k2) and np.array_equal(h, h2) and torch.equal(xh, xd.cpu())
+
+
+def test_history_longer_than_initial_capacity_and_stream():
+    import torch
+    mesh, dt, nu_kind, nu = H.general_case(4, 4, 8, s=5.0)
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    b = _t(np.random.default_rng(5).uniform(-1, 1, mesh.shape))
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        x = torch.zeros_like(b)
+        st, k, h = gpu.solve(b, x, 1e-10, 20000, stream=s)      # maxit+1 > initial history capacity
+    assert st == 0 and k < 200
+    _, k_r, x_r, h_r = oref.pcg(b.cpu().numpy(), None, 1e-10, 20000)
+    assert abs(k - k_r) <= 1
