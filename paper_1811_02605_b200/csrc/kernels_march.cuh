@@ -209,6 +209,217 @@ k1_march(OpDev op, Work w, MarchParams mp, cudaGraphConditionalHandle cond, int 
         k1_finish(st, a1[0], cond, use_cond);
 }
 
+// =============================================================================================
+// K1 "wide": same algorithm, leaner instruction stream.  A warp covers a 128-cell row segment as
+// two coalesced 64-cell halves (A: cells k0+2l.., B: cells k0+64+2l..), i.e. 4 cells per lane, so
+// the per-plane overhead (barrier, loop control, coefficient loads, halo handling) is spread over
+// twice the cells; global addresses are bumped pointers; the step loop is unrolled by
+// lcm(3, DEPTH) so FIFO stage and ring buffer are compile-time; on uniform phi meshes the phi
+// factors are kernel constants.
+// =============================================================================================
+constexpr int WIDE_TK = 128;
+
+struct WideParams {
+    int nkt, njt, nit, ci;
+    double vp, wp, ip;                        // uniform-phi factors (dph_c, 2/dph_f, 1/dph_f)
+};
+
+template <int TJ, int DEPTH>
+struct WideSmem {
+    static constexpr int NW = TJ + 2;
+    static constexpr int NT = NW * 32;
+    static constexpr int NPL = MARCH_CI_MAX + 2;
+    double2 fifo[DEPTH][4][NT];               // [stage][rA rB pA pB][thread]
+    double hfifo[DEPTH][4][NW];               // [stage][r_left r_right p_left p_right][warp]
+    double2 ring[3][NW][64];                  // p_new planes: [buffer][row][A lanes 0..31 | B lanes 32..63]
+    double cE[NPL][NW], cF[NPL][NW], cD[NPL][NW], cAR[NPL][NW], cAT[NPL][NW];
+    double phv[WIDE_TK + 2], phw[WIDE_TK + 2], phi[WIDE_TK + 2];   // general phi: vp, wp, ip of cells k0-1..k0+128
+    double red[32];
+};
+
+template <int TJ, int DEPTH, bool UNIFORM, int MINB>
+__global__ void __launch_bounds__((TJ + 2) * 32, MINB)
+k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int use_cond)
+{
+    using Smem = WideSmem<TJ, DEPTH>;
+    constexpr int NT = Smem::NT, NW = Smem::NW;
+    constexpr int U = (DEPTH % 3 == 0) ? DEPTH : 3 * DEPTH;     // unroll: stage and ring index static
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    Smem &sm = *reinterpret_cast<Smem *>(smem_raw);
+
+    State *st = w.st;
+    if (!st->active) return;
+    const double beta = st->beta;
+    const int par = st->k & 1;
+    const double *__restrict__ pin = par ? w.p1 : w.p0;
+    double *__restrict__ pout = par ? w.p0 : w.p1;
+    const double *__restrict__ rvec = w.r;
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
+    int b = blockIdx.x;
+    const int kt = b % mp.nkt; b /= mp.nkt;
+    const int jt = b % mp.njt;
+    const int it = b / mp.njt;
+    const int i0 = it * mp.ci, i1 = min(i0 + mp.ci, op.nr);
+    const int first = i0 - 1, nsteps = i1 - i0 + 2;
+    const int j = jt * TJ + warp - 1;
+    const int k0 = kt * WIDE_TK;
+    const int tkeff = min(WIDE_TK, op.np - k0);
+    const bool row_ok = (j >= 0) && (j < op.nt);
+    const bool vA = row_ok && (2 * lane < tkeff), vB = row_ok && (64 + 2 * lane < tkeff);
+    const bool interior = (warp >= 1) && (warp <= TJ);
+    const bool qA = interior && vA, qB = interior && vB;
+    const bool left_edge = qA && (lane == 0);
+    const bool right_A = qA && (2 * lane + 2 == tkeff), right_B = qB && (64 + 2 * lane + 2 == tkeff);
+    const bool right_edge = right_A || right_B;
+    const int kl = k0 == 0 ? op.np - 1 : k0 - 1;
+    const int kr = k0 + tkeff >= op.np ? 0 : k0 + tkeff;
+
+    // ---- stage coefficient columns, phi factors; zero the FIFOs (invalid lanes then read zeros) ----
+    for (int e = tid; e < nsteps * NW; e += NT) {
+        const int pl = e / NW, wr = e - pl * NW;
+        const int ii = first + pl, jj = jt * TJ + wr - 1;
+        const bool in = ii >= 0 && ii < op.nr && jj >= 0 && jj < op.nt;
+        const int row = ii * op.nt + jj;
+        sm.cE[pl][wr] = in ? __ldg(op.E + row) : 0.0;
+        sm.cF[pl][wr] = in ? __ldg(op.F + row) : 0.0;
+        sm.cD[pl][wr] = in ? __ldg(op.Dinv + row) : 0.0;
+        sm.cAR[pl][wr] = (ii >= 0 && ii <= op.nr && jj >= 0 && jj < op.nt) ? __ldg(op.AR + row) : 0.0;
+        sm.cAT[pl][wr] = (ii >= 0 && ii < op.nr && jj >= 0 && jj <= op.nt) ? __ldg(op.AT + ii * (op.nt + 1) + jj) : 0.0;
+    }
+    if (!UNIFORM)
+        for (int e = tid; e < WIDE_TK + 2; e += NT) {
+            int kk = k0 - 1 + e;                                  // wrap once in either direction
+            kk = kk < 0 ? kk + op.np : (kk >= op.np ? kk - op.np : kk);
+            kk = kk >= op.np ? kk % op.np : kk;                   // tiny meshes (np < 130)
+            sm.phv[e] = __ldg(op.vp + kk); sm.phw[e] = __ldg(op.wp + kk); sm.phi[e] = __ldg(op.ip + kk);
+        }
+#pragma unroll
+    for (int s = 0; s < DEPTH; s++) {
+#pragma unroll
+        for (int a = 0; a < 4; a++) sm.fifo[s][a][tid] = make_double2(0.0, 0.0);
+        if (lane < 4) sm.hfifo[s][lane][warp] = 0.0;
+    }
+    __syncthreads();
+
+    // phi factors: cells A0,A1 (k, k+1) and B0,B1 (k+64, k+65); index into the staged arrays is cell-k0+1
+    const int ea = 2 * lane + 1, eb = 2 * lane + 65;
+    auto VP = [&](int e) { return UNIFORM ? mp.vp : sm.phv[e]; };
+    auto WP = [&](int e) { return UNIFORM ? mp.wp : sm.phw[e]; };
+    auto IP = [&](int e) { return UNIFORM ? mp.ip : sm.phi[e]; };   // ip of face e+1/2
+    auto zval = [&](double r, double E, double F, double dinv, int e) {
+        return UNIFORM ? r * dinv : r / fma(VP(e), E, F * WP(e));
+    };
+
+    // ---- bumped pointers ----
+    const long long plane = (long long)op.nt * op.np;
+    const long long rowbase0 = (long long)first * plane + (row_ok ? (long long)j * op.np : 0);
+    const double *ldr = rvec + rowbase0;            // row base of the next plane to prefetch
+    const double *ldp = pin + rowbase0;
+    const int ka = k0 + 2 * lane, kb = ka + 64;
+    double *stp = pout + rowbase0 + plane;          // row base of plane i0 (first store of p)
+    double *stq = w.q + rowbase0 + plane;           // row base of plane i0 (first store of q)
+    int ii_ld = first;                              // plane index of the next prefetch
+
+    auto issue = [&](int stage) {
+        if ((unsigned)ii_ld < (unsigned)op.nr && ii_ld <= i1) {
+            if (vA) { cp_async16(&sm.fifo[stage][0][tid], ldr + ka); cp_async16(&sm.fifo[stage][2][tid], ldp + ka); }
+            if (vB) { cp_async16(&sm.fifo[stage][1][tid], ldr + kb); cp_async16(&sm.fifo[stage][3][tid], ldp + kb); }
+            if (left_edge) { cp_async8(&sm.hfifo[stage][0][warp], ldr + kl); cp_async8(&sm.hfifo[stage][2][warp], ldp + kl); }
+            if (right_edge) { cp_async8(&sm.hfifo[stage][1][warp], ldr + kr); cp_async8(&sm.hfifo[stage][3][warp], ldp + kr); }
+        }
+        cp_async_commit();
+        ldr += plane; ldp += plane; ++ii_ld;
+    };
+
+#pragma unroll
+    for (int s = 0; s < DEPTH; s++) issue(s);
+
+    double2 am = make_double2(0.0, 0.0), ac = am, bm = am, bc = am;   // p_new of planes i-1 (m), i (c); halves A, B
+    double hl_c = 0.0, hr_c = 0.0;
+    double acc = 0.0;
+    const int lm = (lane + 31) & 31, lp = (lane + 1) & 31;
+
+    for (int tb = 0; tb < nsteps; tb += U) {
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const int t = tb + u;
+            if (t >= nsteps) break;
+            const int stage = u % DEPTH, rbw = u % 3, rbr = (u + 2) % 3;
+            const int ii = first + t;
+            const bool plane_ok = (unsigned)ii < (unsigned)op.nr;
+            const double En = sm.cE[t][warp], Fn = sm.cF[t][warp], dinv = sm.cD[t][warp];
+            cp_async_wait<DEPTH - 1>();
+            double2 an = make_double2(0.0, 0.0), bn = an;
+            double hl_n = 0.0, hr_n = 0.0;
+            if (plane_ok) {                         // block-uniform
+                const double2 ra = sm.fifo[stage][0][tid], rb = sm.fifo[stage][1][tid];
+                const double2 pa = sm.fifo[stage][2][tid], pb = sm.fifo[stage][3][tid];
+                if (UNIFORM || vA) {
+                    an.x = fma(beta, pa.x, zval(ra.x, En, Fn, dinv, ea));
+                    an.y = fma(beta, pa.y, zval(ra.y, En, Fn, dinv, ea + 1));
+                }
+                if (UNIFORM || vB) {
+                    bn.x = fma(beta, pb.x, zval(rb.x, En, Fn, dinv, eb));
+                    bn.y = fma(beta, pb.y, zval(rb.y, En, Fn, dinv, eb + 1));
+                }
+                if (left_edge) hl_n = fma(beta, sm.hfifo[stage][2][warp], zval(sm.hfifo[stage][0][warp], En, Fn, dinv, 0));
+                if (right_edge) hr_n = fma(beta, sm.hfifo[stage][3][warp], zval(sm.hfifo[stage][1][warp], En, Fn, dinv, tkeff + 1));
+                if (t >= 1 && t <= nsteps - 2) {    // interior plane: store p_new
+                    if (qA) st2(stp, ka, an);
+                    if (qB) st2(stp, kb, bn);
+                    stp += plane;
+                }
+            }
+            issue(stage);
+            sm.ring[rbw][warp][lane] = an;
+            sm.ring[rbw][warp][lane + 32] = bn;
+            __syncthreads();
+            // ---- q for plane i = ii-1 ----
+            const double mA = __shfl_sync(0xffffffffu, ac.y, lm), mB = __shfl_sync(0xffffffffu, bc.y, lm);
+            const double pA = __shfl_sync(0xffffffffu, ac.x, lp), pB = __shfl_sync(0xffffffffu, bc.x, lp);
+            if (t >= 2 && interior && row_ok) {
+                const double Ec = sm.cE[t - 1][warp], Fc = sm.cF[t - 1][warp];
+                const double ARm = sm.cAR[t - 1][warp], ARp = sm.cAR[t][warp];
+                const double ATm = sm.cAT[t - 1][warp], ATp = sm.cAT[t - 1][warp + 1];
+                if (qA) {
+                    const double ukm = left_edge ? hl_c : mA;
+                    const double ukp = right_A ? hr_c : (lane == 31 ? pB : pA);
+                    const double2 ujm = sm.ring[rbr][warp - 1][lane], ujp = sm.ring[rbr][warp + 1][lane];
+                    const double d0 = fma(VP(ea), Ec, Fc * WP(ea)), d1 = fma(VP(ea + 1), Ec, Fc * WP(ea + 1));
+                    const double sx = ARm * am.x + ARp * an.x + ATm * ujm.x + ATp * ujp.x;
+                    const double sy = ARm * am.y + ARp * an.y + ATm * ujm.y + ATp * ujp.y;
+                    double2 q;
+                    q.x = d0 * ac.x - VP(ea) * sx - Fc * (IP(ea) * ac.y + IP(ea - 1) * ukm);
+                    q.y = d1 * ac.y - VP(ea + 1) * sy - Fc * (IP(ea + 1) * ukp + IP(ea) * ac.x);
+                    st2(stq, ka, q);
+                    acc += ac.x * q.x + ac.y * q.y;
+                }
+                if (qB) {
+                    const double ukm = lane == 0 ? mA : mB;
+                    const double ukp = right_B ? hr_c : pB;
+                    const double2 ujm = sm.ring[rbr][warp - 1][lane + 32], ujp = sm.ring[rbr][warp + 1][lane + 32];
+                    const double d0 = fma(VP(eb), Ec, Fc * WP(eb)), d1 = fma(VP(eb + 1), Ec, Fc * WP(eb + 1));
+                    const double sx = ARm * bm.x + ARp * bn.x + ATm * ujm.x + ATp * ujp.x;
+                    const double sy = ARm * bm.y + ARp * bn.y + ATm * ujm.y + ATp * ujp.y;
+                    double2 q;
+                    q.x = d0 * bc.x - VP(eb) * sx - Fc * (IP(eb) * bc.y + IP(eb - 1) * ukm);
+                    q.y = d1 * bc.y - VP(eb + 1) * sy - Fc * (IP(eb + 1) * ukp + IP(eb) * bc.x);
+                    st2(stq, kb, q);
+                    acc += bc.x * q.x + bc.y * q.y;
+                }
+            }
+            if (t >= 2) stq += plane;
+            am = ac; ac = an; bm = bc; bc = bn;
+            hl_c = hl_n; hr_c = hr_n;
+        }
+    }
+    cp_async_wait<0>();
+    double a1[1] = {acc};
+    if (grid_sum<NT, 1>(a1, w.partials, &st->ticket[1], sm.red) && threadIdx.x == 0)
+        k1_finish(st, a1[0], cond, use_cond);
+}
+
 // ---------------------------------------------------------------------------------------------
 // host-side configuration table
 // ---------------------------------------------------------------------------------------------
@@ -247,6 +458,60 @@ inline void march_configure(int nr, int nt, int np, int uniform, int tile, int n
     while (ci > 8 && (long long)mp->nkt * mp->njt * ((nr + ci - 1) / ci) < 8LL * num_sms) ci /= 2;
     mp->ci = ci;
     mp->nit = (nr + ci - 1) / ci;
+    *grid = dim3((unsigned)(mp->nkt * mp->njt * mp->nit));
+}
+
+// ---- wide variant ----
+struct WideTile {
+    int tj, depth, minb;
+};
+static const WideTile kWideTiles[] = {{8, 3, 2}, {6, 3, 2}, {6, 2, 3}, {14, 3, 1}, {8, 2, 2}, {4, 3, 3}, {10, 3, 1}};
+inline int wide_num_tiles() { return (int)(sizeof(kWideTiles) / sizeof(kWideTiles[0])); }
+
+template <int TJ, int DEPTH, int MINB>
+inline void wide_pick(bool uniform, const void **func, dim3 *block, size_t *smem)
+{
+    *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB> : (const void *)k1_wide<TJ, DEPTH, false, MINB>;
+    *block = dim3((TJ + 2) * 32);
+    *smem = sizeof(WideSmem<TJ, DEPTH>);
+    cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);
+}
+
+inline void wide_configure(int nr, int nt, int np, int uniform, int tile, int num_sms, int ci_force, WideParams *mp,
+                           const void **func, dim3 *grid, dim3 *block, size_t *smem)
+{
+    const WideTile T = kWideTiles[tile];
+    switch (tile) {
+        case 0: wide_pick<8, 3, 2>(uniform, func, block, smem); break;
+        case 1: wide_pick<6, 3, 2>(uniform, func, block, smem); break;
+        case 2: wide_pick<6, 2, 3>(uniform, func, block, smem); break;
+        case 3: wide_pick<14, 3, 1>(uniform, func, block, smem); break;
+        case 4: wide_pick<8, 2, 2>(uniform, func, block, smem); break;
+        case 5: wide_pick<4, 3, 3>(uniform, func, block, smem); break;
+        default: wide_pick<10, 3, 1>(uniform, func, block, smem); break;
+    }
+    mp->nkt = (np + WIDE_TK - 1) / WIDE_TK;
+    mp->njt = (nt + T.tj - 1) / T.tj;
+    int occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, *func, (int)block->x, *smem) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        occ = 1;
+    }
+    const long long slots = (long long)num_sms * occ, cols = (long long)mp->nkt * mp->njt;
+    // r-chunk length: minimise rounds x (planes per block + halo planes + start-up), ties -> longer chunks
+    int best = MARCH_CI_MAX;
+    double best_cost = 1e300;
+    for (int ci = MARCH_CI_MAX; ci >= 4; ci -= 2) {
+        const long long tiles = cols * ((nr + ci - 1) / ci);
+        if (tiles > MAX_PARTIALS) continue;
+        const double rounds = (double)((tiles + slots - 1) / slots);
+        const double cost = rounds * (ci + 2 + 3);
+        if (cost < best_cost * 0.999) { best_cost = cost; best = ci; }
+    }
+    if (nr < best) best = nr;
+    if (ci_force > 0 && ci_force <= MARCH_CI_MAX) best = ci_force;
+    mp->ci = best;
+    mp->nit = (nr + best - 1) / best;
     *grid = dim3((unsigned)(mp->nkt * mp->njt * mp->nit));
 }
 

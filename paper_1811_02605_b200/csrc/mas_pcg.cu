@@ -59,7 +59,7 @@ struct mas_pcg {
     int uniform_phi = 0;
     // device planes
     DevBuf<double> V2, SD, CP, CRoff, CT, E, F, AR, AT, Dinv, vp, wp, ip;
-    double vp0 = 0, wp0 = 0;
+    double vp0 = 0, wp0 = 0, ip0 = 0;
     // workspaces
     DevBuf<double> r, p0, p1, q, partials, hist, bdev, xdev;
     DevBuf<State> st;
@@ -72,8 +72,9 @@ struct mas_pcg {
     // loop
     int loop_mode = 1;               // requested: 1 graph-while, 0 host chunks
     int loop_mode_used = 1;
-    int variant = 1;                 // K1 variant (0 = baseline, 1 = 2.5-D marching tiles)
-    int tile = 0;                    // marching tile configuration id
+    int variant = 2;                 // K1 variant: 0 baseline, 1 marching tiles (64 wide), 2 wide marching tiles
+    int tile = 0;                    // tile configuration id of the variant
+    int ci_force = 0;                // >0: override the r-chunk length (tuning)
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
     bool graph_dirty = true;
@@ -253,6 +254,7 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
     for (int k = 0; k < np; k++) wp[k] = ip[k] + ip[(k + np - 1) % np];
     h->vp0 = vp[0];
     h->wp0 = wp[0];
+    h->ip0 = ip[0];
 
     int rc;
     if ((rc = upload(h->V2, V2)) || (rc = upload(h->CP, CP)) || (rc = upload(h->SD, SD)) ||
@@ -296,6 +298,7 @@ struct LoopCtx {                     // storage that kernel argument pointers re
     const SolveArgs *args;
     double *y;
     MarchParams mp;
+    WideParams wp;
 };
 
 int base_grid(const mas_pcg *h, const void *func, int nt_block)
@@ -360,9 +363,17 @@ KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
         k.nargs = 4;
         return k;
     }
-    march_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, &c.mp, &k.func, &k.grid, &k.block,
-                    &k.smem);
-    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.mp; k.args[3] = &c.cond; k.args[4] = &c.use_cond;
+    if (h->variant == 1) {
+        march_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, &c.mp, &k.func, &k.grid, &k.block,
+                        &k.smem);
+        k.args[2] = &c.mp;
+    } else {
+        wide_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, h->ci_force, &c.wp, &k.func, &k.grid,
+                       &k.block, &k.smem);
+        c.wp.vp = h->vp0; c.wp.wp = h->wp0; c.wp.ip = h->ip0;
+        k.args[2] = &c.wp;
+    }
+    k.args[0] = &c.op; k.args[1] = &c.work; k.args[3] = &c.cond; k.args[4] = &c.use_cond;
     k.nargs = 5;
     return k;
 }
@@ -475,11 +486,16 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->loop_mode = value;
     } else if (!strcmp(name, "variant")) {
-        if (value < 0 || value > 1) return MAS_EINVAL;
+        if (value < 0 || value > 2) return MAS_EINVAL;
         h->variant = value;
+        h->tile = 0;
     } else if (!strcmp(name, "tile")) {
-        if (value < 0 || value >= march_num_tiles()) return MAS_EINVAL;
+        const int nt_ = h->variant == 1 ? march_num_tiles() : (h->variant == 2 ? wide_num_tiles() : 1);
+        if (value < 0 || value >= nt_) return MAS_EINVAL;
         h->tile = value;
+    } else if (!strcmp(name, "ci")) {
+        if (value < 0 || value > MARCH_CI_MAX) return MAS_EINVAL;
+        h->ci_force = value;
     } else {
         return MAS_EINVAL;
     }

@@ -53,7 +53,7 @@ def test_gpu_operator_symmetric_and_constant_closed_form():
 
 
 # ------------------------------------------------------------------ full solves: every K1 variant / loop mode
-VARIANTS = [(0, 0)] + [(1, t) for t in range(7)]
+VARIANTS = [(0, 0)] + [(1, t) for t in range(7)] + [(2, t) for t in range(7)]
 
 
 @pytest.mark.parametrize("loop_mode", [1, 0])
