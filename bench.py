@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--tile", type=int, default=None)
     ap.add_argument("--loop-mode", type=int, default=None)
+    ap.add_argument("--xfuse", type=int, default=None)
+    ap.add_argument("--ci", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -207,6 +209,10 @@ def main():
         gpu.set_option("tile", args.tile)
     if args.loop_mode is not None:
         gpu.set_option("loop_mode", args.loop_mode)
+    if args.xfuse is not None:
+        gpu.set_option("xfuse", args.xfuse)
+    if args.ci is not None:
+        gpu.set_option("ci", args.ci)
     b_host = torch.from_numpy(b_np).pin_memory()
     x_host = torch.zeros(prob.mesh.shape, dtype=torch.float64).pin_memory()
     b = b_host.cuda()
@@ -272,7 +278,8 @@ def main():
         value = iters_all / (ms * 1e-3)
         bpc = stats["bytes_per_cell_iter"]
         peak, peak_src = hbm_peak()
-        k1_bytes, k2_bytes = 4 * 8 * n, 6 * 8 * n         # K1: r,p -> p,q ; K2: x,p,r,q -> x,r
+        stats = gpu.stats()                               # after profile(): per-kernel doubles per cell
+        k1_bytes, k2_bytes = stats["k1_doubles_per_cell"] * 8 * n, stats["k2_doubles_per_cell"] * 8 * n
         k1_gbs = k1_bytes / (prof["k1_ms"] * 1e-3) / 1e9
         k2_gbs = k2_bytes / (prof["k2_ms"] * 1e-3) / 1e9
         dom = "k1_fused_matvec" if prof["k1_ms"] >= prof["k2_ms"] else "k2_fused_vector"

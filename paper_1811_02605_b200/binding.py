@@ -169,4 +169,5 @@ def mas_pcg_stats(handle):
     st = lib().mas_pcg_stats(handle, out)
     if st != MAS_OK:
         raise MasError(st, "mas_pcg_stats")
-    return {"loop_launches": out[0], "other_launches": out[1], "loop_mode": out[2], "bytes_per_cell_iter": out[3]}
+    return {"loop_launches": out[0], "other_launches": out[1], "loop_mode": out[2], "bytes_per_cell_iter": out[3],
+            "k1_doubles_per_cell": out[4], "k2_doubles_per_cell": out[5]}

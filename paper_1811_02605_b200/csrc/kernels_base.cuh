@@ -195,7 +195,8 @@ __global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditio
 // K2 (S4+S5): x += alpha p; r -= alpha q; z = r/d; rho' = r.z; rr = r.r; last block: k++,
 // hist[k], beta, convergence test, graph conditional.  6N doubles of traffic.
 // ---------------------------------------------------------------------------------------------
-template <int NT, bool UNIFORM>
+// XF = true: the x-update lives in K1 (deferred one iteration), K2 only touches r and q: 3N doubles.
+template <int NT, bool UNIFORM, bool XF>
 __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond)
 {
     __shared__ double sh[32];
@@ -216,13 +217,17 @@ __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditio
             const size_t base = (size_t)row * op.np;
             for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
                 const size_t cell = base + 2 * kv;
-                double2 xv = ld2(x, cell), rv = ld2(w.r, cell);
-                const double2 pv = ld2(p, cell), qv = ld2(w.q, cell);
-                xv.x = fma(alpha, pv.x, xv.x);
-                xv.y = fma(alpha, pv.y, xv.y);
+                double2 rv = ld2(w.r, cell);
+                const double2 qv = ld2(w.q, cell);
+                if (!XF) {
+                    double2 xv = ld2(x, cell);
+                    const double2 pv = ld2(p, cell);
+                    xv.x = fma(alpha, pv.x, xv.x);
+                    xv.y = fma(alpha, pv.y, xv.y);
+                    st2(x, cell, xv);
+                }
                 rv.x = fma(-alpha, qv.x, rv.x);
                 rv.y = fma(-alpha, qv.y, rv.y);
-                st2(x, cell, xv);
                 st2(w.r, cell, rv);
                 double z0, z1;
                 if (UNIFORM) { z0 = rv.x * dinv; z1 = rv.y * dinv; }
@@ -252,6 +257,32 @@ __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditio
     }
 }
 
+// XF tail (after the loop): the one x-update still pending, x += alpha_{k-1} p_{k-1}.  alpha is 0 when
+// nothing is pending (no iteration ran, or K1 broke down after applying the previous update).
+template <int NT>
+__global__ void __launch_bounds__(NT) k_xtail(OpDev op, Work w)
+{
+    const State *st = w.st;
+    const double alpha = st->alpha;
+    const double *p = (st->k & 1) ? w.p1 : w.p0;
+    double *x = w.args->x;
+    const RowMap m = row_map<NT>(op.nv);
+    if (m.idle) return;
+    for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
+        const int row = rowbase + m.rl;
+        if (row >= op.nrows) break;
+        const size_t base = (size_t)row * op.np;
+        for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
+            const size_t cell = base + 2 * kv;
+            double2 xv = ld2(x, cell);
+            const double2 pv = ld2(p, cell);
+            xv.x = fma(alpha, pv.x, xv.x);
+            xv.y = fma(alpha, pv.y, xv.y);
+            st2(x, cell, xv);
+        }
+    }
+}
+
 // the last block of every K1 variant ends with this: sigma -> alpha, breakdown test (S3)
 __device__ __forceinline__ void k1_finish(State *st, double sigma, cudaGraphConditionalHandle cond, int use_cond)
 {
@@ -260,6 +291,7 @@ __device__ __forceinline__ void k1_finish(State *st, double sigma, cudaGraphCond
     if (!(sigma > 0.0) || isinf(sigma)) {
         st->status = ST_BREAKDOWN;
         st->active = 0;
+        st->alpha = 0.0;                 // nothing pending for the XF tail
         set_cond(cond, use_cond, 0);
     } else {
         st->alpha = st->rho / sigma;

@@ -237,7 +237,7 @@ struct WideSmem {
     double red[32];
 };
 
-template <int TJ, int DEPTH, bool UNIFORM, int MINB>
+template <int TJ, int DEPTH, bool UNIFORM, int MINB, bool XF>
 __global__ void __launch_bounds__((TJ + 2) * 32, MINB)
 k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int use_cond)
 {
@@ -254,6 +254,10 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
     const double *__restrict__ pin = par ? w.p1 : w.p0;
     double *__restrict__ pout = par ? w.p0 : w.p1;
     const double *__restrict__ rvec = w.r;
+    // XF: the x-update of the PREVIOUS iteration, x += alpha_{k-1} p_{k-1}, is applied here (p_old is
+    // p_{k-1}); K2 then only updates r.  Same operations on the same operands as the unfused path.
+    const double alpha_prev = XF ? st->alpha : 0.0;
+    double *__restrict__ xvec = XF ? w.args->x : nullptr;
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
     int b = blockIdx.x;
@@ -319,6 +323,8 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
     const int ka = k0 + 2 * lane, kb = ka + 64;
     double *stp = pout + rowbase0 + plane;          // row base of plane i0 (first store of p)
     double *stq = w.q + rowbase0 + plane;           // row base of plane i0 (first store of q)
+    double *xrow = XF ? xvec + rowbase0 + plane : nullptr;   // row base of plane i0 (x is updated in place)
+    double2 xa = make_double2(0.0, 0.0), xb = xa;   // x of the NEXT interior plane, loaded one step ahead
     int ii_ld = first;                              // plane index of the next prefetch
 
     auto issue = [&](int stage) {
@@ -365,11 +371,20 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
                 }
                 if (left_edge) hl_n = fma(beta, sm.hfifo[stage][2][warp], zval(sm.hfifo[stage][0][warp], En, Fn, dinv, 0));
                 if (right_edge) hr_n = fma(beta, sm.hfifo[stage][3][warp], zval(sm.hfifo[stage][1][warp], En, Fn, dinv, tkeff + 1));
-                if (t >= 1 && t <= nsteps - 2) {    // interior plane: store p_new
+                if (t >= 1 && t <= nsteps - 2) {    // interior plane: store p_new (and the deferred x-update)
                     if (qA) st2(stp, ka, an);
                     if (qB) st2(stp, kb, bn);
                     stp += plane;
+                    if (XF) {
+                        if (qA) { xa.x = fma(alpha_prev, pa.x, xa.x); xa.y = fma(alpha_prev, pa.y, xa.y); st2(xrow, ka, xa); }
+                        if (qB) { xb.x = fma(alpha_prev, pb.x, xb.x); xb.y = fma(alpha_prev, pb.y, xb.y); st2(xrow, kb, xb); }
+                        xrow += plane;
+                    }
                 }
+            }
+            if (XF && t <= nsteps - 3) {            // x of the next step's (interior) plane
+                if (qA) xa = ld2(xrow, ka);
+                if (qB) xb = ld2(xrow, kb);
             }
             issue(stage);
             sm.ring[rbw][warp][lane] = an;
@@ -465,30 +480,33 @@ inline void march_configure(int nr, int nt, int np, int uniform, int tile, int n
 struct WideTile {
     int tj, depth, minb;
 };
-static const WideTile kWideTiles[] = {{8, 3, 2}, {6, 3, 2}, {6, 2, 3}, {14, 3, 1}, {8, 2, 2}, {4, 3, 3}, {10, 3, 1}};
+static const WideTile kWideTiles[] = {{8, 2, 2}, {6, 3, 2}, {6, 2, 3}, {14, 3, 1}, {8, 3, 2}, {4, 3, 3}, {10, 3, 1}};
 inline int wide_num_tiles() { return (int)(sizeof(kWideTiles) / sizeof(kWideTiles[0])); }
 
 template <int TJ, int DEPTH, int MINB>
-inline void wide_pick(bool uniform, const void **func, dim3 *block, size_t *smem)
+inline void wide_pick(bool uniform, bool xf, const void **func, dim3 *block, size_t *smem)
 {
-    *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB> : (const void *)k1_wide<TJ, DEPTH, false, MINB>;
+    if (xf)
+        *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, true> : (const void *)k1_wide<TJ, DEPTH, false, MINB, true>;
+    else
+        *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, false> : (const void *)k1_wide<TJ, DEPTH, false, MINB, false>;
     *block = dim3((TJ + 2) * 32);
     *smem = sizeof(WideSmem<TJ, DEPTH>);
     cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);
 }
 
-inline void wide_configure(int nr, int nt, int np, int uniform, int tile, int num_sms, int ci_force, WideParams *mp,
+inline void wide_configure(int nr, int nt, int np, int uniform, int xf, int tile, int num_sms, int ci_force, WideParams *mp,
                            const void **func, dim3 *grid, dim3 *block, size_t *smem)
 {
     const WideTile T = kWideTiles[tile];
     switch (tile) {
-        case 0: wide_pick<8, 3, 2>(uniform, func, block, smem); break;
-        case 1: wide_pick<6, 3, 2>(uniform, func, block, smem); break;
-        case 2: wide_pick<6, 2, 3>(uniform, func, block, smem); break;
-        case 3: wide_pick<14, 3, 1>(uniform, func, block, smem); break;
-        case 4: wide_pick<8, 2, 2>(uniform, func, block, smem); break;
-        case 5: wide_pick<4, 3, 3>(uniform, func, block, smem); break;
-        default: wide_pick<10, 3, 1>(uniform, func, block, smem); break;
+        case 0: wide_pick<8, 2, 2>(uniform, xf, func, block, smem); break;
+        case 1: wide_pick<6, 3, 2>(uniform, xf, func, block, smem); break;
+        case 2: wide_pick<6, 2, 3>(uniform, xf, func, block, smem); break;
+        case 3: wide_pick<14, 3, 1>(uniform, xf, func, block, smem); break;
+        case 4: wide_pick<8, 3, 2>(uniform, xf, func, block, smem); break;
+        case 5: wide_pick<4, 3, 3>(uniform, xf, func, block, smem); break;
+        default: wide_pick<10, 3, 1>(uniform, xf, func, block, smem); break;
     }
     mp->nkt = (np + WIDE_TK - 1) / WIDE_TK;
     mp->njt = (nt + T.tj - 1) / T.tj;

@@ -75,6 +75,7 @@ struct mas_pcg {
     int variant = 2;                 // K1 variant: 0 baseline, 1 marching tiles (64 wide), 2 wide marching tiles
     int tile = 0;                    // tile configuration id of the variant
     int ci_force = 0;                // >0: override the r-chunk length (tuning)
+    int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
     bool graph_dirty = true;
@@ -344,13 +345,30 @@ KLaunch make_init(const mas_pcg *h, LoopCtx &c)
 KLaunch make_k2(const mas_pcg *h, LoopCtx &c)
 {
     KLaunch k;
-    k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true> : (const void *)k2_vec<NT_BASE, false>;
+    const bool xf = h->xfuse && h->variant == 2;
+    if (xf)
+        k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true, true> : (const void *)k2_vec<NT_BASE, false, true>;
+    else
+        k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true, false> : (const void *)k2_vec<NT_BASE, false, false>;
     k.block = dim3(NT_BASE);
     k.grid = dim3(base_grid(h, k.func, NT_BASE));
     k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
     k.nargs = 4;
     return k;
 }
+
+KLaunch make_xtail(const mas_pcg *h, LoopCtx &c)
+{
+    KLaunch k;
+    k.func = (const void *)k_xtail<NT_BASE>;
+    k.block = dim3(NT_BASE);
+    k.grid = dim3(base_grid(h, k.func, NT_BASE));
+    k.args[0] = &c.op; k.args[1] = &c.work;
+    k.nargs = 2;
+    return k;
+}
+
+bool use_xfuse(const mas_pcg *h) { return h->xfuse && h->variant == 2; }
 
 KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
 {
@@ -368,8 +386,8 @@ KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
                         &k.smem);
         k.args[2] = &c.mp;
     } else {
-        wide_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, h->ci_force, &c.wp, &k.func, &k.grid,
-                       &k.block, &k.smem);
+        wide_configure(h->nr, h->nt, h->np, h->uniform_phi, use_xfuse(h), h->tile, h->num_sms, h->ci_force, &c.wp,
+                       &k.func, &k.grid, &k.block, &k.smem);
         c.wp.vp = h->vp0; c.wp.wp = h->wp0; c.wp.ip = h->ip0;
         k.args[2] = &c.wp;
     }
@@ -435,6 +453,11 @@ int build_graph(mas_pcg *h)
         cudaGetLastError();
         return MAS_ECUDA;
     }
+    if (use_xfuse(h)) {
+        cudaGraphNode_t n_tail;
+        const KLaunch kt = make_xtail(h, c);
+        if (add_node(&n_tail, g, &n_while, kt) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+    }
     if (cudaGraphInstantiate(&h->exec, g, 0) != cudaSuccess) {
         cudaGetLastError();
         h->exec = nullptr;
@@ -493,6 +516,9 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
         const int nt_ = h->variant == 1 ? march_num_tiles() : (h->variant == 2 ? wide_num_tiles() : 1);
         if (value < 0 || value >= nt_) return MAS_EINVAL;
         h->tile = value;
+    } else if (!strcmp(name, "xfuse")) {
+        if (value != 0 && value != 1) return MAS_EINVAL;
+        h->xfuse = value;
     } else if (!strcmp(name, "ci")) {
         if (value < 0 || value > MARCH_CI_MAX) return MAS_EINVAL;
         h->ci_force = value;
@@ -552,7 +578,9 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
             launched_loop += 2LL * chunk;
             done += chunk;
         }
+        if (use_xfuse(h)) CK(launch(make_xtail(h, c), s));
     }
+    if (use_xfuse(h)) launched_outside += 1;
     CK(cudaMemcpyAsync(h->h_st, h->st.p, sizeof(State), cudaMemcpyDeviceToHost, s));
     CK(cudaMemcpyAsync(h->h_hist, h->hist.p, ((size_t)maxit + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));          // the one host sync of a graph-mode solve
@@ -567,7 +595,10 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     h->stats[0] = mode == 1 ? (long long)st.launches : launched_loop;
     h->stats[1] = launched_outside;
     h->stats[2] = mode;
-    h->stats[3] = 80;                      // K1: r,p -> p,q (4N) ; K2: x,p,r,q -> x,r (6N) ; 8 B each
+    // unfused: K1 r,p -> p,q (4N); K2 x,p,r,q -> x,r (6N).  xfuse: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)
+    h->stats[4] = use_xfuse(h) ? 6 : 4;
+    h->stats[5] = use_xfuse(h) ? 3 : 6;
+    h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
     return st.status;
 }
 
@@ -625,5 +656,8 @@ extern "C" int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev,
     }
     for (cudaEvent_t &e : ev) cudaEventDestroy(e);
     ms_out[0] = sum1 / nit; ms_out[1] = sum2 / nit; ms_out[2] = min1; ms_out[3] = min2;
+    h->stats[4] = use_xfuse(h) ? 6 : 4;
+    h->stats[5] = use_xfuse(h) ? 3 : 6;
+    h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
     return MAS_OK;
 }

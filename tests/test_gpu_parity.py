@@ -53,16 +53,18 @@ def test_gpu_operator_symmetric_and_constant_closed_form():
 
 
 # ------------------------------------------------------------------ full solves: every K1 variant / loop mode
-VARIANTS = [(0, 0)] + [(1, t) for t in range(7)] + [(2, t) for t in range(7)]
+# (variant, tile, xfuse)
+VARIANTS = [(0, 0, 0)] + [(1, t, 0) for t in range(7)] + [(2, t, x) for t in range(7) for x in (0, 1)]
 
 
 @pytest.mark.parametrize("loop_mode", [1, 0])
-@pytest.mark.parametrize("variant,tile", VARIANTS)
-def test_solve_parity_general_mesh_all_variants(variant, tile, loop_mode):
+@pytest.mark.parametrize("variant,tile,xfuse", VARIANTS)
+def test_solve_parity_general_mesh_all_variants(variant, tile, xfuse, loop_mode):
     mesh, dt, nu_kind, nu = H.general_case(21, 19, 134, s=500.0)   # 3 phi tiles (ragged), ragged theta
     oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
     gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
+    gpu.set_option("xfuse", xfuse)
     gpu.set_option("loop_mode", loop_mode)
     rng = np.random.default_rng(3)
     b = rng.uniform(-1, 1, mesh.shape)
@@ -71,14 +73,15 @@ def test_solve_parity_general_mesh_all_variants(variant, tile, loop_mode):
     assert gpu.stats()["loop_mode"] == loop_mode
 
 
-@pytest.mark.parametrize("variant,tile", VARIANTS)
-def test_solve_parity_uniform_phi_all_variants(variant, tile):
+@pytest.mark.parametrize("variant,tile,xfuse", VARIANTS)
+def test_solve_parity_uniform_phi_all_variants(variant, tile, xfuse):
     prob = configs.make("c3", shape=(40, 37, 192))
     s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
     oref, gpu = H.both_ops(prob.mesh, 1e3 / s1, prob.nu_kind, prob.nu)
     gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
-    H.check_parity(gpu, oref, configs.rhs_blob(prob), None, 1e-9, 3000, label=f"v{variant} t{tile}")
+    gpu.set_option("xfuse", xfuse)
+    H.check_parity(gpu, oref, configs.rhs_blob(prob), None, 1e-9, 3000, label=f"v{variant} t{tile} x{xfuse}")
 
 
 @pytest.mark.parametrize("bc", [(1, 1), (1, 0)])
@@ -141,6 +144,7 @@ def test_config4_full_size_first_50_iterations_and_fixed_count():
     st, k, h = gpu.solve(bd, xd, 0.0, prob.maxit)
     assert st == 1 and k == prob.maxit and np.isfinite(h).all() and h.size == prob.maxit + 1
     assert gpu.stats()["loop_launches"] == 2 * prob.maxit
+    assert gpu.stats()["bytes_per_cell_iter"] in (72, 80)
     # property that holds at any size: the true residual of the returned x matches the recurrence
     V = _t(oref.volume())
     r_true = V * bd - gpu.apply(xd)
