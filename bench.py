@@ -150,6 +150,19 @@ def time_oracle(prob, dt, b, iters):
     return t, k
 
 
+def reduce_over_ranks(ms, iters, launches, world, device="cuda"):
+    """Replicas: time = MAX over ranks, work (iterations, launches) = SUM over ranks."""
+    if world == 1:
+        return ms, iters, launches
+    import torch
+    import torch.distributed as dist
+    tmax = torch.tensor([ms], dtype=torch.float64, device=device)
+    tsum = torch.tensor([iters, launches], dtype=torch.float64, device=device)
+    dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+    return float(tmax[0]), float(tsum[0]), float(tsum[1])
+
+
 def run_reference(args, rank, world):
     """Base-contract reference arm = the oracle on host cores; rank 0 only."""
     if rank != 0:
@@ -262,17 +275,8 @@ def main():
     prof = gpu.profile(b, x, 40)
     barrier()
 
-    t_all = torch.tensor([ms, e2e_s * 1e3, float(iters_done), float(e2e_iters), float(launches)],
-                         dtype=torch.float64, device="cuda")
-    if world > 1:
-        tmax = t_all.clone()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        tsum = t_all.clone()
-        dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
-        ms, e2e_ms = float(tmax[0]), float(tmax[1])
-        iters_all, e2e_iters_all, launches_all = float(tsum[2]), float(tsum[3]), float(tsum[4])
-    else:
-        e2e_ms, iters_all, e2e_iters_all, launches_all = e2e_s * 1e3, float(iters_done), float(e2e_iters), float(launches)
+    ms, iters_all, launches_all = reduce_over_ranks(ms, float(iters_done), float(launches), world)
+    e2e_ms, e2e_iters_all, _ = reduce_over_ranks(e2e_s * 1e3, float(e2e_iters), 0.0, world)
 
     if rank == 0:
         value = iters_all / (ms * 1e-3)
