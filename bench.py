@@ -133,10 +133,14 @@ def hbm_peak():
 def ncu_traffic(kernel_key):
     """Per-launch DRAM bytes of the dominant kernel from the committed ncu --set full summary."""
     try:
-        with open(os.path.join(ROOT, "profiles", "roofline_traffic.json")) as f:
-            return json.load(f).get(kernel_key)
+        import csv
+        with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["kernel"] == kernel_key:
+                    return int(row["dram_bytes_per_launch"])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def time_oracle(prob, dt, b, iters):
