@@ -47,7 +47,10 @@ def parse():
     ap.add_argument("--loop-mode", type=int, default=None)
     ap.add_argument("--xfuse", type=int, default=None)
     ap.add_argument("--ci", type=int, default=None)
+    ap.add_argument("--serpentine", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--chain-steps", type=int, default=20,
+                    help="--workload c5: consecutive solves timed (BASELINE.json config 5 has 100)")
     return ap.parse_args()
 
 
@@ -192,8 +195,64 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_chain(args):
+    """BASELINE.json config 5, time-step proxy: consecutive warm-started solves on 192x256x384, dt varying
+    +-20 % per step, RHS(k+1) = x(k) + 0.05 N(0,1).  Timed per solve with CUDA events (set_dt + solve);
+    RHS construction and its H2D copy are outside the timed regions."""
+    import numpy as np
+    import torch
+    from mas_inputs import configs
+    from paper_1811_02605_b200 import MasPcg
+    torch.cuda.set_device(0)
+    prob = configs.make("c5")
+    dt0 = prob.dt_for(prob.stiffness[-1])
+    chain = configs.Chain(prob, max(args.chain_steps, 1))
+    gpu = MasPcg(prob.mesh, dt0, prob.nu_kind, prob.nu, prob.bc)
+    stream = torch.cuda.current_stream()
+    x = torch.zeros(prob.mesh.shape, dtype=torch.float64, device="cuda")
+    rhs = torch.from_numpy(chain.state0 + chain.noise()).cuda()
+    # warm-up on a scratch vector (graph build, clocks)
+    xs = torch.zeros_like(x)
+    for _ in range(max(args.warmup, 3)):
+        xs.zero_()
+        gpu.solve(rhs, xs, prob.rtol, prob.maxit, want_hist=False)
+    total_ms, iters, launches = 0.0, [], 0
+    for step in range(args.chain_steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        gpu.set_dt(dt0 * chain.dt_factor[step])
+        st, k, _ = gpu.solve(rhs, x, prob.rtol, prob.maxit, want_hist=False)      # x: warm start, in place
+        e1.record(stream)
+        torch.cuda.synchronize()
+        total_ms += e0.elapsed_time(e1)
+        iters.append(k)
+        sstat = gpu.stats()
+        launches += sstat["loop_launches"] + sstat["other_launches"] + 1
+        if st != 0:
+            raise SystemExit(f"chain step {step}: status {st}")
+        rhs = x + torch.from_numpy(chain.noise()).cuda()                           # untimed
+    n = prob.mesh.ncells
+    bpc = gpu.stats()["bytes_per_cell_iter"]
+    line = {"metric": "pcg_solves_per_s_192x256x384_timestep_proxy", "value": args.chain_steps / (total_ms * 1e-3),
+            "unit": "solves/s", "n_gpus": 1, "steps": args.chain_steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": total_ms / args.chain_steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"c5: 192x256x384 fp64, s=100 at dt0, dt +-20 %/step, warm start, rtol 1e-9, "
+                                   f"first {args.chain_steps} of 100 chained solves",
+                       "mean_iters_per_solve": float(np.mean(iters)), "iters": iters,
+                       "bytes_per_cell_iter": bpc},
+            "iterations_per_s": float(np.sum(iters)) / (total_ms * 1e-3),
+            "model_gbs": bpc * n * float(np.sum(iters)) / (total_ms * 1e-3) / 1e9,
+            "gpu_launches": int(launches)}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
+    if args.impl == "ours" and args.workload == "c5":
+        run_chain(args)
+        return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -230,6 +289,8 @@ def main():
         gpu.set_option("xfuse", args.xfuse)
     if args.ci is not None:
         gpu.set_option("ci", args.ci)
+    if args.serpentine is not None:
+        gpu.set_option("serpentine", args.serpentine)
     b_host = torch.from_numpy(b_np).pin_memory()
     x_host = torch.zeros(prob.mesh.shape, dtype=torch.float64).pin_memory()
     b = b_host.cuda()

@@ -196,8 +196,12 @@ __global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditio
 // hist[k], beta, convergence test, graph conditional.  6N doubles of traffic.
 // ---------------------------------------------------------------------------------------------
 // XF = true: the x-update lives in K1 (deferred one iteration), K2 only touches r and q: 3N doubles.
+// `reverse`: sweep the rows from the last to the first (serpentine: K1 marches forward in r, so the
+// planes it touched last -- q, r -- are still in L2 when K2 starts there, and K2's last rows are in L2
+// when the next K1 starts at i = 0).  The row -> block -> partial mapping stays fixed, so determinism holds.
 template <int NT, bool UNIFORM, bool XF>
-__global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond)
+__global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond,
+                                             int reverse)
 {
     __shared__ double sh[32];
     State *st = w.st;
@@ -207,39 +211,57 @@ __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditio
     double *x = w.args->x;
     const RowMap m = row_map<NT>(op.nv);
     double acc[2] = {0.0, 0.0};   // rho', rr
-    if (!m.idle)
-        for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
-            const int row = rowbase + m.rl;
-            if (row >= op.nrows) break;
-            double E = 0, F = 0, dinv = 0;
-            if (UNIFORM) dinv = __ldg(op.Dinv + row);
-            else { E = __ldg(op.E + row); F = __ldg(op.F + row); }
-            const size_t base = (size_t)row * op.np;
+    // Two row groups per trip (A and B, one grid stride apart): their loads are issued together, which
+    // doubles the bytes in flight per thread -- K2 has no other latency hiding than memory parallelism.
+    auto body = [&](int row, int kv, double2 rv, double2 qv, double2 xv, double2 pv, double E, double F, double dinv) {
+        const size_t cell = (size_t)row * op.np + 2 * kv;
+        if (!XF) {
+            xv.x = fma(alpha, pv.x, xv.x);
+            xv.y = fma(alpha, pv.y, xv.y);
+            st2(x, cell, xv);
+        }
+        rv.x = fma(-alpha, qv.x, rv.x);
+        rv.y = fma(-alpha, qv.y, rv.y);
+        st2(w.r, cell, rv);
+        double z0, z1;
+        if (UNIFORM) { z0 = rv.x * dinv; z1 = rv.y * dinv; }
+        else {
+            const int k = 2 * kv;
+            z0 = rv.x / fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k));
+            z1 = rv.y / fma(__ldg(op.vp + k + 1), E, F * __ldg(op.wp + k + 1));
+        }
+        acc[0] += rv.x * z0 + rv.y * z1;
+        acc[1] += rv.x * rv.x + rv.y * rv.y;
+    };
+    if (!m.idle) {
+        const int stride = gridDim.x * m.rb;
+        const double2 zero = make_double2(0.0, 0.0);
+        for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += 2 * stride) {
+            int rowA = rowbase + m.rl, rowB = rowA + stride;
+            const bool okA = rowA < op.nrows, okB = rowB < op.nrows;
+            if (!okA) break;
+            if (reverse) { rowA = op.nrows - 1 - rowA; rowB = op.nrows - 1 - rowB; }
+            double EA = 0, FA = 0, dA = 0, EB = 0, FB = 0, dB = 0;
+            if (UNIFORM) { dA = __ldg(op.Dinv + rowA); if (okB) dB = __ldg(op.Dinv + rowB); }
+            else {
+                EA = __ldg(op.E + rowA); FA = __ldg(op.F + rowA);
+                if (okB) { EB = __ldg(op.E + rowB); FB = __ldg(op.F + rowB); }
+            }
+            const size_t baseA = (size_t)rowA * op.np, baseB = okB ? (size_t)rowB * op.np : 0;
             for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
-                const size_t cell = base + 2 * kv;
-                double2 rv = ld2(w.r, cell);
-                const double2 qv = ld2(w.q, cell);
+                const size_t cA = baseA + 2 * kv, cB = baseB + 2 * kv;
+                const double2 rA = ld2(w.r, cA), qA = ld2(w.q, cA);
+                const double2 rB = okB ? ld2(w.r, cB) : zero, qB = okB ? ld2(w.q, cB) : zero;
+                double2 xA = zero, pA = zero, xB = zero, pB = zero;
                 if (!XF) {
-                    double2 xv = ld2(x, cell);
-                    const double2 pv = ld2(p, cell);
-                    xv.x = fma(alpha, pv.x, xv.x);
-                    xv.y = fma(alpha, pv.y, xv.y);
-                    st2(x, cell, xv);
+                    xA = ld2(x, cA); pA = ld2(p, cA);
+                    if (okB) { xB = ld2(x, cB); pB = ld2(p, cB); }
                 }
-                rv.x = fma(-alpha, qv.x, rv.x);
-                rv.y = fma(-alpha, qv.y, rv.y);
-                st2(w.r, cell, rv);
-                double z0, z1;
-                if (UNIFORM) { z0 = rv.x * dinv; z1 = rv.y * dinv; }
-                else {
-                    const int k = 2 * kv;
-                    z0 = rv.x / fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k));
-                    z1 = rv.y / fma(__ldg(op.vp + k + 1), E, F * __ldg(op.wp + k + 1));
-                }
-                acc[0] += rv.x * z0 + rv.y * z1;
-                acc[1] += rv.x * rv.x + rv.y * rv.y;
+                body(rowA, kv, rA, qA, xA, pA, EA, FA, dA);
+                if (okB) body(rowB, kv, rB, qB, xB, pB, EB, FB, dB);
             }
         }
+    }
     if (grid_sum<NT, 2>(acc, w.partials, &st->ticket[2], sh) && threadIdx.x == 0) {
         const double rho1 = acc[0], rr = acc[1];
         const int k = st->k + 1;

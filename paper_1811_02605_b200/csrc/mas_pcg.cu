@@ -75,6 +75,7 @@ struct mas_pcg {
     int variant = 2;                 // K1 variant: 0 baseline, 1 marching tiles (64 wide), 2 wide marching tiles
     int tile = 0;                    // tile configuration id of the variant
     int ci_force = 0;                // >0: override the r-chunk length (tuning)
+    int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
     int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
@@ -295,6 +296,7 @@ struct LoopCtx {                     // storage that kernel argument pointers re
     Work work;
     cudaGraphConditionalHandle cond;
     int use_cond;
+    int reverse;
     const double *xin;
     const SolveArgs *args;
     double *y;
@@ -352,8 +354,9 @@ KLaunch make_k2(const mas_pcg *h, LoopCtx &c)
         k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true, false> : (const void *)k2_vec<NT_BASE, false, false>;
     k.block = dim3(NT_BASE);
     k.grid = dim3(base_grid(h, k.func, NT_BASE));
-    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
-    k.nargs = 4;
+    c.reverse = h->serpentine;
+    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond; k.args[4] = &c.reverse;
+    k.nargs = 5;
     return k;
 }
 
@@ -516,6 +519,9 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
         const int nt_ = h->variant == 1 ? march_num_tiles() : (h->variant == 2 ? wide_num_tiles() : 1);
         if (value < 0 || value >= nt_) return MAS_EINVAL;
         h->tile = value;
+    } else if (!strcmp(name, "serpentine")) {
+        if (value != 0 && value != 1) return MAS_EINVAL;
+        h->serpentine = value;
     } else if (!strcmp(name, "xfuse")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->xfuse = value;
