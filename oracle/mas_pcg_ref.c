@@ -268,3 +268,92 @@ done:
     free(d); free(r); free(z); free(p); free(q);
     return status;
 }
+
+/* ==============================================================================================
+ * NEXT-1: the explicit alternative to the viscosity PCG solve -- "a Runge-Kutta
+ * Legendre super time-stepping (STS) scheme [21]" (~200 sub-steps per step, PAPER.md:80;
+ * the fastest GPU choice).  The paper gives no formulas; R7 restates the
+ * second-order scheme RKL2 of its reference [21] (Meyer, Balsara & Aslam, J. Comput. Phys. 257, 2014):
+ *
+ *   du/dt = M u,   M u = -(1/V) sum_f G_f (u_c - u_nb)      [FD form of div(nu grad u); A_phys = I - dt M]
+ *   b_0 = b_1 = b_2 = 1/3,  b_j = (j^2 + j - 2) / (2 j (j + 1)),  a_j = 1 - b_j,  w_1 = 4 / (s^2 + s - 2)
+ *   Y_0 = u,   Y_1 = Y_0 + mu~_1 tau M Y_0,                      mu~_1 = b_1 w_1
+ *   Y_j = mu_j Y_{j-1} + nu_j Y_{j-2} + (1 - mu_j - nu_j) Y_0 + mu~_j tau M Y_{j-1} + gamma~_j tau M Y_0
+ *   mu_j = (2j-1)/j * b_j/b_{j-1},  nu_j = -(j-1)/j * b_j/b_{j-2},  mu~_j = mu_j w_1,  gamma~_j = -a_{j-1} mu~_j
+ *   u <- Y_s.      Stable for tau <= (s^2 + s - 2)/4 * 2/lambda_max.
+ * Pinned by tests/test_oracle_sts_pins.py: the closed-form stability polynomial
+ * R_s(z) = a_s + b_s P_s(1 + w_1 z) (Legendre P_s) on eigenvectors, third-order local error against
+ * the matrix exponential, conservation, stability at the limit.
+ * ============================================================================================== */
+
+/* y = M u */
+void mas_ref_lop(const ref_op *op, const double *u, double *y)
+{
+    const int nr = op->nr, nt = op->nt, np = op->np;
+    double g[6];
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j < nt; j++)
+            for (int k = 0; k < np; k++) {
+                const size_t c = ((size_t)i * nt + j) * np + k;
+                const int kp = (k + 1) % np, km = (k + np - 1) % np;
+                faces(op, i, j, k, g);
+                const double uc = u[c];
+                const double u_im = i > 0      ? u[c - (size_t)nt * np] : 0.0;
+                const double u_ip = i < nr - 1 ? u[c + (size_t)nt * np] : 0.0;
+                const double u_jm = j > 0      ? u[c - np] : 0.0;
+                const double u_jp = j < nt - 1 ? u[c + np] : 0.0;
+                const double flux = g[0] * (uc - u_im) + g[1] * (uc - u_ip) + g[2] * (uc - u_jm)
+                                  + g[3] * (uc - u_jp) + g[4] * (uc - u[c - k + km]) + g[5] * (uc - u[c - k + kp]);
+                y[c] = -flux / volume(op, i, j, k);
+            }
+}
+
+/* Gershgorin bound on the spectral radius of M: max over cells of 2 (sum of face conductances) / V */
+double mas_ref_lambda_max_bound(const ref_op *op)
+{
+    double g[6], m = 0.0;
+    for (int i = 0; i < op->nr; i++)
+        for (int j = 0; j < op->nt; j++)
+            for (int k = 0; k < op->np; k++) {
+                faces(op, i, j, k, g);
+                const double s = 2.0 * (g[0] + g[1] + g[2] + g[3] + g[4] + g[5]) / volume(op, i, j, k);
+                if (s > m) m = s;
+            }
+    return m;
+}
+
+static double rkl2_b(int j) { return j < 3 ? 1.0 / 3.0 : ((double)j * j + j - 2.0) / (2.0 * j * (j + 1.0)); }
+
+/* one RKL2 super-step of size tau with s >= 2 stages, in place */
+int mas_ref_sts(const ref_op *op, double *u, double tau, int s)
+{
+    if (!op || !u || s < 2 || !(tau >= 0.0)) return REF_EINVAL;
+    const size_t n = (size_t)op->nr * op->nt * op->np;
+    double *y0 = (double *)malloc(n * sizeof(double)), *my0 = (double *)malloc(n * sizeof(double));
+    double *yjm2 = (double *)malloc(n * sizeof(double)), *yjm1 = (double *)malloc(n * sizeof(double));
+    double *yj = (double *)malloc(n * sizeof(double)), *my = (double *)malloc(n * sizeof(double));
+    int status = REF_ENOMEM;
+    if (!y0 || !my0 || !yjm2 || !yjm1 || !yj || !my) goto done;
+    const double w1 = 4.0 / ((double)s * s + s - 2.0);
+    memcpy(y0, u, n * sizeof(double));
+    mas_ref_lop(op, y0, my0);
+    const double mut1 = rkl2_b(1) * w1;
+    for (size_t c = 0; c < n; c++) yjm1[c] = y0[c] + mut1 * tau * my0[c];      /* Y_1 */
+    memcpy(yjm2, y0, n * sizeof(double));                                       /* Y_0 */
+    for (int j = 2; j <= s; j++) {
+        const double bj = rkl2_b(j), bjm1 = rkl2_b(j - 1), bjm2 = rkl2_b(j - 2);
+        const double mu = (2.0 * j - 1.0) / j * bj / bjm1;
+        const double nu = -(j - 1.0) / j * bj / bjm2;
+        const double mut = mu * w1;
+        const double gat = -(1.0 - bjm1) * mut;
+        mas_ref_lop(op, yjm1, my);
+        for (size_t c = 0; c < n; c++)
+            yj[c] = mu * yjm1[c] + nu * yjm2[c] + (1.0 - mu - nu) * y0[c] + mut * tau * my[c] + gat * tau * my0[c];
+        double *t = yjm2; yjm2 = yjm1; yjm1 = yj; yj = t;
+    }
+    memcpy(u, yjm1, n * sizeof(double));
+    status = REF_OK;
+done:
+    free(y0); free(my0); free(yjm2); free(yjm1); free(yj); free(my);
+    return status;
+}

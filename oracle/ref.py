@@ -50,6 +50,11 @@ def lib():
         L.mas_ref_pcg.restype = ctypes.c_int
         L.mas_ref_pcg.argtypes = [ctypes.c_void_p, _dp, _dp, ctypes.c_double, ctypes.c_int,
                                   ctypes.POINTER(ctypes.c_int), _dp]
+        L.mas_ref_lop.argtypes = [ctypes.c_void_p, _dp, _dp]
+        L.mas_ref_lambda_max_bound.restype = ctypes.c_double
+        L.mas_ref_lambda_max_bound.argtypes = [ctypes.c_void_p]
+        L.mas_ref_sts.restype = ctypes.c_int
+        L.mas_ref_sts.argtypes = [ctypes.c_void_p, _dp, ctypes.c_double, ctypes.c_int]
         _lib = L
     return _lib
 
@@ -113,6 +118,25 @@ class RefOperator:
         it = ctypes.c_int(0)
         st = lib().mas_ref_pcg(self._h, _p(b), _p(x), float(rtol), int(maxit), ctypes.byref(it), _p(hist))
         return st, it.value, x, hist[: it.value + 1].copy()
+
+    # ---- NEXT-1: explicit operator and RKL2 super time stepping ----
+    def lop(self, u: np.ndarray) -> np.ndarray:
+        """M u = -(1/V) sum_f G_f (u_c - u_nb): the FD form of div(nu grad u)."""
+        u = np.ascontiguousarray(u, dtype=np.float64).reshape(self.shape)
+        y = np.empty(self.shape)
+        lib().mas_ref_lop(self._h, _p(u), _p(y))
+        return y
+
+    def lambda_max_bound(self) -> float:
+        return float(lib().mas_ref_lambda_max_bound(self._h))
+
+    def sts(self, u: np.ndarray, tau: float, s: int) -> np.ndarray:
+        """One RKL2 super-step of size tau with s stages; returns the new field."""
+        y = np.array(u, dtype=np.float64, order="C").reshape(self.shape)
+        st = lib().mas_ref_sts(self._h, _p(y), float(tau), int(s))
+        if st != REF_OK:
+            raise ValueError(f"mas_ref_sts status {st}")
+        return y
 
     def dense(self) -> np.ndarray:
         """Dense A_sym, column by column from unit vectors (tiny meshes only)."""
