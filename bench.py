@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "sts"])
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--tile", type=int, default=None)
     ap.add_argument("--loop-mode", type=int, default=None)
@@ -248,10 +248,71 @@ def run_chain(args):
     print(json.dumps(line), flush=True)
 
 
+def run_sts(args):
+    """NEXT-1: RKL2 super time stepping of the viscosity term on the 256x256x512 mesh of config 4 (same nu),
+    one super-step of 200 stages per step ("~200 sub-steps per time-step"), tau at 90 % of the
+    stability limit.  Algorithmic traffic per stage: Y_{j-1}, Y_{j-2}, Y_0, M Y_0 -> Y_j = 5 doubles per cell."""
+    import numpy as np
+    import torch
+    from mas_inputs import configs
+    from paper_1811_02605_b200 import MasPcg
+    torch.cuda.set_device(0)
+    prob = configs.make("c4")
+    S = 200
+    gpu = MasPcg(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
+    tau = 0.9 * (S * S + S - 2.0) / 4.0 * 2.0 / gpu.lambda_max()
+    u0 = torch.from_numpy(configs.rhs_uniform(prob)).cuda()
+    u = u0.clone()
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        u.copy_(u0)
+        gpu.sts_advance(u, tau, S)
+    sampler = ClockSampler(0)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ms = 0.0
+    for _ in range(args.steps):
+        u.copy_(u0)                                   # untimed reset
+        torch.cuda.synchronize()
+        e0.record(stream)
+        gpu.sts_advance(u, tau, S)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms += e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    n = prob.mesh.ncells
+    stage_ms = ms / (args.steps * S)
+    alg = (5.0 * (S - 1) + 3.0) / S * 8 * n            # bytes per stage, averaged (stage 1 moves 3N)
+    peak, peak_src = hbm_peak()
+    gbs = alg / (stage_ms * 1e-3) / 1e9
+    line = {"metric": "rkl2_sts_stages_per_s_256x256x512", "value": 1e3 / stage_ms, "unit": "stages/s", "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "sts: 256x256x512 fp64, nu(r) of config 4, one RKL2 super-step of 200 stages, "
+                                   "tau = 0.9 tau_max", "l2": "inputs larger than L2"},
+            "clocks": clocks, "gpu_launches": args.steps * S,
+            "roofline": {"bound": "hbm", "kernel": "k_stencil<EPI_STS>", "achieved": gbs, "peak": peak, "unit": "GB/s",
+                         "frac": gbs / peak, "traffic": ncu_traffic("k_stencil_sts"), "peak_source": peak_src}}
+    if not args.no_cpu_baseline:
+        from oracle import ref
+        op = ref.RefOperator(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
+        ub = configs.rhs_uniform(prob)
+        t0 = time.perf_counter()
+        op.sts(ub, tau * 1e-3, 6)
+        t = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": 6 / t, "unit": "stages/s", "cores": 1, "kind": "oracle",
+                                "sample": "one RKL2 super-step of 6 stages on the same mesh, one host thread, gcc -O2"}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
     if args.impl == "ours" and args.workload == "c5":
         run_chain(args)
+        return
+    if args.impl == "ours" and args.workload == "sts":
+        run_sts(args)
         return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

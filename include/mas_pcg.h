@@ -108,9 +108,30 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
 /* Tuning / debugging knob, takes effect at the next solve.  name in
  *   "loop_mode" (0 host chunks, 1 graph while), "variant" (K1: 0 baseline, 1 marching, 2 wide marching),
  *   "tile" (tile configuration of the variant), "ci" (r-chunk length, 0 = automatic),
- *   "xfuse" (1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B).  See DESIGN.md.
+ *   "xfuse" (1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B), "serpentine" (K2 sweeps
+ *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile".  See DESIGN.md.
  * Unknown name or value: MAS_EINVAL. */
 int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value);
+
+/* ---- NEXT-1: the explicit alternative for the viscosity term, "a Runge-Kutta Legendre super
+ * time-stepping (STS) scheme [21]" (~200 sub-steps per step; the fastest GPU
+ * choice).  M u = -(1/V) sum_faces G_f (u - u_nb) is the FD form of div(nu grad u), so that
+ * A_phys = I - dt M.  Scheme: RKL2 of the paper's ref. [21], restated in DESIGN.md R7. ---- */
+
+/* y = M u (asynchronous on `stream`); u_dev != y_dev, DEVICE vectors of N doubles. */
+int mas_pcg_lop(mas_pcg_t *h, const double *u_dev, double *y_dev, void *stream);
+
+/* *out = Gershgorin bound on the spectral radius of M (HOST double), computed at create. */
+int mas_pcg_lambda_max(const mas_pcg_t *h, double *out);
+
+/* Smallest stage count s >= 2 for which one RKL2 super-step of size tau is stable:
+ * tau <= (s^2 + s - 2)/4 * 2/lambda_max. */
+int mas_sts_stages(const mas_pcg_t *h, double tau, int *s_out);
+
+/* Advance du/dt = M u by ONE RKL2 super-step of size tau with s >= 2 stages, in place in u_dev (DEVICE).
+ * s kernel launches on `stream`, asynchronous.  Uses the handle's PCG workspaces as stage buffers, so it
+ * must not overlap a solve on the same handle. */
+int mas_sts_advance(mas_pcg_t *h, double *u_dev, double tau, int s, void *stream);
 
 void mas_pcg_destroy(mas_pcg_t *h);            /* NULL is allowed                                 */
 

@@ -60,6 +60,14 @@ def _load():
     L.mas_pcg_apply.argtypes = [vp, vp, vp, vp]
     L.mas_pcg_profile.restype = ctypes.c_int
     L.mas_pcg_profile.argtypes = [vp, vp, vp, ctypes.c_int, vp, _dp]
+    L.mas_pcg_lop.restype = ctypes.c_int
+    L.mas_pcg_lop.argtypes = [vp, vp, vp, vp]
+    L.mas_pcg_lambda_max.restype = ctypes.c_int
+    L.mas_pcg_lambda_max.argtypes = [vp, _dp]
+    L.mas_sts_stages.restype = ctypes.c_int
+    L.mas_sts_stages.argtypes = [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int)]
+    L.mas_sts_advance.restype = ctypes.c_int
+    L.mas_sts_advance.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp]
     L.mas_pcg_stats.restype = ctypes.c_int
     L.mas_pcg_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong)]
     L.mas_pcg_set_option.restype = ctypes.c_int
@@ -162,6 +170,34 @@ def mas_pcg_profile(handle, b_ptr, x_ptr, nit, stream=0):
     if st != MAS_OK:
         raise MasError(st, "mas_pcg_profile")
     return {"k1_ms": out[0], "k2_ms": out[1], "k1_min_ms": out[2], "k2_min_ms": out[3]}
+
+
+def mas_pcg_lop(handle, u_ptr, y_ptr, stream=0):
+    st = lib().mas_pcg_lop(handle, u_ptr, y_ptr, stream)
+    if st != MAS_OK:
+        raise MasError(st, "mas_pcg_lop")
+
+
+def mas_pcg_lambda_max(handle) -> float:
+    out = ctypes.c_double(0.0)
+    st = lib().mas_pcg_lambda_max(handle, ctypes.byref(out))
+    if st != MAS_OK:
+        raise MasError(st, "mas_pcg_lambda_max")
+    return out.value
+
+
+def mas_sts_stages(handle, tau) -> int:
+    out = ctypes.c_int(0)
+    st = lib().mas_sts_stages(handle, float(tau), ctypes.byref(out))
+    if st != MAS_OK:
+        raise MasError(st, "mas_sts_stages")
+    return out.value
+
+
+def mas_sts_advance(handle, u_ptr, tau, s, stream=0):
+    st = lib().mas_sts_advance(handle, u_ptr, float(tau), int(s), stream)
+    if st != MAS_OK:
+        raise MasError(st, "mas_sts_advance")
 
 
 def mas_pcg_stats(handle):

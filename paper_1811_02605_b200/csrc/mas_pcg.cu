@@ -15,6 +15,7 @@
 #include "common.cuh"
 #include "kernels_base.cuh"
 #include "kernels_march.cuh"
+#include "kernels_stencil.cuh"
 
 using namespace mas;
 
@@ -58,7 +59,8 @@ struct mas_pcg {
     double dt = 0.0;
     int uniform_phi = 0;
     // device planes
-    DevBuf<double> V2, SD, CP, CRoff, CT, E, F, AR, AT, Dinv, vp, wp, ip;
+    DevBuf<double> V2, SD, CP, CRoff, CT, E, F, AR, AT, Dinv, vp, wp, ip, Vinv;
+    double lambda_max = 0.0;         // Gershgorin bound on the spectral radius of M = -V^-1 L_sym
     double vp0 = 0, wp0 = 0, ip0 = 0;
     // workspaces
     DevBuf<double> r, p0, p1, q, partials, hist, bdev, xdev;
@@ -75,6 +77,8 @@ struct mas_pcg {
     int variant = 2;                 // K1 variant: 0 baseline, 1 marching tiles (64 wide), 2 wide marching tiles
     int tile = 0;                    // tile configuration id of the variant
     int ci_force = 0;                // >0: override the r-chunk length (tuning)
+    int apply_variant = 1;           // 1: k_stencil marching kernel for A x (apply / initial residual); 0: k_apply
+    int stencil_tile = 0;
     int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
     int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
     cudaGraph_t graph = nullptr;
@@ -165,7 +169,7 @@ extern "C" void mas_pcg_destroy(mas_pcg_t *h)
     if (h->exec) cudaGraphExecDestroy(h->exec);
     if (h->graph) cudaGraphDestroy(h->graph);
     DevBuf<double> *bufs[] = {&h->V2, &h->SD, &h->CP, &h->CRoff, &h->CT, &h->E, &h->F, &h->AR, &h->AT, &h->Dinv,
-                              &h->vp, &h->wp, &h->ip, &h->r, &h->p0, &h->p1, &h->q, &h->partials, &h->hist,
+                              &h->vp, &h->wp, &h->ip, &h->Vinv, &h->r, &h->p0, &h->p1, &h->q, &h->partials, &h->hist,
                               &h->bdev, &h->xdev};
     for (DevBuf<double> *b : bufs) b->release();
     h->st.release();
@@ -254,6 +258,13 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
         if (m->dph_c[k] != m->dph_c[0] || m->dph_f[k] != m->dph_f[0]) h->uniform_phi = 0;
     }
     for (int k = 0; k < np; k++) wp[k] = ip[k] + ip[(k + np - 1) % np];
+    std::vector<double> Vinv(nrows);
+    double gmax = 0.0;                                      // max_k wp[k]/vp[k]
+    for (int k = 0; k < np; k++) gmax = fmax(gmax, wp[k] / vp[k]);
+    for (int t = 0; t < nrows; t++) {
+        Vinv[t] = 1.0 / V2[t];
+        h->lambda_max = fmax(h->lambda_max, 2.0 * (SD[t] + CP[t] * gmax) / V2[t]);
+    }
     h->vp0 = vp[0];
     h->wp0 = wp[0];
     h->ip0 = ip[0];
@@ -261,7 +272,7 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
     int rc;
     if ((rc = upload(h->V2, V2)) || (rc = upload(h->CP, CP)) || (rc = upload(h->SD, SD)) ||
         (rc = upload(h->CRoff, CRoff)) || (rc = upload(h->CT, CT)) || (rc = upload(h->vp, vp)) ||
-        (rc = upload(h->wp, wp)) || (rc = upload(h->ip, ip)))
+        (rc = upload(h->wp, wp)) || (rc = upload(h->ip, ip)) || (rc = upload(h->Vinv, Vinv)))
         return fail(h, rc);
     if (h->E.alloc(nrows) || h->F.alloc(nrows) || h->Dinv.alloc(nrows) || h->AR.alloc((size_t)(nr + 1) * nt) ||
         h->AT.alloc((size_t)nr * (nt + 1)) || h->r.alloc(h->n) || h->p0.alloc(h->n) || h->p1.alloc(h->n) ||
@@ -302,6 +313,7 @@ struct LoopCtx {                     // storage that kernel argument pointers re
     double *y;
     MarchParams mp;
     WideParams wp;
+    StencilParams sp;
 };
 
 int base_grid(const mas_pcg *h, const void *func, int nt_block)
@@ -322,9 +334,26 @@ int base_grid(const mas_pcg *h, const void *func, int nt_block)
     return (int)gsz;
 }
 
+void stencil_common(const mas_pcg *h, StencilParams &sp)
+{
+    memset(&sp, 0, sizeof(sp));
+    sp.vp = h->vp0; sp.wp = h->wp0; sp.ip = h->ip0;
+    sp.args = h->args.p;
+}
+
 KLaunch make_apply(const mas_pcg *h, LoopCtx &c)
 {
     KLaunch k;
+    if (h->apply_variant == 1) {                 // marching stencil kernel: S = A_sym (dt-scaled planes)
+        stencil_common(h, c.sp);
+        c.sp.E = h->E.p; c.sp.F = h->F.p; c.sp.AR = h->AR.p; c.sp.AT = h->AT.p;
+        c.sp.u = c.xin; c.sp.out = c.y;
+        stencil_configure(h->nr, h->nt, h->np, h->uniform_phi, EPI_APPLY, h->stencil_tile, h->num_sms, &c.sp, &k.func,
+                          &k.grid, &k.block, &k.smem);
+        k.args[0] = &c.op; k.args[1] = &c.sp;
+        k.nargs = 2;
+        return k;
+    }
     k.func = (const void *)k_apply<NT_BASE>;
     k.block = dim3(NT_BASE);
     k.grid = dim3(base_grid(h, k.func, NT_BASE));
@@ -519,6 +548,12 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
         const int nt_ = h->variant == 1 ? march_num_tiles() : (h->variant == 2 ? wide_num_tiles() : 1);
         if (value < 0 || value >= nt_) return MAS_EINVAL;
         h->tile = value;
+    } else if (!strcmp(name, "apply_variant")) {
+        if (value != 0 && value != 1) return MAS_EINVAL;
+        h->apply_variant = value;
+    } else if (!strcmp(name, "stencil_tile")) {
+        if (value < 0 || value >= stencil_num_tiles()) return MAS_EINVAL;
+        h->stencil_tile = value;
     } else if (!strcmp(name, "serpentine")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->serpentine = value;
@@ -665,5 +700,93 @@ extern "C" int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev,
     h->stats[4] = use_xfuse(h) ? 6 : 4;
     h->stats[5] = use_xfuse(h) ? 3 : 6;
     h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
+    return MAS_OK;
+}
+
+// =============================================================================================
+// NEXT-1: explicit viscosity advance by RKL2 super time stepping (R7)
+// =============================================================================================
+namespace {
+
+double rkl2_b(int j) { return j < 3 ? 1.0 / 3.0 : ((double)j * j + j - 2.0) / (2.0 * j * (j + 1.0)); }
+
+void sts_planes(const mas_pcg *h, StencilParams &sp)
+{
+    stencil_common(h, sp);                       // S = L_sym: the dt-independent planes
+    sp.E = h->SD.p; sp.F = h->CP.p; sp.AR = h->CRoff.p; sp.AT = h->CT.p; sp.Vinv = h->Vinv.p;
+}
+
+int launch_stencil(const mas_pcg *h, StencilParams &sp, int epi, cudaStream_t s)
+{
+    KLaunch k;
+    OpDev op = h->op;
+    stencil_configure(h->nr, h->nt, h->np, h->uniform_phi, epi, h->stencil_tile, h->num_sms, &sp, &k.func, &k.grid,
+                      &k.block, &k.smem);
+    k.args[0] = &op; k.args[1] = &sp;
+    CK(launch(k, s));
+    return MAS_OK;
+}
+
+}  // namespace
+
+extern "C" int mas_pcg_lambda_max(const mas_pcg_t *h, double *out)
+{
+    if (!h || !out) return MAS_EINVAL;
+    *out = h->lambda_max;
+    return MAS_OK;
+}
+
+extern "C" int mas_sts_stages(const mas_pcg_t *h, double tau, int *s_out)
+{
+    if (!h || !s_out || !(tau >= 0.0) || !isfinite(tau)) return MAS_EINVAL;
+    // stable iff tau <= (s^2 + s - 2)/4 * 2/lambda_max
+    const double need = 2.0 * tau * h->lambda_max;          // s^2 + s - 2 >= need
+    long long s = (long long)ceil(0.5 * (-1.0 + sqrt(9.0 + 4.0 * need)));
+    if (s < 2) s = 2;
+    while ((double)s * s + s - 2.0 < need) ++s;
+    if (s > (1LL << 30)) return MAS_EINVAL;
+    *s_out = (int)s;
+    return MAS_OK;
+}
+
+extern "C" int mas_pcg_lop(mas_pcg_t *h, const double *u_dev, double *y_dev, void *stream)
+{
+    if (!h || !u_dev || !y_dev || u_dev == y_dev || !aligned16(u_dev) || !aligned16(y_dev)) return MAS_EINVAL;
+    StencilParams sp;
+    sts_planes(h, sp);
+    sp.u = u_dev; sp.out = y_dev; sp.c_u = 0.0; sp.c_L = 1.0;     // out = M u
+    return launch_stencil(h, sp, EPI_STS, (cudaStream_t)stream);
+}
+
+extern "C" int mas_sts_advance(mas_pcg_t *h, double *u_dev, double tau, int s, void *stream)
+{
+    if (!h || !u_dev || !aligned16(u_dev) || s < 2 || !(tau >= 0.0) || !isfinite(tau)) return MAS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    double *my0 = h->q.p, *ya = h->p0.p, *yb = h->p1.p;           // the PCG workspaces double as stage buffers
+    const double w1 = 4.0 / ((double)s * s + s - 2.0);
+    StencilParams sp;
+    // stage 1: Y_1 = Y_0 + mu~_1 tau M Y_0 ; keep M Y_0
+    sts_planes(h, sp);
+    sp.u = u_dev; sp.out = ya; sp.out2 = my0; sp.c_u = 1.0; sp.c_L = rkl2_b(1) * w1 * tau;
+    int rc = launch_stencil(h, sp, EPI_STS, st);
+    if (rc != MAS_OK) return rc;
+    const double *yjm1 = ya, *yjm2 = u_dev;
+    for (int j = 2; j <= s; j++) {
+        const double bj = rkl2_b(j), bjm1 = rkl2_b(j - 1), bjm2 = rkl2_b(j - 2);
+        const double mu = (2.0 * j - 1.0) / j * bj / bjm1;
+        const double nu = -(j - 1.0) / j * bj / bjm2;
+        const double mut = mu * w1, gat = -(1.0 - bjm1) * mut;
+        // Y_j overwrites Y_{j-2}'s buffer (each cell is read by the thread that writes it), except that
+        // Y_0 = u_dev must survive until the last stage, which writes the result into it.
+        double *out = (j == s) ? u_dev : (yjm2 == u_dev ? yb : const_cast<double *>(yjm2));
+        sts_planes(h, sp);
+        sp.u = yjm1; sp.a1 = yjm2; sp.a2 = u_dev; sp.a3 = my0; sp.out = out;
+        sp.c_u = mu; sp.c_a1 = nu; sp.c_a2 = 1.0 - mu - nu; sp.c_L = mut * tau; sp.c_a3 = gat * tau;
+        rc = launch_stencil(h, sp, EPI_STS, st);
+        if (rc != MAS_OK) return rc;
+        yjm2 = yjm1;
+        yjm1 = out;
+    }
+    h->graph_dirty = h->graph_dirty;             // PCG workspaces were clobbered; solves re-initialise them
     return MAS_OK;
 }

@@ -64,5 +64,24 @@ class MasPcg:
     def profile(self, b: torch.Tensor, x: torch.Tensor, nit: int, stream=None):
         return B.mas_pcg_profile(self._h, _dev_ptr(b, self.n), _dev_ptr(x, self.n), nit, _stream_ptr(stream))
 
+    # ---- NEXT-1: explicit operator and RKL2 super time stepping ----
+    def lop(self, u: torch.Tensor, y: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+        """y = M u, the FD form of div(nu grad u)."""
+        if y is None:
+            y = torch.empty_like(u)
+        B.mas_pcg_lop(self._h, _dev_ptr(u, self.n), _dev_ptr(y, self.n), _stream_ptr(stream))
+        return y
+
+    def lambda_max(self) -> float:
+        return B.mas_pcg_lambda_max(self._h)
+
+    def sts_stages(self, tau: float) -> int:
+        return B.mas_sts_stages(self._h, tau)
+
+    def sts_advance(self, u: torch.Tensor, tau: float, s: int, stream=None) -> torch.Tensor:
+        """One RKL2 super-step of size tau with s stages, in place in u."""
+        B.mas_sts_advance(self._h, _dev_ptr(u, self.n), tau, s, _stream_ptr(stream))
+        return u
+
     def stats(self):
         return B.mas_pcg_stats(self._h)
