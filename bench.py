@@ -48,6 +48,7 @@ def parse():
     ap.add_argument("--xfuse", type=int, default=None)
     ap.add_argument("--ci", type=int, default=None)
     ap.add_argument("--serpentine", type=int, default=None)
+    ap.add_argument("--stencil-tile", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chain-steps", type=int, default=20,
                     help="--workload c5: consecutive solves timed (BASELINE.json config 5 has 100)")
@@ -260,6 +261,8 @@ def run_sts(args):
     prob = configs.make("c4")
     S = 200
     gpu = MasPcg(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
+    if args.stencil_tile is not None:
+        gpu.set_option("stencil_tile", args.stencil_tile)
     tau = 0.9 * (S * S + S - 2.0) / 4.0 * 2.0 / gpu.lambda_max()
     u0 = torch.from_numpy(configs.rhs_uniform(prob)).cuda()
     u = u0.clone()

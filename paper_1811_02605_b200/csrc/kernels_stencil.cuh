@@ -30,23 +30,25 @@ struct StencilParams {
     double c_u, c_a1, c_a2, c_L, c_a3;
 };
 
-template <int TJ, int DEPTH>
+template <int TJ, int DEPTH, int NX>      // NX = 6: extra streams through a cp.async FIFO; 0: none / via registers
 struct StencilSmem {
     static constexpr int NW = TJ + 2;
     static constexpr int NT = NW * 32;
     static constexpr int R = DEPTH + 2;
     static constexpr int NPL = MARCH_CI_MAX + 2;
+    double2 xf[NX ? DEPTH : 1][NX ? NX : 1][NX ? NT : 1];   // [stage][a1A a1B a2A a2B a3A a3B][thread]
     double2 ring[R][NW][64];              // planes of u: [slot][row][A lanes 0..31 | B lanes 32..63]
     double halo[R][NW][2];                // phi-halo cells of each row: [slot][row][left|right]
     double cE[NPL][NW], cF[NPL][NW], cAR[NPL][NW], cAT[NPL][NW], cV[NPL][NW];
     double phv[WIDE_TK + 2], phw[WIDE_TK + 2], phi[WIDE_TK + 2];
 };
 
-template <int TJ, int DEPTH, bool UNIFORM, int MINB, int EPI>
+template <int TJ, int DEPTH, bool UNIFORM, int MINB, int EPI, bool XFIFO>
 __global__ void __launch_bounds__((TJ + 2) * 32, MINB)
 k_stencil(OpDev op, StencilParams mp)
 {
-    using Smem = StencilSmem<TJ, DEPTH>;
+    static_assert(!XFIFO || (EPI == EPI_STS && DEPTH == 2), "extras FIFO: STS epilogue, DEPTH 2 (unroll = R = 4)");
+    using Smem = StencilSmem<TJ, DEPTH, XFIFO ? 6 : 0>;
     constexpr int NT = Smem::NT, NW = Smem::NW, R = Smem::R;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem &sm = *reinterpret_cast<Smem *>(smem_raw);
@@ -111,26 +113,40 @@ k_stencil(OpDev op, StencilParams mp)
     long long orow = rowbase0 + plane;              // row base (element offset) of plane i0: outputs / extras
     int ii_ld = first;
 
-    auto issue = [&](int slot) {
+    const bool has1 = EPI == EPI_STS && mp.a1 != nullptr, has2 = EPI == EPI_STS && mp.a2 != nullptr,
+               has3 = EPI == EPI_STS && mp.a3 != nullptr;
+    long long xoff = rowbase0 - plane;              // row base of plane ii_ld - 1: the plane whose outputs are
+                                                    // formed when ring plane ii_ld is consumed
+    auto issue = [&](int slot, int xstage) {
         if ((unsigned)ii_ld < (unsigned)op.nr && ii_ld <= i1) {
             if (vA) cp_async16(&sm.ring[slot][warp][lane], ldu + ka);
             if (vB) cp_async16(&sm.ring[slot][warp][lane + 32], ldu + kb);
             if (left_edge) cp_async8(&sm.halo[slot][warp][0], ldu + kl);
             if (right_edge) cp_async8(&sm.halo[slot][warp][1], ldu + kr);
         }
+        if (XFIFO && ii_ld - 1 >= i0 && ii_ld - 1 < i1) {
+            if (qA) {
+                if (has1) cp_async16(&sm.xf[xstage][0][tid], mp.a1 + xoff + ka);
+                if (has2) cp_async16(&sm.xf[xstage][2][tid], mp.a2 + xoff + ka);
+                if (has3) cp_async16(&sm.xf[xstage][4][tid], mp.a3 + xoff + ka);
+            }
+            if (qB) {
+                if (has1) cp_async16(&sm.xf[xstage][1][tid], mp.a1 + xoff + kb);
+                if (has2) cp_async16(&sm.xf[xstage][3][tid], mp.a2 + xoff + kb);
+                if (has3) cp_async16(&sm.xf[xstage][5][tid], mp.a3 + xoff + kb);
+            }
+        }
         cp_async_commit();
-        ldu += plane; ++ii_ld;
+        ldu += plane; xoff += plane; ++ii_ld;
     };
 #pragma unroll
-    for (int s = 0; s < DEPTH; s++) issue(s);
+    for (int s = 0; s < DEPTH; s++) issue(s, s % DEPTH);
 
     const double2 zero2 = make_double2(0.0, 0.0);
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
     double2 x1a = zero2, x1b = zero2, x2a = zero2, x2b = zero2, x3a = zero2, x3b = zero2;   // extras of the next plane
     const int lm = (lane + 31) & 31, lp = (lane + 1) & 31;
-    const bool has1 = EPI == EPI_STS && mp.a1 != nullptr, has2 = EPI == EPI_STS && mp.a2 != nullptr,
-               has3 = EPI == EPI_STS && mp.a3 != nullptr;
 
     for (int tb = 0; tb < nsteps; tb += R) {
 #pragma unroll
@@ -174,6 +190,15 @@ k_stencil(OpDev op, StencilParams mp)
                     }
                     st2(mp.out, orow + kcell, o);
                 };
+                // extras of this plane: the thread's own FIFO slots (landed with plane ii), or the registers
+                // loaded one step ahead.  Fresh locals, so nothing is carried across steps in FIFO mode.
+                const int xs = u % DEPTH;
+                const double2 e1a = XFIFO ? ((has1 && qA) ? sm.xf[xs][0][tid] : zero2) : x1a;
+                const double2 e1b = XFIFO ? ((has1 && qB) ? sm.xf[xs][1][tid] : zero2) : x1b;
+                const double2 e2a = XFIFO ? ((has2 && qA) ? sm.xf[xs][2][tid] : zero2) : x2a;
+                const double2 e2b = XFIFO ? ((has2 && qB) ? sm.xf[xs][3][tid] : zero2) : x2b;
+                const double2 e3a = XFIFO ? ((has3 && qA) ? sm.xf[xs][4][tid] : zero2) : x3a;
+                const double2 e3b = XFIFO ? ((has3 && qB) ? sm.xf[xs][5][tid] : zero2) : x3b;
                 if (qA) {
                     const double ukm = left_edge ? hl_c : mA;
                     const double ukp = right_A ? hr_c : (lane == 31 ? pB : pA);
@@ -184,7 +209,7 @@ k_stencil(OpDev op, StencilParams mp)
                     double2 s;
                     s.x = d0 * ac.x - VP(ea) * sx - Fc * (IP(ea) * ac.y + IP(ea - 1) * ukm);
                     s.y = d1 * ac.y - VP(ea + 1) * sy - Fc * (IP(ea + 1) * ukp + IP(ea) * ac.x);
-                    finish(s, ac, x1a, x2a, x3a, ea, ka);
+                    finish(s, ac, e1a, e2a, e3a, ea, ka);
                 }
                 if (qB) {
                     const double ukm = lane == 0 ? mA : mB;
@@ -196,12 +221,12 @@ k_stencil(OpDev op, StencilParams mp)
                     double2 s;
                     s.x = d0 * bc.x - VP(eb) * sx - Fc * (IP(eb) * bc.y + IP(eb - 1) * ukm);
                     s.y = d1 * bc.y - VP(eb + 1) * sy - Fc * (IP(eb + 1) * ukp + IP(eb) * bc.x);
-                    finish(s, bc, x1b, x2b, x3b, eb, kb);
+                    finish(s, bc, e1b, e2b, e3b, eb, kb);
                 }
             }
             if (t >= 2) orow += plane;
             // extras of plane ii (consumed at the next step): orow now points at plane ii when t >= 1
-            if (EPI == EPI_STS && t >= 1 && t <= nsteps - 2) {
+            if (EPI == EPI_STS && !XFIFO && t >= 1 && t <= nsteps - 2) {
                 if (qA) {
                     if (has1) x1a = ld2(mp.a1, orow + ka);
                     if (has2) x2a = ld2(mp.a2, orow + ka);
@@ -213,7 +238,7 @@ k_stencil(OpDev op, StencilParams mp)
                     if (has3) x3b = ld2(mp.a3, orow + kb);
                 }
             }
-            issue(slot_ld);
+            issue(slot_ld, u % DEPTH);
             __syncthreads();                          // plane ii complete for everyone; slot (t-2) free
             am = ac; ac = an; bm = bc; bc = bn;
             hl_c = hl_n; hr_c = hr_n;
@@ -225,30 +250,35 @@ k_stencil(OpDev op, StencilParams mp)
 // ---------------------------------------------------------------------------------------------
 // host-side configuration
 // ---------------------------------------------------------------------------------------------
-template <int TJ, int DEPTH, int MINB>
+template <int TJ, int DEPTH, int MINB, bool XFIFO>
 inline void stencil_pick(bool uniform, int epi, const void **func, dim3 *block, size_t *smem)
 {
-    if (epi == EPI_APPLY)
-        *func = uniform ? (const void *)k_stencil<TJ, DEPTH, true, MINB, EPI_APPLY>
-                        : (const void *)k_stencil<TJ, DEPTH, false, MINB, EPI_APPLY>;
-    else
-        *func = uniform ? (const void *)k_stencil<TJ, DEPTH, true, MINB, EPI_STS>
-                        : (const void *)k_stencil<TJ, DEPTH, false, MINB, EPI_STS>;
+    if (epi == EPI_APPLY) {
+        *func = uniform ? (const void *)k_stencil<TJ, DEPTH, true, MINB, EPI_APPLY, false>
+                        : (const void *)k_stencil<TJ, DEPTH, false, MINB, EPI_APPLY, false>;
+        *smem = sizeof(StencilSmem<TJ, DEPTH, 0>);
+    } else {
+        *func = uniform ? (const void *)k_stencil<TJ, DEPTH, true, MINB, EPI_STS, XFIFO>
+                        : (const void *)k_stencil<TJ, DEPTH, false, MINB, EPI_STS, XFIFO>;
+        *smem = sizeof(StencilSmem<TJ, DEPTH, XFIFO ? 6 : 0>);
+    }
     *block = dim3((TJ + 2) * 32);
-    *smem = sizeof(StencilSmem<TJ, DEPTH>);
     cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);
 }
 
-inline int stencil_num_tiles() { return 3; }
+inline int stencil_num_tiles() { return 6; }
 
 inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int tile, int num_sms, StencilParams *mp,
                               const void **func, dim3 *grid, dim3 *block, size_t *smem)
 {
     int tj;
     switch (tile) {
-        case 0: tj = 8; stencil_pick<8, 2, 2>(uniform, epi, func, block, smem); break;
-        case 1: tj = 8; stencil_pick<8, 3, 2>(uniform, epi, func, block, smem); break;
-        default: tj = 14; stencil_pick<14, 2, 1>(uniform, epi, func, block, smem); break;
+        case 0: tj = 6; stencil_pick<6, 2, 2, true>(uniform, epi, func, block, smem); break;
+        case 1: tj = 8; stencil_pick<8, 2, 2, false>(uniform, epi, func, block, smem); break;
+        case 2: tj = 14; stencil_pick<14, 2, 1, false>(uniform, epi, func, block, smem); break;
+        case 3: tj = 4; stencil_pick<4, 2, 3, true>(uniform, epi, func, block, smem); break;
+        case 4: tj = 8; stencil_pick<8, 2, 1, true>(uniform, epi, func, block, smem); break;
+        default: tj = 8; stencil_pick<8, 3, 2, false>(uniform, epi, func, block, smem); break;
     }
     mp->nkt = (np + WIDE_TK - 1) / WIDE_TK;
     mp->njt = (nt + tj - 1) / tj;

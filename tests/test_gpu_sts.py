@@ -17,7 +17,7 @@ def _t(a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2])
+@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("shape,bc", [((9, 11, 70), (0, 0)), ((21, 19, 134), (1, 0)), ((1, 1, 2), (0, 0)),
                                       ((5, 17, 260), (1, 1)), ((40, 9, 128), (0, 1))])
 def test_lop_and_apply_match_oracle_general_mesh(shape, bc, tile):
@@ -47,9 +47,10 @@ def test_lop_uniform_phi_and_baseline_apply_kernel_agree():
         assert np.abs(a - a_ref).max() <= H.APPLY_RTOL * np.abs(a_ref).max()
 
 
+@pytest.mark.parametrize("tile", [0, 1, 3, 4])
 @pytest.mark.parametrize("s", [2, 3, 5, 16, 64])
 @pytest.mark.parametrize("uniform", [False, True])
-def test_sts_advance_matches_oracle(s, uniform):
+def test_sts_advance_matches_oracle(s, uniform, tile):
     if uniform:
         prob = configs.make("c3", shape=(24, 21, 128))
         mesh, nu_kind, nu, bc = prob.mesh, prob.nu_kind, prob.nu, (0, 0)
@@ -59,6 +60,7 @@ def test_sts_advance_matches_oracle(s, uniform):
         bc = (0, 1)
         u = np.random.default_rng(5).standard_normal(mesh.shape)
     oref, gpu = H.both_ops(mesh, 1.0, nu_kind, nu, bc)
+    gpu.set_option("stencil_tile", tile)
     lam = gpu.lambda_max()
     lim = lambda n: (n * n + n - 2.0) / 4.0 * 2.0 / lam        # largest stable tau with n stages
     tau = 0.5 * (lim(s - 1) + lim(s)) if s > 2 else 0.9 * lim(2)  # needs exactly s stages
