@@ -224,12 +224,12 @@ struct WideParams {
     double vp, wp, ip;                        // uniform-phi factors (dph_c, 2/dph_f, 1/dph_f)
 };
 
-template <int TJ, int DEPTH>
+template <int TJ, int DEPTH, bool XF>
 struct WideSmem {
     static constexpr int NW = TJ + 2;
     static constexpr int NT = NW * 32;
     static constexpr int NPL = MARCH_CI_MAX + 2;
-    double2 fifo[DEPTH][4][NT];               // [stage][rA rB pA pB][thread]
+    double2 fifo[DEPTH][XF ? 6 : 4][NT];      // [stage][rA rB pA pB (xA xB)][thread]
     double hfifo[DEPTH][4][NW];               // [stage][r_left r_right p_left p_right][warp]
     double2 ring[3][NW][64];                  // p_new planes: [buffer][row][A lanes 0..31 | B lanes 32..63]
     double cE[NPL][NW], cF[NPL][NW], cD[NPL][NW], cAR[NPL][NW], cAT[NPL][NW];
@@ -241,7 +241,7 @@ template <int TJ, int DEPTH, bool UNIFORM, int MINB, bool XF>
 __global__ void __launch_bounds__((TJ + 2) * 32, MINB)
 k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int use_cond)
 {
-    using Smem = WideSmem<TJ, DEPTH>;
+    using Smem = WideSmem<TJ, DEPTH, XF>;
     constexpr int NT = Smem::NT, NW = Smem::NW;
     constexpr int U = (DEPTH % 3 == 0) ? DEPTH : 3 * DEPTH;     // unroll: stage and ring index static
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -301,7 +301,7 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
 #pragma unroll
     for (int s = 0; s < DEPTH; s++) {
 #pragma unroll
-        for (int a = 0; a < 4; a++) sm.fifo[s][a][tid] = make_double2(0.0, 0.0);
+        for (int a = 0; a < (XF ? 6 : 4); a++) sm.fifo[s][a][tid] = make_double2(0.0, 0.0);
         if (lane < 4) sm.hfifo[s][lane][warp] = 0.0;
     }
     __syncthreads();
@@ -324,7 +324,7 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
     double *stp = pout + rowbase0 + plane;          // row base of plane i0 (first store of p)
     double *stq = w.q + rowbase0 + plane;           // row base of plane i0 (first store of q)
     double *xrow = XF ? xvec + rowbase0 + plane : nullptr;   // row base of plane i0 (x is updated in place)
-    double2 xa = make_double2(0.0, 0.0), xb = xa;   // x of the NEXT interior plane, loaded one step ahead
+    const double *ldx = XF ? xvec + rowbase0 : nullptr;       // x rides in the FIFO with r and p_old of its plane
     int ii_ld = first;                              // plane index of the next prefetch
 
     auto issue = [&](int stage) {
@@ -333,9 +333,14 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
             if (vB) { cp_async16(&sm.fifo[stage][1][tid], ldr + kb); cp_async16(&sm.fifo[stage][3][tid], ldp + kb); }
             if (left_edge) { cp_async8(&sm.hfifo[stage][0][warp], ldr + kl); cp_async8(&sm.hfifo[stage][2][warp], ldp + kl); }
             if (right_edge) { cp_async8(&sm.hfifo[stage][1][warp], ldr + kr); cp_async8(&sm.hfifo[stage][3][warp], ldp + kr); }
+            if (XF && ii_ld >= i0 && ii_ld < i1) {              // interior plane: its x
+                if (qA) cp_async16(&sm.fifo[stage][XF ? 4 : 0][tid], ldx + ka);
+                if (qB) cp_async16(&sm.fifo[stage][XF ? 5 : 0][tid], ldx + kb);
+            }
         }
         cp_async_commit();
         ldr += plane; ldp += plane; ++ii_ld;
+        if (XF) ldx += plane;
     };
 
 #pragma unroll
@@ -376,15 +381,19 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
                     if (qB) st2(stp, kb, bn);
                     stp += plane;
                     if (XF) {
-                        if (qA) { xa.x = fma(alpha_prev, pa.x, xa.x); xa.y = fma(alpha_prev, pa.y, xa.y); st2(xrow, ka, xa); }
-                        if (qB) { xb.x = fma(alpha_prev, pb.x, xb.x); xb.y = fma(alpha_prev, pb.y, xb.y); st2(xrow, kb, xb); }
+                        if (qA) {
+                            double2 xa = sm.fifo[stage][XF ? 4 : 0][tid];
+                            xa.x = fma(alpha_prev, pa.x, xa.x); xa.y = fma(alpha_prev, pa.y, xa.y);
+                            st2(xrow, ka, xa);
+                        }
+                        if (qB) {
+                            double2 xb = sm.fifo[stage][XF ? 5 : 0][tid];
+                            xb.x = fma(alpha_prev, pb.x, xb.x); xb.y = fma(alpha_prev, pb.y, xb.y);
+                            st2(xrow, kb, xb);
+                        }
                         xrow += plane;
                     }
                 }
-            }
-            if (XF && t <= nsteps - 3) {            // x of the next step's (interior) plane
-                if (qA) xa = ld2(xrow, ka);
-                if (qB) xb = ld2(xrow, kb);
             }
             issue(stage);
             sm.ring[rbw][warp][lane] = an;
@@ -491,7 +500,7 @@ inline void wide_pick(bool uniform, bool xf, const void **func, dim3 *block, siz
     else
         *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, false> : (const void *)k1_wide<TJ, DEPTH, false, MINB, false>;
     *block = dim3((TJ + 2) * 32);
-    *smem = sizeof(WideSmem<TJ, DEPTH>);
+    *smem = xf ? sizeof(WideSmem<TJ, DEPTH, true>) : sizeof(WideSmem<TJ, DEPTH, false>);
     cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);
 }
 
