@@ -49,6 +49,8 @@ def parse():
     ap.add_argument("--ci", type=int, default=None)
     ap.add_argument("--serpentine", type=int, default=None)
     ap.add_argument("--stencil-tile", type=int, default=None)
+    ap.add_argument("--qrecompute", type=int, default=None)
+    ap.add_argument("--k2r-tile", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chain-steps", type=int, default=20,
                     help="--workload c5: consecutive solves timed (BASELINE.json config 5 has 100)")
@@ -355,6 +357,10 @@ def main():
         gpu.set_option("ci", args.ci)
     if args.serpentine is not None:
         gpu.set_option("serpentine", args.serpentine)
+    if args.qrecompute is not None:
+        gpu.set_option("qrecompute", args.qrecompute)
+    if args.k2r_tile is not None:
+        gpu.set_option("k2r_tile", args.k2r_tile)
     b_host = torch.from_numpy(b_np).pin_memory()
     x_host = torch.zeros(prob.mesh.shape, dtype=torch.float64).pin_memory()
     b = b_host.cuda()

@@ -196,6 +196,24 @@ __global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditio
 // hist[k], beta, convergence test, graph conditional.  6N doubles of traffic.
 // ---------------------------------------------------------------------------------------------
 // XF = true: the x-update lives in K1 (deferred one iteration), K2 only touches r and q: 3N doubles.
+// the last block of every K2 variant ends with this (S5): k++, hist[k], beta, convergence test
+__device__ __forceinline__ void k2_finish(State *st, const Work &w, double rho1, double rr,
+                                          cudaGraphConditionalHandle cond, int use_cond)
+{
+    const int k = st->k + 1;
+    const double h = sqrt(rr / st->bb);
+    w.hist[k] = h;
+    st->beta = rho1 / st->rho;
+    st->rho = rho1;
+    st->rr = rr;
+    st->k = k;
+    st->launches += 1;
+    const int active = (k < w.args->maxit) && (h > w.args->rtol) && (rho1 != 0.0);
+    if (!active) st->status = (h <= w.args->rtol || rho1 == 0.0) ? ST_OK : ST_MAXIT;
+    st->active = active;
+    set_cond(cond, use_cond, active);
+}
+
 // `reverse`: sweep the rows from the last to the first (serpentine: K1 marches forward in r, so the
 // planes it touched last -- q, r -- are still in L2 when K2 starts there, and K2's last rows are in L2
 // when the next K1 starts at i = 0).  The row -> block -> partial mapping stays fixed, so determinism holds.
@@ -262,21 +280,8 @@ __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditio
             }
         }
     }
-    if (grid_sum<NT, 2>(acc, w.partials, &st->ticket[2], sh) && threadIdx.x == 0) {
-        const double rho1 = acc[0], rr = acc[1];
-        const int k = st->k + 1;
-        const double h = sqrt(rr / st->bb);
-        w.hist[k] = h;
-        st->beta = rho1 / st->rho;
-        st->rho = rho1;
-        st->rr = rr;
-        st->k = k;
-        st->launches += 1;
-        const int active = (k < w.args->maxit) && (h > w.args->rtol) && (rho1 != 0.0);
-        if (!active) st->status = (h <= w.args->rtol || rho1 == 0.0) ? ST_OK : ST_MAXIT;
-        st->active = active;
-        set_cond(cond, use_cond, active);
-    }
+    if (grid_sum<NT, 2>(acc, w.partials, &st->ticket[2], sh) && threadIdx.x == 0)
+        k2_finish(st, w, acc[0], acc[1], cond, use_cond);
 }
 
 // XF tail (after the loop): the one x-update still pending, x += alpha_{k-1} p_{k-1}.  alpha is 0 when

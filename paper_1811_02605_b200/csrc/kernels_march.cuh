@@ -237,7 +237,8 @@ struct WideSmem {
     double red[32];
 };
 
-template <int TJ, int DEPTH, bool UNIFORM, int MINB, bool XF>
+// NOQ: q is not stored (K2R recomputes it from p_new): K1 then moves 5 doubles per cell.
+template <int TJ, int DEPTH, bool UNIFORM, int MINB, bool XF, bool NOQ>
 __global__ void __launch_bounds__((TJ + 2) * 32, MINB)
 k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int use_cond)
 {
@@ -416,7 +417,7 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
                     double2 q;
                     q.x = d0 * ac.x - VP(ea) * sx - Fc * (IP(ea) * ac.y + IP(ea - 1) * ukm);
                     q.y = d1 * ac.y - VP(ea + 1) * sy - Fc * (IP(ea + 1) * ukp + IP(ea) * ac.x);
-                    st2(stq, ka, q);
+                    if (!NOQ) st2(stq, ka, q);
                     acc += ac.x * q.x + ac.y * q.y;
                 }
                 if (qB) {
@@ -429,7 +430,7 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
                     double2 q;
                     q.x = d0 * bc.x - VP(eb) * sx - Fc * (IP(eb) * bc.y + IP(eb - 1) * ukm);
                     q.y = d1 * bc.y - VP(eb + 1) * sy - Fc * (IP(eb + 1) * ukp + IP(eb) * bc.x);
-                    st2(stq, kb, q);
+                    if (!NOQ) st2(stq, kb, q);
                     acc += bc.x * q.x + bc.y * q.y;
                 }
             }
@@ -493,12 +494,14 @@ static const WideTile kWideTiles[] = {{8, 2, 2}, {6, 3, 2}, {6, 2, 3}, {14, 3, 1
 inline int wide_num_tiles() { return (int)(sizeof(kWideTiles) / sizeof(kWideTiles[0])); }
 
 template <int TJ, int DEPTH, int MINB>
-inline void wide_pick(bool uniform, bool xf, const void **func, dim3 *block, size_t *smem)
+inline void wide_pick(bool uniform, int xf, const void **func, dim3 *block, size_t *smem)
 {
-    if (xf)
-        *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, true> : (const void *)k1_wide<TJ, DEPTH, false, MINB, true>;
+    if (xf == 2)        // xfuse + q not stored
+        *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, true, true> : (const void *)k1_wide<TJ, DEPTH, false, MINB, true, true>;
+    else if (xf)
+        *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, true, false> : (const void *)k1_wide<TJ, DEPTH, false, MINB, true, false>;
     else
-        *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, false> : (const void *)k1_wide<TJ, DEPTH, false, MINB, false>;
+        *func = uniform ? (const void *)k1_wide<TJ, DEPTH, true, MINB, false, false> : (const void *)k1_wide<TJ, DEPTH, false, MINB, false, false>;
     *block = dim3((TJ + 2) * 32);
     *smem = xf ? sizeof(WideSmem<TJ, DEPTH, true>) : sizeof(WideSmem<TJ, DEPTH, false>);
     cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);

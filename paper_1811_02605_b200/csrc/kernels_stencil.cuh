@@ -16,7 +16,7 @@
 
 namespace mas {
 
-enum { EPI_APPLY = 0, EPI_STS = 1 };
+enum { EPI_APPLY = 0, EPI_STS = 1, EPI_K2R = 2 };   // K2R: PCG's K2 with q = A p recomputed (64 B/cell/it)
 
 struct StencilParams {
     int nkt, njt, nit, ci;
@@ -28,6 +28,11 @@ struct StencilParams {
     double *out, *out2;
     const double *a1, *a2, *a3;           // EPI_STS: Y_{j-2}, Y_0, M Y_0 (null = absent)
     double c_u, c_a1, c_a2, c_L, c_a3;
+    // EPI_K2R
+    Work w;
+    const double *Dinv;
+    cudaGraphConditionalHandle cond;
+    int use_cond;
 };
 
 template <int TJ, int DEPTH, int NX>      // NX = 6: extra streams through a cp.async FIFO; 0: none / via registers
@@ -41,19 +46,28 @@ struct StencilSmem {
     double halo[R][NW][2];                // phi-halo cells of each row: [slot][row][left|right]
     double cE[NPL][NW], cF[NPL][NW], cAR[NPL][NW], cAT[NPL][NW], cV[NPL][NW];
     double phv[WIDE_TK + 2], phw[WIDE_TK + 2], phi[WIDE_TK + 2];
+    double red[32];
 };
 
 template <int TJ, int DEPTH, bool UNIFORM, int MINB, int EPI, bool XFIFO>
 __global__ void __launch_bounds__((TJ + 2) * 32, MINB)
 k_stencil(OpDev op, StencilParams mp)
 {
-    static_assert(!XFIFO || (EPI == EPI_STS && DEPTH == 2), "extras FIFO: STS epilogue, DEPTH 2 (unroll = R = 4)");
-    using Smem = StencilSmem<TJ, DEPTH, XFIFO ? 6 : 0>;
+    static_assert(!XFIFO || (EPI != EPI_APPLY && DEPTH == 2), "extras FIFO: STS / K2R epilogue, DEPTH 2 (unroll = R = 4)");
+    static_assert(EPI != EPI_K2R || XFIFO, "K2R takes r through the FIFO");
+    using Smem = StencilSmem<TJ, DEPTH, XFIFO ? (EPI == EPI_K2R ? 2 : 6) : 0>;
     constexpr int NT = Smem::NT, NW = Smem::NW, R = Smem::R;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem &sm = *reinterpret_cast<Smem *>(smem_raw);
 
-    const double *__restrict__ uvec = mp.u ? mp.u : mp.args->x;
+    double alpha = 0.0;
+    const double *uk2 = nullptr;
+    if (EPI == EPI_K2R) {                            // u = p written by K1 of this iteration; r updated in place
+        if (!mp.w.st->active) return;
+        alpha = mp.w.st->alpha;
+        uk2 = (mp.w.st->k & 1) ? mp.w.p0 : mp.w.p1;
+    }
+    const double *__restrict__ uvec = EPI == EPI_K2R ? uk2 : (mp.u ? mp.u : mp.args->x);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
     int b = blockIdx.x;
     const int kt = b % mp.nkt; b /= mp.nkt;
@@ -82,7 +96,7 @@ k_stencil(OpDev op, StencilParams mp)
         const int row = ii * op.nt + jj;
         sm.cE[pl][wr] = in ? __ldg(mp.E + row) : 0.0;
         sm.cF[pl][wr] = in ? __ldg(mp.F + row) : 0.0;
-        sm.cV[pl][wr] = (in && EPI == EPI_STS) ? __ldg(mp.Vinv + row) : 0.0;
+        sm.cV[pl][wr] = (in && EPI == EPI_STS) ? __ldg(mp.Vinv + row) : ((in && EPI == EPI_K2R) ? __ldg(mp.Dinv + row) : 0.0);
         sm.cAR[pl][wr] = (ii >= 0 && ii <= op.nr && jj >= 0 && jj < op.nt) ? __ldg(mp.AR + row) : 0.0;
         sm.cAT[pl][wr] = (ii >= 0 && ii < op.nr && jj >= 0 && jj <= op.nt) ? __ldg(mp.AT + ii * (op.nt + 1) + jj) : 0.0;
     }
@@ -113,8 +127,10 @@ k_stencil(OpDev op, StencilParams mp)
     long long orow = rowbase0 + plane;              // row base (element offset) of plane i0: outputs / extras
     int ii_ld = first;
 
-    const bool has1 = EPI == EPI_STS && mp.a1 != nullptr, has2 = EPI == EPI_STS && mp.a2 != nullptr,
-               has3 = EPI == EPI_STS && mp.a3 != nullptr;
+    const double *a1p = EPI == EPI_K2R ? mp.w.r : mp.a1;          // K2R: the one extra stream is r
+    const bool has1 = (EPI == EPI_STS && mp.a1 != nullptr) || EPI == EPI_K2R,
+               has2 = EPI == EPI_STS && mp.a2 != nullptr, has3 = EPI == EPI_STS && mp.a3 != nullptr;
+    double acc[2] = {0.0, 0.0};                                  // K2R: rho', rr
     long long xoff = rowbase0 - plane;              // row base of plane ii_ld - 1: the plane whose outputs are
                                                     // formed when ring plane ii_ld is consumed
     auto issue = [&](int slot, int xstage) {
@@ -126,12 +142,12 @@ k_stencil(OpDev op, StencilParams mp)
         }
         if (XFIFO && ii_ld - 1 >= i0 && ii_ld - 1 < i1) {
             if (qA) {
-                if (has1) cp_async16(&sm.xf[xstage][0][tid], mp.a1 + xoff + ka);
+                if (has1) cp_async16(&sm.xf[xstage][0][tid], a1p + xoff + ka);
                 if (has2) cp_async16(&sm.xf[xstage][2][tid], mp.a2 + xoff + ka);
                 if (has3) cp_async16(&sm.xf[xstage][4][tid], mp.a3 + xoff + ka);
             }
             if (qB) {
-                if (has1) cp_async16(&sm.xf[xstage][1][tid], mp.a1 + xoff + kb);
+                if (has1) cp_async16(&sm.xf[xstage][1][tid], a1p + xoff + kb);
                 if (has2) cp_async16(&sm.xf[xstage][3][tid], mp.a2 + xoff + kb);
                 if (has3) cp_async16(&sm.xf[xstage][5][tid], mp.a3 + xoff + kb);
             }
@@ -172,11 +188,19 @@ k_stencil(OpDev op, StencilParams mp)
                 const double Ec = sm.cE[t - 1][warp], Fc = sm.cF[t - 1][warp];
                 const double ARm = sm.cAR[t - 1][warp], ARp = sm.cAR[t][warp];
                 const double ATm = sm.cAT[t - 1][warp], ATp = sm.cAT[t - 1][warp + 1];
-                const double vinv = EPI == EPI_STS ? sm.cV[t - 1][warp] : 0.0;
+                const double vinv = EPI != EPI_APPLY ? sm.cV[t - 1][warp] : 0.0;
                 auto finish = [&](double2 s, double2 uc, double2 x1, double2 x2, double2 x3, int e, int kcell) {
                     double2 o;
                     if (EPI == EPI_APPLY) {
                         o = s;
+                    } else if (EPI == EPI_K2R) {                     // s = q = A p;  x1 = r
+                        o.x = fma(-alpha, s.x, x1.x);
+                        o.y = fma(-alpha, s.y, x1.y);
+                        double z0, z1;
+                        if (UNIFORM) { z0 = o.x * vinv; z1 = o.y * vinv; }     // vinv holds Dinv here
+                        else { z0 = o.x / fma(VP(e), Ec, Fc * WP(e)); z1 = o.y / fma(VP(e + 1), Ec, Fc * WP(e + 1)); }
+                        acc[0] += o.x * z0 + o.y * z1;
+                        acc[1] += o.x * o.x + o.y * o.y;
                     } else {
                         double2 mu;                                  // M u = -S u / (V2 vp)
                         mu.x = UNIFORM ? -(s.x * vinv) * (1.0 / mp.vp) : -(s.x * vinv) / VP(e);
@@ -188,7 +212,7 @@ k_stencil(OpDev op, StencilParams mp)
                         if (has2) { o.x = fma(mp.c_a2, x2.x, o.x); o.y = fma(mp.c_a2, x2.y, o.y); }
                         if (has3) { o.x = fma(mp.c_a3, x3.x, o.x); o.y = fma(mp.c_a3, x3.y, o.y); }
                     }
-                    st2(mp.out, orow + kcell, o);
+                    st2(EPI == EPI_K2R ? mp.w.r : mp.out, orow + kcell, o);
                 };
                 // extras of this plane: the thread's own FIFO slots (landed with plane ii), or the registers
                 // loaded one step ahead.  Fresh locals, so nothing is carried across steps in FIFO mode.
@@ -245,6 +269,10 @@ k_stencil(OpDev op, StencilParams mp)
         }
     }
     cp_async_wait<0>();
+    if (EPI == EPI_K2R) {
+        if (grid_sum<NT, 2>(acc, mp.w.partials, &mp.w.st->ticket[2], sm.red) && threadIdx.x == 0)
+            k2_finish(mp.w.st, mp.w, acc[0], acc[1], mp.cond, mp.use_cond);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -257,6 +285,10 @@ inline void stencil_pick(bool uniform, int epi, const void **func, dim3 *block, 
         *func = uniform ? (const void *)k_stencil<TJ, DEPTH, true, MINB, EPI_APPLY, false>
                         : (const void *)k_stencil<TJ, DEPTH, false, MINB, EPI_APPLY, false>;
         *smem = sizeof(StencilSmem<TJ, DEPTH, 0>);
+    } else if (epi == EPI_K2R) {
+        *func = uniform ? (const void *)k_stencil<TJ, 2, true, MINB, EPI_K2R, true>
+                        : (const void *)k_stencil<TJ, 2, false, MINB, EPI_K2R, true>;
+        *smem = sizeof(StencilSmem<TJ, 2, 2>);
     } else {
         *func = uniform ? (const void *)k_stencil<TJ, DEPTH, true, MINB, EPI_STS, XFIFO>
                         : (const void *)k_stencil<TJ, DEPTH, false, MINB, EPI_STS, XFIFO>;
@@ -292,6 +324,7 @@ inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int 
     double best_cost = 1e300;
     for (int ci = MARCH_CI_MAX; ci >= 4; ci -= 2) {
         const long long tiles = cols * ((nr + ci - 1) / ci);
+        if (epi == EPI_K2R && tiles > MAX_PARTIALS) continue;
         const double rounds = (double)((tiles + slots - 1) / slots);
         const double cost = rounds * (ci + 2 + 3);
         if (cost < best_cost * 0.999) { best_cost = cost; best = ci; }

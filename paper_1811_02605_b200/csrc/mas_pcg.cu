@@ -79,7 +79,9 @@ struct mas_pcg {
     int ci_force = 0;                // >0: override the r-chunk length (tuning)
     int apply_variant = 1;           // 1: k_stencil marching kernel for A x (apply / initial residual); 0: k_apply
     int stencil_tile = 0;
+    int k2r_tile = 0;
     int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
+    int qrecompute = 0;              // 1 (needs xfuse, wide): q is not stored, K2 recomputes it: 64 B/cell/iteration
     int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
@@ -313,7 +315,7 @@ struct LoopCtx {                     // storage that kernel argument pointers re
     double *y;
     MarchParams mp;
     WideParams wp;
-    StencilParams sp;
+    StencilParams sp, sp2;
 };
 
 int base_grid(const mas_pcg *h, const void *func, int nt_block)
@@ -333,6 +335,9 @@ int base_grid(const mas_pcg *h, const void *func, int nt_block)
     if (gsz < 1) gsz = 1;
     return (int)gsz;
 }
+
+bool use_xfuse(const mas_pcg *h) { return h->xfuse && h->variant == 2; }
+bool use_qrec(const mas_pcg *h) { return h->qrecompute && use_xfuse(h); }
 
 void stencil_common(const mas_pcg *h, StencilParams &sp)
 {
@@ -376,6 +381,16 @@ KLaunch make_init(const mas_pcg *h, LoopCtx &c)
 KLaunch make_k2(const mas_pcg *h, LoopCtx &c)
 {
     KLaunch k;
+    if (use_qrec(h)) {                           // marching stencil kernel: q = A p recomputed, r updated in place
+        stencil_common(h, c.sp2);
+        c.sp2.E = h->E.p; c.sp2.F = h->F.p; c.sp2.AR = h->AR.p; c.sp2.AT = h->AT.p; c.sp2.Dinv = h->Dinv.p;
+        c.sp2.w = c.work; c.sp2.cond = c.cond; c.sp2.use_cond = c.use_cond;
+        stencil_configure(h->nr, h->nt, h->np, h->uniform_phi, EPI_K2R, h->k2r_tile, h->num_sms, &c.sp2, &k.func,
+                          &k.grid, &k.block, &k.smem);
+        k.args[0] = &c.op; k.args[1] = &c.sp2;
+        k.nargs = 2;
+        return k;
+    }
     const bool xf = h->xfuse && h->variant == 2;
     if (xf)
         k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true, true> : (const void *)k2_vec<NT_BASE, false, true>;
@@ -400,7 +415,7 @@ KLaunch make_xtail(const mas_pcg *h, LoopCtx &c)
     return k;
 }
 
-bool use_xfuse(const mas_pcg *h) { return h->xfuse && h->variant == 2; }
+
 
 KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
 {
@@ -418,7 +433,7 @@ KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
                         &k.smem);
         k.args[2] = &c.mp;
     } else {
-        wide_configure(h->nr, h->nt, h->np, h->uniform_phi, use_xfuse(h), h->tile, h->num_sms, h->ci_force, &c.wp,
+        wide_configure(h->nr, h->nt, h->np, h->uniform_phi, use_qrec(h) ? 2 : (use_xfuse(h) ? 1 : 0), h->tile, h->num_sms, h->ci_force, &c.wp,
                        &k.func, &k.grid, &k.block, &k.smem);
         c.wp.vp = h->vp0; c.wp.wp = h->wp0; c.wp.ip = h->ip0;
         k.args[2] = &c.wp;
@@ -557,6 +572,12 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
     } else if (!strcmp(name, "serpentine")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->serpentine = value;
+    } else if (!strcmp(name, "qrecompute")) {
+        if (value != 0 && value != 1) return MAS_EINVAL;
+        h->qrecompute = value;
+    } else if (!strcmp(name, "k2r_tile")) {
+        if (value < 0 || value >= stencil_num_tiles()) return MAS_EINVAL;
+        h->k2r_tile = value;
     } else if (!strcmp(name, "xfuse")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->xfuse = value;
@@ -637,7 +658,7 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     h->stats[1] = launched_outside;
     h->stats[2] = mode;
     // unfused: K1 r,p -> p,q (4N); K2 x,p,r,q -> x,r (6N).  xfuse: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)
-    h->stats[4] = use_xfuse(h) ? 6 : 4;
+    h->stats[4] = use_qrec(h) ? 5 : (use_xfuse(h) ? 6 : 4);
     h->stats[5] = use_xfuse(h) ? 3 : 6;
     h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
     return st.status;
@@ -697,7 +718,7 @@ extern "C" int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev,
     }
     for (cudaEvent_t &e : ev) cudaEventDestroy(e);
     ms_out[0] = sum1 / nit; ms_out[1] = sum2 / nit; ms_out[2] = min1; ms_out[3] = min2;
-    h->stats[4] = use_xfuse(h) ? 6 : 4;
+    h->stats[4] = use_qrec(h) ? 5 : (use_xfuse(h) ? 6 : 4);
     h->stats[5] = use_xfuse(h) ? 3 : 6;
     h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
     return MAS_OK;
