@@ -14,8 +14,11 @@
 //     registers held;
 //   * p_new of the current plane goes to a 3-plane shared ring for the theta neighbours; phi
 //     neighbours come by warp shuffle, r neighbours stay in registers across steps;
-//   * the phi-halo cells (k0-1, k0+64; periodic wrap) are two scalar loads by the edge lanes.
+//   * the phi-halo cells (k0-1, k0+64; periodic wrap) ride in the same FIFO as 8-byte cp.async copies
+//     issued by the edge lanes; the block's coefficient columns are staged in shared memory once.
 // Each cell's r and p_old are read from DRAM once; halo rows/planes are L2 hits.
+// k1_march (64-cell rows, "variant 1") is kept as the validated predecessor of k1_wide ("variant 2",
+// further down), which is the default.
 // p is double-buffered in global memory (p[k&1] -> p[(k+1)&1]) because neighbouring blocks read
 // p_old halos while this block writes p_new.
 #pragma once

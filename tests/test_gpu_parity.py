@@ -251,3 +251,43 @@ def test_rerun_bit_identity_every_kernel_family(variant, tile, xfuse):
         st, k, h = gpu.solve(b, x, 0.0, 60)
         runs.append((k, h.tobytes(), x.cpu().numpy().tobytes()))
     assert all(r == runs[0] for r in runs[1:])
+
+
+# ------------------------------------------------------------------ large meshes: byte offsets beyond 4 GiB
+def test_large_mesh_64bit_offsets_closed_forms():
+    """320 x 1024 x 2048 = 671 M cells, 5.4 GB per vector (N < 2^31 is the documented maximum; element offsets
+    fit 32 bits, byte offsets do not).  The oracle cannot run this in seconds, so the checks are properties that
+    hold at any size: with Neumann radial faces A_sym 1 = V exactly (P5) and M 1 = 0; and after a few PCG
+    iterations the recurrence residual equals the true residual b_s - A x."""
+    import torch
+    from mas_inputs import grids
+    from paper_1811_02605_b200 import MasPcg
+    nr, nt, np_ = 320, 1024, 2048
+    if torch.cuda.mem_get_info()[0] < 60e9:
+        pytest.skip("needs ~45 GB of free device memory")
+    mesh = grids.full_sphere_mesh(grids.radial_faces_pack(nr, 4.0), nt, np_)
+    nu = configs.nu_profile(mesh)
+    gpu = MasPcg(mesh, 1e-3, 1, nu, (1, 1))
+    V = (torch.from_numpy(mesh.r_c ** 2 * mesh.dr_c)[:, None, None]
+         * torch.from_numpy(mesh.sin_c * mesh.dth_c)[None, :, None]
+         * torch.from_numpy(mesh.dph_c)[None, None, :]).cuda()
+    one = torch.ones(mesh.shape, dtype=torch.float64, device="cuda")
+    y = gpu.apply(one)
+    assert float(((y - V).abs() / V).max()) <= 1e-12
+    gpu.lop(one, y)
+    lam = gpu.lambda_max()
+    assert float(y.abs().max()) <= 1e-12 * lam
+    del one
+    # a few iterations: true residual == recurrence residual, also at the far end of the arrays
+    g = torch.Generator(device="cuda").manual_seed(7)
+    b = torch.rand(mesh.shape, dtype=torch.float64, device="cuda", generator=g) * 2 - 1
+    gpu.set_dt(50.0 / lam)
+    x = torch.zeros_like(b)
+    st, k, h = gpu.solve(b, x, 0.0, 5)
+    assert (st, k) == (1, 5) and np.isfinite(h).all() and (np.diff(h) != 0).all()
+    gpu.apply(x, y)                       # y = A x
+    y.neg_().add_(V * b)                  # true residual b_s - A x
+    bs_norm = float((V * b).norm())
+    assert float(y.norm()) / bs_norm == pytest.approx(h[-1], rel=1e-9)
+    # last plane was really updated (a wrapped 32-bit byte offset would leave it untouched)
+    assert float(x[-1].abs().max()) > 0 and float(x[0].abs().max()) > 0
