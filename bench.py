@@ -50,6 +50,7 @@ def parse():
     ap.add_argument("--serpentine", type=int, default=None)
     ap.add_argument("--stencil-tile", type=int, default=None)
     ap.add_argument("--qrecompute", type=int, default=None)
+    ap.add_argument("--persistent", type=int, default=None)
     ap.add_argument("--k2r-tile", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chain-steps", type=int, default=20,
@@ -359,6 +360,8 @@ def main():
         gpu.set_option("serpentine", args.serpentine)
     if args.qrecompute is not None:
         gpu.set_option("qrecompute", args.qrecompute)
+    if args.persistent is not None:
+        gpu.set_option("persistent", args.persistent)
     if args.k2r_tile is not None:
         gpu.set_option("k2r_tile", args.k2r_tile)
     b_host = torch.from_numpy(b_np).pin_memory()
@@ -392,6 +395,7 @@ def main():
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
     stats = gpu.stats()
+    loop_mode = stats["loop_mode"]
 
     # ---------------- end to end through the C ABI with host buffers ----------------
     gpu.solve_host(b_host, x_host.zero_(), rtol, maxit, want_hist=False)          # warm (allocates staging)
@@ -430,7 +434,7 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": desc, "parallelism": "replicas only" if world > 1 else "1 gpu",
                        "l2": "inputs larger than L2 (5 live vectors x %.0f MB vs 126 MB)" % (8 * n / 1e6),
-                       "loop_mode": "cuda-graph while" if stats["loop_mode"] == 1 else "host chunks",
+                       "loop_mode": {0: "host chunks", 1: "cuda-graph while", 2: "persistent cooperative kernel"}[loop_mode],
                        "bytes_per_cell_iter": bpc, "status": st, "iters_per_step": k},
             "clocks": clocks,
             "e2e": {"value": e2e_iters_all / (e2e_ms * 1e-3), "unit": UNIT,

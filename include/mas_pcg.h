@@ -100,7 +100,7 @@ int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev, int nit, v
 
 /* Fills HOST array out[8] with counters of the last solve:
  *   [0] kernels launched inside the iteration loop, [1] kernels launched outside it,
- *   [2] loop mode used (1 = CUDA-graph WHILE node, 0 = host-driven chunks),
+ *   [2] loop mode used (1 = CUDA-graph WHILE node, 0 = host-driven chunks, 2 = one persistent cooperative kernel),
  *   [3] algorithmic bytes per cell per iteration of the kernels in use,
  *   [4] doubles per cell K1 moves, [5] doubles per cell K2 moves, [6..7] reserved (0). */
 int mas_pcg_stats(const mas_pcg_t *h, long long *out);
@@ -109,7 +109,8 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
  *   "loop_mode" (0 host chunks, 1 graph while), "variant" (K1: 0 baseline, 1 marching, 2 wide marching),
  *   "tile" (tile configuration of the variant), "ci" (r-chunk length, 0 = automatic),
  *   "xfuse" (1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B), "serpentine" (K2 sweeps
- *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile".  See DESIGN.md.
+ *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile", "qrecompute" (64 B),
+ *   "persistent" (small meshes: whole solve in one cooperative kernel; 0 off, 1 whenever it fits, 2 auto).
  * Unknown name or value: MAS_EINVAL. */
 int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value);
 

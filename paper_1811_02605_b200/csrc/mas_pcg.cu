@@ -16,6 +16,7 @@
 #include "kernels_base.cuh"
 #include "kernels_march.cuh"
 #include "kernels_stencil.cuh"
+#include "kernels_persistent.cuh"
 
 using namespace mas;
 
@@ -81,6 +82,8 @@ struct mas_pcg {
     int stencil_tile = 0;
     int k2r_tile = 0;
     int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
+    int persistent = 2;              // one cooperative kernel for the whole solve: 0 off, 1 whenever it fits, 2 auto
+    int coop_ok = 0;
     int qrecompute = 0;              // 1 (needs xfuse, wide): q is not stored, K2 recomputes it: 64 B/cell/iteration
     int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
     cudaGraph_t graph = nullptr;
@@ -278,7 +281,7 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
         return fail(h, rc);
     if (h->E.alloc(nrows) || h->F.alloc(nrows) || h->Dinv.alloc(nrows) || h->AR.alloc((size_t)(nr + 1) * nt) ||
         h->AT.alloc((size_t)nr * (nt + 1)) || h->r.alloc(h->n) || h->p0.alloc(h->n) || h->p1.alloc(h->n) ||
-        h->q.alloc(h->n) || h->partials.alloc(4 * (size_t)MAX_PARTIALS) || h->st.alloc(1) || h->args.alloc(1)) {
+        h->q.alloc(h->n) || h->partials.alloc(8 * (size_t)MAX_PARTIALS) || h->st.alloc(1) || h->args.alloc(1)) {
         cudaGetLastError();
         return fail(h, MAS_ENOMEM);
     }
@@ -293,6 +296,7 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
         cudaMemset(h->p1.p, 0, h->n * sizeof(double)) != cudaSuccess)
         return fail(h, MAS_ECUDA);
     fill_op(h);
+    if (cudaDeviceGetAttribute(&h->coop_ok, cudaDevAttrCooperativeLaunch, h->device) != cudaSuccess) h->coop_ok = 0;
     if ((rc = scale_planes(h, dt, nullptr)) != MAS_OK) return fail(h, rc);
     if (cudaDeviceSynchronize() != cudaSuccess) return fail(h, MAS_ECUDA);
     *out = h;
@@ -532,6 +536,37 @@ int ensure_hist(mas_pcg *h, int maxit)
 
 bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
 
+constexpr long long PERSIST_AUTO_CELLS = 1LL << 40;   // auto mode: measured faster wherever the state fits on chip
+                                                      // (config 1: 2.0x, config 2 = 786 k cells: 1.46x)
+
+// Plan the one-kernel solve; returns false when it does not apply (too large, no cooperative launch, off).
+bool plan_persistent(const mas_pcg *h, PersistParams *pp, int *grid, size_t *smem, const void **func)
+{
+    if (!h->persistent || !h->coop_ok) return false;
+    if (h->persistent == 2 && (long long)h->n > PERSIST_AUTO_CELLS) return false;
+    const long long nvec = (long long)h->n / 2;
+    long long g = (nvec + PNT - 1) / PNT;
+    if (g > h->num_sms) g = h->num_sms;
+    const long long M = (nvec + g * PNT - 1) / (g * PNT);
+    if (M > 64 || persist_smem((int)M) > (size_t)PMAX_SMEM) return false;
+    *func = h->uniform_phi ? (const void *)k_pcg_persistent<true> : (const void *)k_pcg_persistent<false>;
+    *smem = persist_smem((int)M);
+    if (cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, *func, PNT, *smem) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        return false;
+    }
+    pp->Z = h->r.p; pp->P0 = h->p0.p; pp->P1 = h->p1.p;
+    pp->partials = h->partials.p; pp->hist = h->hist.p; pp->st = h->st.p; pp->args = h->args.p;
+    pp->nvec = (int)nvec; pp->M = (int)M;
+    *grid = (int)g;
+    return true;
+}
+
 }  // namespace
 
 extern "C" int mas_pcg_set_dt(mas_pcg_t *h, double dt, void *stream)
@@ -572,6 +607,9 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
     } else if (!strcmp(name, "serpentine")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->serpentine = value;
+    } else if (!strcmp(name, "persistent")) {
+        if (value < 0 || value > 2) return MAS_EINVAL;
+        h->persistent = value;
     } else if (!strcmp(name, "qrecompute")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->qrecompute = value;
@@ -612,6 +650,12 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     CK(cudaMemcpyAsync(h->args.p, h->h_args, sizeof(SolveArgs), cudaMemcpyHostToDevice, s));
 
     int mode = h->loop_mode;
+    PersistParams ppar;
+    int pgrid = 0;
+    size_t psmem = 0;
+    const void *pfunc = nullptr;
+    const bool persistent = plan_persistent(h, &ppar, &pgrid, &psmem, &pfunc);
+    if (persistent) mode = 2;
     if (mode == 1 && (h->graph_dirty || !h->exec)) {
         if (build_graph(h) != MAS_OK) {       // driver without conditional nodes: fall back, and say so in stats
             drop_graph(h);
@@ -619,7 +663,13 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
         }
     }
     long long launched_outside = 2, launched_loop = 0;
-    if (mode == 1) {
+    if (mode == 2) {                       // init + loop + finish in one cooperative kernel
+        OpDev op = h->op;
+        void *kargs[2] = {&op, &ppar};
+        CK(cudaLaunchCooperativeKernel(pfunc, dim3(pgrid), dim3(PNT), kargs, psmem, s));
+        launched_outside = 0;
+        launched_loop = 1;
+    } else if (mode == 1) {
         CK(cudaGraphLaunch(h->exec, s));
     } else {
         LoopCtx c;
@@ -642,7 +692,7 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
         }
         if (use_xfuse(h)) CK(launch(make_xtail(h, c), s));
     }
-    if (use_xfuse(h)) launched_outside += 1;
+    if (use_xfuse(h) && mode != 2) launched_outside += 1;
     CK(cudaMemcpyAsync(h->h_st, h->st.p, sizeof(State), cudaMemcpyDeviceToHost, s));
     CK(cudaMemcpyAsync(h->h_hist, h->hist.p, ((size_t)maxit + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));          // the one host sync of a graph-mode solve
@@ -655,6 +705,7 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     if (reshist_host) memcpy(reshist_host, h->h_hist, ((size_t)st.k + 1) * sizeof(double));
     h->loop_mode_used = mode;
     h->stats[0] = mode == 1 ? (long long)st.launches : launched_loop;
+    h->stats[6] = mode == 2 ? pgrid : 0;
     h->stats[1] = launched_outside;
     h->stats[2] = mode;
     // unfused: K1 r,p -> p,q (4N); K2 x,p,r,q -> x,r (6N).  xfuse: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)

@@ -63,6 +63,7 @@ VARIANTS = [(0, 0, 0)] + [(1, t, 0) for t in range(7)] + [(2, t, x) for t in ran
 def test_solve_parity_general_mesh_all_variants(variant, tile, xfuse, loop_mode):
     mesh, dt, nu_kind, nu = H.general_case(21, 19, 134, s=500.0)   # 3 phi tiles (ragged), ragged theta
     oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    gpu.set_option("persistent", 0)              # this test is about the streaming kernels
     gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
     gpu.set_option("xfuse", min(xfuse, 1))
@@ -81,6 +82,7 @@ def test_solve_parity_uniform_phi_all_variants(variant, tile, xfuse):
     prob = configs.make("c3", shape=(40, 37, 192))
     s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
     oref, gpu = H.both_ops(prob.mesh, 1e3 / s1, prob.nu_kind, prob.nu)
+    gpu.set_option("persistent", 0)
     gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
     gpu.set_option("xfuse", min(xfuse, 1))
@@ -88,19 +90,23 @@ def test_solve_parity_uniform_phi_all_variants(variant, tile, xfuse):
     H.check_parity(gpu, oref, configs.rhs_blob(prob), None, 1e-9, 3000, label=f"v{variant} t{tile} x{xfuse}")
 
 
+@pytest.mark.parametrize("persistent", [0, 1])
 @pytest.mark.parametrize("bc", [(1, 1), (1, 0)])
-def test_solve_parity_neumann(bc):
+def test_solve_parity_neumann(bc, persistent):
     mesh, dt, nu_kind, nu = H.general_case(10, 9, 66, s=50.0, bc=bc)
     oref, gpu = H.both_ops(mesh, dt, nu_kind, nu, bc)
+    gpu.set_option("persistent", persistent)
     b = np.random.default_rng(8).uniform(-1, 1, mesh.shape)
     H.check_parity(gpu, oref, b, None, 1e-10, 2000, label=f"bc{bc}")
 
 
 # ------------------------------------------------------------------ BASELINE.json configs
-def test_config1_parity_and_rerun_bit_identity():
+@pytest.mark.parametrize("persistent", [0, 1])
+def test_config1_parity_and_rerun_bit_identity(persistent):
     import torch
     prob = configs.make("c1")
     oref, gpu = H.both_ops(prob.mesh, prob.dt_for(2.0), prob.nu_kind, prob.nu)
+    gpu.set_option("persistent", persistent)
     b = configs.rhs_uniform(prob)
     k_r, k_g = H.check_parity(gpu, oref, b, None, prob.rtol, prob.maxit, label="c1")
     # north_star (3): a rerun gives the same bits
@@ -113,11 +119,15 @@ def test_config1_parity_and_rerun_bit_identity():
     assert runs[0] == runs[1] == runs[2]
 
 
+@pytest.mark.parametrize("persistent", [0, 1])
 @pytest.mark.parametrize("s", configs.STIFFNESS["c2"])
-def test_config2_parity_and_manufactured_solution(s):
+def test_config2_parity_and_manufactured_solution(s, persistent):
     import torch
     prob = configs.make("c2")
     oref, gpu = H.both_ops(prob.mesh, prob.dt_for(s), prob.nu_kind, prob.nu)
+    gpu.set_option("persistent", persistent)
+    gpu.solve(_t(np.ones(prob.mesh.shape)), _t(np.zeros(prob.mesh.shape)), 0.0, 1)
+    assert gpu.stats()["loop_mode"] == (2 if persistent else 1)        # config 2 fits the one-kernel path
     u = configs.field_manufactured(prob)
     b = oref.apply_phys(u)                       # the same b for both sides
     H.check_parity(gpu, oref, b, None, 1e-10, prob.maxit, label=f"c2 s={s}")
@@ -176,10 +186,12 @@ def test_config5_chain_first_3_solves():
 
 
 # ------------------------------------------------------------------ edge and degenerate cases
-def test_zero_rhs_maxit_zero_dt_zero():
+@pytest.mark.parametrize("persistent", [0, 1])
+def test_zero_rhs_maxit_zero_dt_zero(persistent):
     import torch
     mesh, dt, nu_kind, nu = H.general_case(6, 5, 8)
     oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    gpu.set_option("persistent", persistent)
     z = torch.zeros(mesh.shape, dtype=torch.float64, device="cuda")
     x = torch.ones_like(z)
     st, k, h = gpu.solve(z, x, 1e-10, 10)                  # zero RHS: x = 0, no iterations
@@ -194,10 +206,12 @@ def test_zero_rhs_maxit_zero_dt_zero():
     assert torch.allclose(x, b, rtol=1e-15, atol=0)
 
 
-def test_smallest_mesh_and_single_row():
+@pytest.mark.parametrize("persistent", [0, 1])
+def test_smallest_mesh_and_single_row(persistent):
     for shape in [(1, 1, 2), (1, 7, 4), (7, 1, 2)]:
         mesh, dt, nu_kind, nu = H.general_case(*shape, s=20.0)
         oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+        gpu.set_option("persistent", persistent)
         b = np.random.default_rng(2).uniform(-1, 1, mesh.shape)
         H.check_parity(gpu, oref, b, None, 1e-12, 200, label=str(shape))
 
@@ -240,6 +254,7 @@ def test_rerun_bit_identity_every_kernel_family(variant, tile, xfuse):
     s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
     from paper_1811_02605_b200 import MasPcg
     gpu = MasPcg(prob.mesh, 1e3 / s1, prob.nu_kind, prob.nu)
+    gpu.set_option("persistent", 0)
     gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
     gpu.set_option("xfuse", min(xfuse, 1))
@@ -292,3 +307,40 @@ def test_large_mesh_64bit_offsets_closed_forms():
     assert float(y.norm()) / bs_norm == pytest.approx(h[-1], rel=1e-9)
     # last plane was really updated (a wrapped 32-bit byte offset would leave it untouched)
     assert float(x[-1].abs().max()) > 0 and float(x[0].abs().max()) > 0
+
+
+# ------------------------------------------------------------------ the one-kernel (persistent cooperative) path
+@pytest.mark.parametrize("shape,bc", [((21, 19, 134), (0, 0)), ((9, 11, 70), (1, 0)), ((40, 37, 192), (0, 1)),
+                                      ((3, 2, 64), (1, 1))])
+def test_persistent_kernel_parity_general_mesh_warm_start_and_bits(shape, bc):
+    import torch
+    mesh, dt, nu_kind, nu = H.general_case(*shape, s=500.0, bc=bc)
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu, bc)
+    gpu.set_option("persistent", 1)
+    rng = np.random.default_rng(3)
+    b = rng.uniform(-1, 1, mesh.shape)
+    x0 = rng.standard_normal(mesh.shape)
+    H.check_parity(gpu, oref, b, x0, 1e-10, 2000, label=f"persistent {shape}")
+    assert gpu.stats()["loop_mode"] == 2 and gpu.stats()["loop_launches"] == 1
+    runs = []
+    for _ in range(3):
+        xd = _t(x0)
+        st, k, h = gpu.solve(_t(b), xd, 1e-10, 2000)
+        runs.append((k, h.tobytes(), xd.cpu().numpy().tobytes()))
+    assert runs[0] == runs[1] == runs[2]
+
+
+def test_persistent_auto_threshold_and_too_large_falls_back():
+    from paper_1811_02605_b200 import MasPcg
+    small = configs.make("c1")
+    gpu = MasPcg(small.mesh, small.dt_for(2.0), small.nu_kind, small.nu)
+    b = _t(configs.rhs_uniform(small))
+    gpu.solve(b, _t(np.zeros(small.mesh.shape)), 1e-10, 100)
+    assert gpu.stats()["loop_mode"] == 2                     # auto: small mesh -> one kernel
+    big = configs.make("c3", shape=(64, 96, 256))            # 1.6 M cells: state does not fit on chip
+    s1 = H.oracle_s1(big.mesh, big.nu_kind, big.nu)
+    gpu = MasPcg(big.mesh, 100.0 / s1, big.nu_kind, big.nu)
+    gpu.set_option("persistent", 1)
+    bb = _t(configs.rhs_blob(big))
+    st, k, h = gpu.solve(bb, _t(np.zeros(big.mesh.shape)), 1e-8, 500)
+    assert st == 0 and gpu.stats()["loop_mode"] == 1         # falls back to the graph loop
