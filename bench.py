@@ -51,6 +51,7 @@ def parse():
     ap.add_argument("--stencil-tile", type=int, default=None)
     ap.add_argument("--qrecompute", type=int, default=None)
     ap.add_argument("--persistent", type=int, default=None)
+    ap.add_argument("--opt", action="append", default=[], help="name=value passed to mas_pcg_set_option (tuning)")
     ap.add_argument("--k2r-tile", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chain-steps", type=int, default=20,
@@ -362,6 +363,9 @@ def main():
         gpu.set_option("qrecompute", args.qrecompute)
     if args.persistent is not None:
         gpu.set_option("persistent", args.persistent)
+    for kv in args.opt:
+        name, val = kv.split("=")
+        gpu.set_option(name, int(val))
     if args.k2r_tile is not None:
         gpu.set_option("k2r_tile", args.k2r_tile)
     b_host = torch.from_numpy(b_np).pin_memory()
