@@ -28,8 +28,8 @@ class MasPcg:
         self._h = B.mas_pcg_create(self.shape, mesh.metric_arrays(), dt, nu_kind, nu, bc)
 
     def close(self):
-        if getattr(self, "_h", None):
-            B.mas_pcg_destroy(self._h)
+        if getattr(self, "_h", None) and B is not None and getattr(B, "mas_pcg_destroy", None):
+            B.mas_pcg_destroy(self._h)          # (module globals may already be gone at interpreter exit)
             self._h = None
 
     __del__ = close
