@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "sts"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "sts", "visc"])
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--tile", type=int, default=None)
     ap.add_argument("--loop-mode", type=int, default=None)
@@ -313,8 +313,55 @@ def run_sts(args):
     print(json.dumps(line), flush=True)
 
 
+def run_visc(args):
+    """The paper's algorithm comparison for the viscosity advance (PCG+PC1 needs ~550
+    iterations, STS ~200 sub-steps, PC1+STS about 2x faster than PC1+PC1 for the whole step) on the synthetic
+    256x256x512 mesh: the same dt (stiffness 1e4) advanced implicitly by the PCG solve and explicitly by RKL2."""
+    import numpy as np
+    import torch
+    from mas_inputs import configs
+    from paper_1811_02605_b200 import MasPcg
+    torch.cuda.set_device(0)
+    prob = configs.make("c4")
+    dt = prob.dt_for(1e4)
+    gpu = MasPcg(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)
+    u0 = torch.from_numpy(configs.blob(prob.mesh)
+                          + 0.01 * np.random.default_rng(2).standard_normal(prob.mesh.shape)).cuda()
+    x, u = torch.zeros_like(u0), u0.clone()
+    S = gpu.sts_stages(dt)
+    stream = torch.cuda.current_stream()
+
+    def timed(fn):
+        for _ in range(max(args.warmup, 1)):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(args.steps):
+            out = fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / args.steps, out
+
+    ms_pcg, (st, k, _) = timed(lambda: gpu.solve(u0, x.zero_(), 1e-9, 5000, want_hist=False))
+    ms_sts, _ = timed(lambda: gpu.sts_advance(u.copy_(u0), dt, S))
+    line = {"metric": "viscosity_advance_ms_256x256x512", "value": ms_sts, "unit": "ms", "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 1), "ms_per_step": ms_sts, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "visc: 256x256x512 fp64, nu(r), dt at stiffness 1e4, blob + noise field (each "
+                                   "timing includes one 268 MB reset of the field)"},
+            "pcg_pc1": {"ms": ms_pcg, "iterations": k, "status": st, "rtol": 1e-9},
+            "sts_rkl2": {"ms": ms_sts, "stages": S},
+            "sts_speedup_over_pcg": ms_pcg / ms_sts,
+            "implicit_vs_explicit_max_rel_diff": float((u - x).abs().max() / u0.abs().max())}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
+    if args.impl == "ours" and args.workload == "visc":
+        run_visc(args)
+        return
     if args.impl == "ours" and args.workload == "c5":
         run_chain(args)
         return
