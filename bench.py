@@ -129,6 +129,15 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def gpu_selector(torch):
+    """What nvidia-smi -i should get for the current CUDA device: its UUID (robust to CUDA_VISIBLE_DEVICES)."""
+    try:
+        u = str(torch.cuda.get_device_properties(torch.cuda.current_device()).uuid)
+        return u if u.startswith("GPU-") else "GPU-" + u
+    except Exception:
+        return torch.cuda.current_device()
+
+
 def hbm_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -274,7 +283,7 @@ def run_sts(args):
     for _ in range(max(args.warmup, 3)):
         u.copy_(u0)
         gpu.sts_advance(u, tau, S)
-    sampler = ClockSampler(0)
+    sampler = ClockSampler(gpu_selector(torch))
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -429,7 +438,7 @@ def main():
     for _ in range(max(args.warmup, 3)):
         st, k, _ = step()
     barrier()
-    sampler = ClockSampler(torch.cuda.current_device() if "CUDA_VISIBLE_DEVICES" not in os.environ else 0)
+    sampler = ClockSampler(gpu_selector(torch))
     if rank == 0:
         sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
