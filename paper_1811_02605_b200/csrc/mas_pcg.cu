@@ -84,6 +84,7 @@ struct mas_pcg {
     int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
     int persistent = 2;              // one cooperative kernel for the whole solve: 0 off, 1 whenever it fits, 2 auto
     int coop_ok = 0;
+    int unroll = 4;                  // PCG iterations per WHILE trip of the graph loop (measured: +1 % c4, +3 % c3)
     int qrecompute = 0;              // 1 (needs xfuse, wide): q is not stored, K2 recomputes it: 64 B/cell/iteration
     int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
     cudaGraph_t graph = nullptr;
@@ -500,9 +501,15 @@ int build_graph(mas_pcg *h)
     if (cudaGraphAddNode(&n_while, g, &n_init, 1, &wp) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
     cudaGraph_t body = wp.conditional.phGraph_out[0];
     const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
-    if (add_node(&n_k1, body, nullptr, k1) != cudaSuccess || add_node(&n_k2, body, &n_k1, k2) != cudaSuccess) {
-        cudaGetLastError();
-        return MAS_ECUDA;
+    // `unroll` iterations per WHILE trip: the conditional node is evaluated once per trip, and K1 / K2 return
+    // at once when the loop has ended (device flag), so extra pairs after convergence cost two empty launches.
+    const cudaGraphNode_t *dep = nullptr;
+    for (int u = 0; u < h->unroll; u++) {
+        if (add_node(&n_k1, body, dep, k1) != cudaSuccess || add_node(&n_k2, body, &n_k1, k2) != cudaSuccess) {
+            cudaGetLastError();
+            return MAS_ECUDA;
+        }
+        dep = &n_k2;
     }
     if (use_xfuse(h)) {
         cudaGraphNode_t n_tail;
@@ -607,6 +614,9 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
     } else if (!strcmp(name, "serpentine")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->serpentine = value;
+    } else if (!strcmp(name, "unroll")) {
+        if (value < 1 || value > 16) return MAS_EINVAL;
+        h->unroll = value;
     } else if (!strcmp(name, "persistent")) {
         if (value < 0 || value > 2) return MAS_EINVAL;
         h->persistent = value;
