@@ -110,7 +110,8 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
  *   "tile" (tile configuration of the variant), "ci" (r-chunk length, 0 = automatic),
  *   "xfuse" (1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B), "serpentine" (K2 sweeps
  *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile", "qrecompute" (64 B),
- *   "unroll" (PCG iterations per WHILE trip of the graph loop, 1..16),
+ *   "unroll" (PCG iterations per WHILE trip of the graph loop, 1..16), "pdl" (programmatic dependent launch
+ *   edges inside the loop body; default 0: measured slower),
  *   "persistent" (small meshes: whole solve in one cooperative kernel; 0 off, 1 whenever it fits, 2 auto).
  * Unknown name or value: MAS_EINVAL. */
 int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value);

@@ -222,6 +222,7 @@ __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditio
                                              int reverse)
 {
     __shared__ double sh[32];
+    cudaGridDependencySynchronize();                  // PDL edge from K1 (no-op for a plain launch)
     State *st = w.st;
     if (!st->active) return;
     const double alpha = st->alpha;
@@ -280,6 +281,7 @@ __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditio
             }
         }
     }
+    cudaTriggerProgrammaticLaunchCompletion();        // PDL: K1 of the next iteration may start its prologue
     if (grid_sum<NT, 2>(acc, w.partials, &st->ticket[2], sh) && threadIdx.x == 0)
         k2_finish(st, w, acc[0], acc[1], cond, use_cond);
 }

@@ -251,18 +251,6 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Smem &sm = *reinterpret_cast<Smem *>(smem_raw);
 
-    State *st = w.st;
-    if (!st->active) return;
-    const double beta = st->beta;
-    const int par = st->k & 1;
-    const double *__restrict__ pin = par ? w.p1 : w.p0;
-    double *__restrict__ pout = par ? w.p0 : w.p1;
-    const double *__restrict__ rvec = w.r;
-    // XF: the x-update of the PREVIOUS iteration, x += alpha_{k-1} p_{k-1}, is applied here (p_old is
-    // p_{k-1}); K2 then only updates r.  Same operations on the same operands as the unfused path.
-    const double alpha_prev = XF ? st->alpha : 0.0;
-    double *__restrict__ xvec = XF ? w.args->x : nullptr;
-
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
     int b = blockIdx.x;
     const int kt = b % mp.nkt; b /= mp.nkt;
@@ -309,6 +297,23 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
         if (lane < 4) sm.hfifo[s][lane][warp] = 0.0;
     }
     __syncthreads();
+
+    // Everything above depends only on the operator, not on the previous kernel: with a programmatic
+    // (PDL) edge this block may have been launched while K2 of the previous iteration was still draining.
+    // From here on the iteration state and the vectors are read, so wait for the predecessor to complete
+    // (a no-op when the kernel was launched without the programmatic attribute).
+    cudaGridDependencySynchronize();
+    State *st = w.st;
+    if (!st->active) return;
+    const double beta = st->beta;
+    const int par = st->k & 1;
+    const double *__restrict__ pin = par ? w.p1 : w.p0;
+    double *__restrict__ pout = par ? w.p0 : w.p1;
+    const double *__restrict__ rvec = w.r;
+    // XF: the x-update of the PREVIOUS iteration, x += alpha_{k-1} p_{k-1}, is applied here (p_old is
+    // p_{k-1}); K2 then only updates r.  Same operations on the same operands as the unfused path.
+    const double alpha_prev = XF ? st->alpha : 0.0;
+    double *__restrict__ xvec = XF ? w.args->x : nullptr;
 
     // phi factors: cells A0,A1 (k, k+1) and B0,B1 (k+64, k+65); index into the staged arrays is cell-k0+1
     const int ea = 2 * lane + 1, eb = 2 * lane + 65;
@@ -442,6 +447,7 @@ k1_wide(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int us
             hl_c = hl_n; hr_c = hr_n;
         }
     }
+    cudaTriggerProgrammaticLaunchCompletion();      // PDL: the successor's blocks may start their prologue
     cp_async_wait<0>();
     double a1[1] = {acc};
     if (grid_sum<NT, 1>(a1, w.partials, &st->ticket[1], sm.red) && threadIdx.x == 0)

@@ -84,6 +84,8 @@ struct mas_pcg {
     int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
     int persistent = 2;              // one cooperative kernel for the whole solve: 0 off, 1 whenever it fits, 2 auto
     int coop_ok = 0;
+    int pdl = 0;                     // programmatic dependent launch edges inside the loop body: measured 5 % SLOWER
+                                     // (early K1 blocks park their shared memory while K2 drains), so off
     int unroll = 4;                  // PCG iterations per WHILE trip of the graph loop (measured: +1 % c4, +3 % c3)
     int qrecompute = 0;              // 1 (needs xfuse, wide): q is not stored, K2 recomputes it: 64 B/cell/iteration
     int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
@@ -503,14 +505,29 @@ int build_graph(mas_pcg *h)
     const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
     // `unroll` iterations per WHILE trip: the conditional node is evaluated once per trip, and K1 / K2 return
     // at once when the loop has ended (device flag), so extra pairs after convergence cost two empty launches.
-    const cudaGraphNode_t *dep = nullptr;
-    for (int u = 0; u < h->unroll; u++) {
-        if (add_node(&n_k1, body, dep, k1) != cudaSuccess || add_node(&n_k2, body, &n_k1, k2) != cudaSuccess) {
-            cudaGetLastError();
-            return MAS_ECUDA;
+    // Edges inside the body are programmatic (PDL) when both kernels wait with cudaGridDependencySynchronize
+    // (k1_wide and k2_vec): the successor's blocks launch while the predecessor drains and run the part of
+    // their prologue that does not depend on it.
+    const bool pdl = h->pdl && h->variant == 2 && !use_qrec(h);
+    cudaGraphNode_t prev = nullptr;
+    for (int u = 0; u < 2 * h->unroll; u++) {
+        cudaGraphNode_t node;
+        if (add_node(&node, body, nullptr, (u & 1) ? k2 : k1) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+        if (prev) {
+            cudaGraphEdgeData ed;
+            memset(&ed, 0, sizeof(ed));
+            if (pdl) {
+                ed.type = cudaGraphDependencyTypeProgrammatic;
+                ed.from_port = cudaGraphKernelNodePortProgrammatic;
+            }
+            if (cudaGraphAddDependencies_v2(body, &prev, &node, &ed, 1) != cudaSuccess) {
+                cudaGetLastError();
+                return MAS_ECUDA;
+            }
         }
-        dep = &n_k2;
+        prev = node;
     }
+    (void)n_k1; (void)n_k2;
     if (use_xfuse(h)) {
         cudaGraphNode_t n_tail;
         const KLaunch kt = make_xtail(h, c);
@@ -614,6 +631,9 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
     } else if (!strcmp(name, "serpentine")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->serpentine = value;
+    } else if (!strcmp(name, "pdl")) {
+        if (value != 0 && value != 1) return MAS_EINVAL;
+        h->pdl = value;
     } else if (!strcmp(name, "unroll")) {
         if (value < 1 || value > 16) return MAS_EINVAL;
         h->unroll = value;
@@ -667,8 +687,12 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     const bool persistent = plan_persistent(h, &ppar, &pgrid, &psmem, &pfunc);
     if (persistent) mode = 2;
     if (mode == 1 && (h->graph_dirty || !h->exec)) {
-        if (build_graph(h) != MAS_OK) {       // driver without conditional nodes: fall back, and say so in stats
+        if (build_graph(h) != MAS_OK && h->pdl) {   // programmatic edges refused: plain edges
+            h->pdl = 0;
             drop_graph(h);
+        }
+        if ((h->graph_dirty || !h->exec) && build_graph(h) != MAS_OK) {
+            drop_graph(h);                    // driver without conditional nodes: fall back, and say so in stats
             mode = 0;
         }
     }
@@ -716,6 +740,7 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     h->loop_mode_used = mode;
     h->stats[0] = mode == 1 ? (long long)st.launches : launched_loop;
     h->stats[6] = mode == 2 ? pgrid : 0;
+    h->stats[7] = (mode == 1 && h->pdl && h->variant == 2 && !use_qrec(h)) ? 1 : 0;
     h->stats[1] = launched_outside;
     h->stats[2] = mode;
     // unfused: K1 r,p -> p,q (4N); K2 x,p,r,q -> x,r (6N).  xfuse: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)
