@@ -472,6 +472,8 @@ def main():
     # ---------------- per-kernel durations (CUDA events around each launch) ----------------
     x.zero_()
     prof = gpu.profile(b, x, 40)
+    # what a trivial linear kernel with the same DRAM read/write mix sustains (context for the rooflines)
+    mix = {"k1_mix_ms": gpu.mix_probe(6, 100), "k2_mix_ms": gpu.mix_probe(3, 100)} if args.workload == "c4" else None
     barrier()
 
     ms, iters_all, launches_all = reduce_over_ranks(ms, float(iters_done), float(launches), world)
@@ -507,6 +509,12 @@ def main():
                                             "alg_bytes": k1_bytes, "gbs": k1_gbs},
                         "k2_fused_vector": {"ms": prof["k2_ms"], "min_ms": prof["k2_min_ms"],
                                             "alg_bytes": k2_bytes, "gbs": k2_gbs}},
+            "mix_ceiling": None if mix is None else {
+                "what": "trivial linear kernels with the same DRAM mix (K1: 3 vectors read + 3 written, K2: 2 read + 1 "
+                        "written in place), best grid size, 100 back-to-back launches",
+                "k1_mix_gbs": k1_bytes / (mix["k1_mix_ms"] * 1e-3) / 1e9,
+                "k2_mix_gbs": k2_bytes / (mix["k2_mix_ms"] * 1e-3) / 1e9,
+                "k1_frac_of_mix": mix["k1_mix_ms"] / prof["k1_ms"], "k2_frac_of_mix": mix["k2_mix_ms"] / prof["k2_ms"]},
             "iteration": {"ms": it_ms, "model_gbs": bpc * n / (it_ms * 1e-3) / 1e9,
                           "frac_of_peak": bpc * n / (it_ms * 1e-3) / 1e9 / peak,
                           "frac_of_nominal_8000": bpc * n / (it_ms * 1e-3) / 1e9 / 8000.0},

@@ -98,6 +98,12 @@ int mas_pcg_apply(mas_pcg_t *h, const double *x_dev, double *y_dev, void *stream
  * (K1 = fused matvec, K2 = fused vector kernel).  1 <= nit <= 256.  x_dev is overwritten. */
 int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev, int nit, void *stream, double *ms_out);
 
+/* Measurement aid (bench.py): *ms_out (HOST) = best sustained time per launch, over `reps` back-to-back
+ * launches, of a trivial LINEAR kernel with the DRAM read/write mix of K1 (which = 6: three N-vectors read,
+ * three written, one of them in place) or K2 (which = 3: two read, one written in place) and none of their
+ * structure: what the memory system sustains for that mix.  Clobbers the handle's workspaces. */
+int mas_pcg_mix_probe(mas_pcg_t *h, int which, int reps, void *stream, double *ms_out);
+
 /* Fills HOST array out[8] with counters of the last solve:
  *   [0] kernels launched inside the iteration loop, [1] kernels launched outside it,
  *   [2] loop mode used (1 = CUDA-graph WHILE node, 0 = host-driven chunks, 2 = one persistent cooperative kernel),

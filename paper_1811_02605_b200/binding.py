@@ -68,6 +68,8 @@ def _load():
     L.mas_sts_stages.argtypes = [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int)]
     L.mas_sts_advance.restype = ctypes.c_int
     L.mas_sts_advance.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp]
+    L.mas_pcg_mix_probe.restype = ctypes.c_int
+    L.mas_pcg_mix_probe.argtypes = [vp, ctypes.c_int, ctypes.c_int, vp, _dp]
     L.mas_pcg_stats.restype = ctypes.c_int
     L.mas_pcg_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong)]
     L.mas_pcg_set_option.restype = ctypes.c_int
@@ -198,6 +200,15 @@ def mas_sts_advance(handle, u_ptr, tau, s, stream=0):
     st = lib().mas_sts_advance(handle, u_ptr, float(tau), int(s), stream)
     if st != MAS_OK:
         raise MasError(st, "mas_sts_advance")
+
+
+def mas_pcg_mix_probe(handle, which, reps, stream=0) -> float:
+    """ms per launch of a trivial linear kernel with K1's (which=6) or K2's (which=3) DRAM read/write mix."""
+    out = ctypes.c_double(0.0)
+    st = lib().mas_pcg_mix_probe(handle, int(which), int(reps), stream, ctypes.byref(out))
+    if st != MAS_OK:
+        raise MasError(st, "mas_pcg_mix_probe")
+    return out.value
 
 
 def mas_pcg_stats(handle):

@@ -388,4 +388,27 @@ __global__ void __launch_bounds__(NT) k1_v0(OpDev op, Work w, cudaGraphCondition
         k1_finish(st, acc[0], cond, use_cond);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Measurement aids (mas_pcg_mix_probe): trivial LINEAR kernels with the DRAM read/write mix of K1 and K2 and
+// none of their structure -- what the memory system sustains for that mix, as context for the rooflines.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_mix6(const double2 *a, const double2 *b, double2 *x, double2 *p, double2 *q,
+                                              size_t n2)        // K1 (xfuse): reads a, b, x; writes p, q, x
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x) {
+        const double2 av = a[i], bv = b[i], xv = x[i];
+        p[i] = make_double2(av.x + bv.x, av.y + bv.y);
+        q[i] = make_double2(av.x - bv.x, av.y - bv.y);
+        x[i] = make_double2(xv.x + 0.5 * av.x, xv.y + 0.5 * av.y);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_mix3(double2 *r, const double2 *q, size_t n2)   // K2: reads r, q; writes r
+{
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x) {
+        const double2 rv = r[i], qv = q[i];
+        r[i] = make_double2(rv.x - 0.5 * qv.x, rv.y - 0.5 * qv.y);
+    }
+}
+
 }  // namespace mas

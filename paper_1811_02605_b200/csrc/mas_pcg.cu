@@ -897,3 +897,44 @@ extern "C" int mas_sts_advance(mas_pcg_t *h, double *u_dev, double tau, int s, v
     h->graph_dirty = h->graph_dirty;             // PCG workspaces were clobbered; solves re-initialise them
     return MAS_OK;
 }
+
+// Measurement aid: sustained time of a trivial linear kernel with K1's (which = 6) or K2's (which = 3) DRAM mix
+// over the handle's own N-vectors (their contents are destroyed; the next solve re-initialises them).
+extern "C" int mas_pcg_mix_probe(mas_pcg_t *h, int which, int reps, void *stream, double *ms_out)
+{
+    if (!h || !ms_out || (which != 6 && which != 3) || reps < 1 || reps > 100000) return MAS_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!h->bdev.p && h->bdev.alloc(h->n) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    CK(cudaMemsetAsync(h->bdev.p, 0, h->n * sizeof(double), s));
+    CK(cudaMemsetAsync(h->r.p, 0, h->n * sizeof(double), s));
+    CK(cudaMemsetAsync(h->q.p, 0, h->n * sizeof(double), s));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    const size_t n2 = h->n / 2;
+    double best = 1e30;
+    for (int mult = 4; mult <= 32; mult *= 2) {                 // the grid size matters by a few percent: take the best
+        const int blocks = h->num_sms * mult;
+        for (int pass = 0; pass < 2; pass++) {                  // pass 0 = warm-up
+            const int n = pass ? reps : 3;
+            CK(cudaEventRecord(e0, s));
+            for (int r = 0; r < n; r++) {
+                if (which == 6)
+                    k_mix6<<<blocks, 256, 0, s>>>((const double2 *)h->r.p, (const double2 *)h->p0.p, (double2 *)h->bdev.p,
+                                                  (double2 *)h->p1.p, (double2 *)h->q.p, n2);
+                else
+                    k_mix3<<<blocks, 256, 0, s>>>((double2 *)h->r.p, (const double2 *)h->q.p, n2);
+            }
+            CK(cudaEventRecord(e1, s));
+            CK(cudaEventSynchronize(e1));
+            float ms = 0;
+            CK(cudaEventElapsedTime(&ms, e0, e1));
+            if (pass && ms / n < best) best = ms / n;
+        }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    CK(cudaGetLastError());
+    *ms_out = best;
+    return MAS_OK;
+}

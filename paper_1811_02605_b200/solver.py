@@ -83,5 +83,8 @@ class MasPcg:
         B.mas_sts_advance(self._h, _dev_ptr(u, self.n), tau, s, _stream_ptr(stream))
         return u
 
+    def mix_probe(self, which: int, reps: int = 50, stream=None) -> float:
+        return B.mas_pcg_mix_probe(self._h, which, reps, _stream_ptr(stream))
+
     def stats(self):
         return B.mas_pcg_stats(self._h)
