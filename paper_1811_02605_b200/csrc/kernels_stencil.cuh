@@ -298,24 +298,14 @@ inline void stencil_pick(bool uniform, int epi, const void **func, dim3 *block, 
     cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);
 }
 
-inline int stencil_num_tiles() { return 6; }
-
-inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int tile, int num_sms, StencilParams *mp,
-                              const void **func, dim3 *grid, dim3 *block, size_t *smem)
+// tiles and r-chunk length for a picked kernel (shared by the cp.async and the TMA variants)
+inline void stencil_grid(int nr, int nt, int np, int epi, int tj, int num_sms, const void *func, dim3 block, size_t smem,
+                         StencilParams *mp, dim3 *grid)
 {
-    int tj;
-    switch (tile) {
-        case 0: tj = 6; stencil_pick<6, 2, 2, true>(uniform, epi, func, block, smem); break;
-        case 1: tj = 8; stencil_pick<8, 2, 2, false>(uniform, epi, func, block, smem); break;
-        case 2: tj = 14; stencil_pick<14, 2, 1, false>(uniform, epi, func, block, smem); break;
-        case 3: tj = 4; stencil_pick<4, 2, 3, true>(uniform, epi, func, block, smem); break;
-        case 4: tj = 8; stencil_pick<8, 2, 1, true>(uniform, epi, func, block, smem); break;
-        default: tj = 8; stencil_pick<8, 3, 2, false>(uniform, epi, func, block, smem); break;
-    }
     mp->nkt = (np + WIDE_TK - 1) / WIDE_TK;
     mp->njt = (nt + tj - 1) / tj;
     int occ = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, *func, (int)block->x, *smem) != cudaSuccess || occ < 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, func, (int)block.x, smem) != cudaSuccess || occ < 1) {
         cudaGetLastError();
         occ = 1;
     }
@@ -333,6 +323,23 @@ inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int 
     mp->ci = best;
     mp->nit = (nr + best - 1) / best;
     *grid = dim3((unsigned)(mp->nkt * mp->njt * mp->nit));
+}
+
+inline int stencil_num_tiles() { return 6; }
+
+inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int tile, int num_sms, StencilParams *mp,
+                              const void **func, dim3 *grid, dim3 *block, size_t *smem)
+{
+    int tj;
+    switch (tile) {
+        case 0: tj = 6; stencil_pick<6, 2, 2, true>(uniform, epi, func, block, smem); break;
+        case 1: tj = 8; stencil_pick<8, 2, 2, false>(uniform, epi, func, block, smem); break;
+        case 2: tj = 14; stencil_pick<14, 2, 1, false>(uniform, epi, func, block, smem); break;
+        case 3: tj = 4; stencil_pick<4, 2, 3, true>(uniform, epi, func, block, smem); break;
+        case 4: tj = 8; stencil_pick<8, 2, 1, true>(uniform, epi, func, block, smem); break;
+        default: tj = 8; stencil_pick<8, 3, 2, false>(uniform, epi, func, block, smem); break;
+    }
+    stencil_grid(nr, nt, np, epi, tj, num_sms, *func, *block, *smem, mp, grid);
 }
 
 }  // namespace mas

@@ -16,6 +16,7 @@
 #include "kernels_base.cuh"
 #include "kernels_march.cuh"
 #include "kernels_stencil.cuh"
+#include "kernels_stencil_tma.cuh"
 #include "kernels_persistent.cuh"
 
 using namespace mas;
@@ -360,8 +361,8 @@ KLaunch make_apply(const mas_pcg *h, LoopCtx &c)
         stencil_common(h, c.sp);
         c.sp.E = h->E.p; c.sp.F = h->F.p; c.sp.AR = h->AR.p; c.sp.AT = h->AT.p;
         c.sp.u = c.xin; c.sp.out = c.y;
-        stencil_configure(h->nr, h->nt, h->np, h->uniform_phi, EPI_APPLY, h->stencil_tile, h->num_sms, &c.sp, &k.func,
-                          &k.grid, &k.block, &k.smem);
+        stencil_configure_any(h->nr, h->nt, h->np, h->uniform_phi, EPI_APPLY, h->stencil_tile, h->num_sms, &c.sp,
+                              &k.func, &k.grid, &k.block, &k.smem);
         k.args[0] = &c.op; k.args[1] = &c.sp;
         k.nargs = 2;
         return k;
@@ -626,7 +627,7 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->apply_variant = value;
     } else if (!strcmp(name, "stencil_tile")) {
-        if (value < 0 || value >= stencil_num_tiles()) return MAS_EINVAL;
+        if (value < 0 || value >= stencil_num_tiles_any()) return MAS_EINVAL;
         h->stencil_tile = value;
     } else if (!strcmp(name, "serpentine")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
@@ -827,8 +828,8 @@ int launch_stencil(const mas_pcg *h, StencilParams &sp, int epi, cudaStream_t s)
 {
     KLaunch k;
     OpDev op = h->op;
-    stencil_configure(h->nr, h->nt, h->np, h->uniform_phi, epi, h->stencil_tile, h->num_sms, &sp, &k.func, &k.grid,
-                      &k.block, &k.smem);
+    stencil_configure_any(h->nr, h->nt, h->np, h->uniform_phi, epi, h->stencil_tile, h->num_sms, &sp, &k.func, &k.grid,
+                          &k.block, &k.smem);
     k.args[0] = &op; k.args[1] = &sp;
     CK(launch(k, s));
     return MAS_OK;

@@ -38,7 +38,7 @@ def test_stencil_kernels_all_tiles_ragged_phi(np_, uniform):
     oref, gpu = H.both_ops(mesh, dt, nu_kind, nu, bc)
     u = np.random.default_rng(np_).standard_normal(mesh.shape)
     a_ref, l_ref = oref.apply(u), oref.lop(u)
-    for tile in range(6):
+    for tile in range(8):
         gpu.set_option("stencil_tile", tile)
         a = gpu.apply(_t(u)).cpu().numpy().reshape(mesh.shape)
         l = gpu.lop(_t(u)).cpu().numpy().reshape(mesh.shape)
@@ -74,7 +74,7 @@ def test_sts_ragged_theta(nt):
     tau = 40.0 / gpu.lambda_max()
     s = gpu.sts_stages(tau)
     y_ref = oref.sts(u, tau, s)
-    for tile in (0, 1, 3, 4):
+    for tile in (0, 1, 3, 4, 6, 7):
         gpu.set_option("stencil_tile", tile)
         ud = _t(u)
         gpu.sts_advance(ud, tau, s)
