@@ -112,7 +112,8 @@ int mas_pcg_mix_probe(mas_pcg_t *h, int which, int reps, void *stream, double *m
 int mas_pcg_stats(const mas_pcg_t *h, long long *out);
 
 /* Tuning / debugging knob, takes effect at the next solve.  name in
- *   "loop_mode" (0 host chunks, 1 graph while), "variant" (K1: 0 baseline, 1 marching, 2 wide marching),
+ *   "loop_mode" (0 host chunks, 1 graph while), "variant" (K1: 0 baseline, 1 marching, 2 wide marching with cp.async,
+ *   3 wide marching with TMA bulk copies + mbarriers = default),
  *   "tile" (tile configuration of the variant), "ci" (r-chunk length, 0 = automatic),
  *   "xfuse" (1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B), "serpentine" (K2 sweeps
  *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile", "qrecompute" (64 B),

@@ -17,6 +17,7 @@
 #include "kernels_march.cuh"
 #include "kernels_stencil.cuh"
 #include "kernels_stencil_tma.cuh"
+#include "kernels_k1_tma.cuh"
 #include "kernels_persistent.cuh"
 
 using namespace mas;
@@ -76,11 +77,12 @@ struct mas_pcg {
     // loop
     int loop_mode = 1;               // requested: 1 graph-while, 0 host chunks
     int loop_mode_used = 1;
-    int variant = 2;                 // K1 variant: 0 baseline, 1 marching tiles (64 wide), 2 wide marching tiles
+    int variant = 3;                 // K1 variant: 0 baseline, 1 marching tiles (64 wide), 2 wide marching tiles (cp.async),
+                                     // 3 wide marching tiles with TMA bulk copies + mbarriers (default)
     int tile = 0;                    // tile configuration id of the variant
     int ci_force = 0;                // >0: override the r-chunk length (tuning)
     int apply_variant = 1;           // 1: k_stencil marching kernel for A x (apply / initial residual); 0: k_apply
-    int stencil_tile = 0;
+    int stencil_tile = 7;            // 0..5 cp.async k_stencil, 6..11 TMA k_stencil_tma (7 = TJ 8, 2 blocks/SM: fastest)
     int k2r_tile = 0;
     int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
     int persistent = 2;              // one cooperative kernel for the whole solve: 0 off, 1 whenever it fits, 2 auto
@@ -344,8 +346,8 @@ int base_grid(const mas_pcg *h, const void *func, int nt_block)
     return (int)gsz;
 }
 
-bool use_xfuse(const mas_pcg *h) { return h->xfuse && h->variant == 2; }
-bool use_qrec(const mas_pcg *h) { return h->qrecompute && use_xfuse(h); }
+bool use_xfuse(const mas_pcg *h) { return (h->xfuse && h->variant == 2) || h->variant == 3; }   // k1_tma is always xfuse
+bool use_qrec(const mas_pcg *h) { return h->qrecompute && h->xfuse && h->variant == 2; }
 
 void stencil_common(const mas_pcg *h, StencilParams &sp)
 {
@@ -399,7 +401,7 @@ KLaunch make_k2(const mas_pcg *h, LoopCtx &c)
         k.nargs = 2;
         return k;
     }
-    const bool xf = h->xfuse && h->variant == 2;
+    const bool xf = use_xfuse(h);
     if (xf)
         k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true, true> : (const void *)k2_vec<NT_BASE, false, true>;
     else
@@ -434,6 +436,14 @@ KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
         k.grid = dim3(base_grid(h, k.func, NT_BASE));
         k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
         k.nargs = 4;
+        return k;
+    }
+    if (h->variant == 3) {
+        k1_tma_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, h->ci_force, &c.wp, &k.func, &k.grid,
+                         &k.block, &k.smem);
+        c.wp.vp = h->vp0; c.wp.wp = h->wp0; c.wp.ip = h->ip0;
+        k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.wp; k.args[3] = &c.cond; k.args[4] = &c.use_cond;
+        k.nargs = 5;
         return k;
     }
     if (h->variant == 1) {
@@ -509,7 +519,7 @@ int build_graph(mas_pcg *h)
     // Edges inside the body are programmatic (PDL) when both kernels wait with cudaGridDependencySynchronize
     // (k1_wide and k2_vec): the successor's blocks launch while the predecessor drains and run the part of
     // their prologue that does not depend on it.
-    const bool pdl = h->pdl && h->variant == 2 && !use_qrec(h);
+    const bool pdl = h->pdl && h->variant >= 2 && !use_qrec(h);
     cudaGraphNode_t prev = nullptr;
     for (int u = 0; u < 2 * h->unroll; u++) {
         cudaGraphNode_t node;
@@ -616,11 +626,11 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->loop_mode = value;
     } else if (!strcmp(name, "variant")) {
-        if (value < 0 || value > 2) return MAS_EINVAL;
+        if (value < 0 || value > 3) return MAS_EINVAL;
         h->variant = value;
         h->tile = 0;
     } else if (!strcmp(name, "tile")) {
-        const int nt_ = h->variant == 1 ? march_num_tiles() : (h->variant == 2 ? wide_num_tiles() : 1);
+        const int nt_ = h->variant == 1 ? march_num_tiles() : (h->variant == 2 ? wide_num_tiles() : (h->variant == 3 ? k1_tma_num_tiles() : 1));
         if (value < 0 || value >= nt_) return MAS_EINVAL;
         h->tile = value;
     } else if (!strcmp(name, "apply_variant")) {
@@ -741,7 +751,7 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     h->loop_mode_used = mode;
     h->stats[0] = mode == 1 ? (long long)st.launches : launched_loop;
     h->stats[6] = mode == 2 ? pgrid : 0;
-    h->stats[7] = (mode == 1 && h->pdl && h->variant == 2 && !use_qrec(h)) ? 1 : 0;
+    h->stats[7] = (mode == 1 && h->pdl && h->variant >= 2 && !use_qrec(h)) ? 1 : 0;
     h->stats[1] = launched_outside;
     h->stats[2] = mode;
     // unfused: K1 r,p -> p,q (4N); K2 x,p,r,q -> x,r (6N).  xfuse: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)

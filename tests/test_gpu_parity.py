@@ -55,7 +55,7 @@ def test_gpu_operator_symmetric_and_constant_closed_form():
 # ------------------------------------------------------------------ full solves: every K1 variant / loop mode
 # (variant, tile, xfuse); xfuse = 2 means xfuse + qrecompute (q not stored, K2 recomputes it: 64 B/cell/it)
 VARIANTS = [(0, 0, 0)] + [(1, t, 0) for t in range(7)] + [(2, t, x) for t in range(7) for x in (0, 1)] \
-    + [(2, 0, 2), (2, 1, 2), (2, 3, 2)]
+    + [(2, 0, 2), (2, 1, 2), (2, 3, 2)] + [(3, t, 1) for t in range(7)]      # variant 3: TMA + mbarrier K1
 
 
 @pytest.mark.parametrize("loop_mode", [1, 0])
@@ -244,7 +244,8 @@ def test_history_longer_than_initial_capacity_and_stream():
 
 
 # ------------------------------------------------------------------ determinism as a race detector
-@pytest.mark.parametrize("variant,tile,xfuse", [(0, 0, 0), (1, 1, 0), (2, 0, 0), (2, 0, 1), (2, 1, 1), (2, 3, 1), (2, 0, 2)])
+@pytest.mark.parametrize("variant,tile,xfuse", [(0, 0, 0), (1, 1, 0), (2, 0, 0), (2, 0, 1), (2, 1, 1), (2, 3, 1), (2, 0, 2), (3, 0, 1), (3, 1, 1),
+                                                (3, 3, 1)])
 def test_rerun_bit_identity_every_kernel_family(variant, tile, xfuse):
     """north_star (3): deterministic reductions => a rerun gives the same bits.  compute-sanitizer is closed on
     this GPU pool, so this doubles as the race check of the shared-memory rings: a missing barrier shows up as

@@ -17,7 +17,7 @@ def _t(a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
 
 
-@pytest.mark.parametrize("tile", [0, 1, 2, 3, 4, 5, 6, 7])      # 6, 7: TMA bulk-copy + mbarrier variant
+@pytest.mark.parametrize("tile", list(range(12)))      # 6, 7: TMA bulk-copy + mbarrier variant
 @pytest.mark.parametrize("shape,bc", [((9, 11, 70), (0, 0)), ((21, 19, 134), (1, 0)), ((1, 1, 2), (0, 0)),
                                       ((5, 17, 260), (1, 1)), ((40, 9, 128), (0, 1))])
 def test_lop_and_apply_match_oracle_general_mesh(shape, bc, tile):
@@ -47,7 +47,7 @@ def test_lop_uniform_phi_and_baseline_apply_kernel_agree():
         assert np.abs(a - a_ref).max() <= H.APPLY_RTOL * np.abs(a_ref).max()
 
 
-@pytest.mark.parametrize("tile", [0, 1, 3, 4, 6, 7])
+@pytest.mark.parametrize("tile", [0, 1, 3, 4, 6, 7, 8, 11])
 @pytest.mark.parametrize("s", [2, 3, 5, 16, 64])
 @pytest.mark.parametrize("uniform", [False, True])
 def test_sts_advance_matches_oracle(s, uniform, tile):

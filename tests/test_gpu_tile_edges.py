@@ -38,7 +38,7 @@ def test_stencil_kernels_all_tiles_ragged_phi(np_, uniform):
     oref, gpu = H.both_ops(mesh, dt, nu_kind, nu, bc)
     u = np.random.default_rng(np_).standard_normal(mesh.shape)
     a_ref, l_ref = oref.apply(u), oref.lop(u)
-    for tile in range(8):
+    for tile in range(12):
         gpu.set_option("stencil_tile", tile)
         a = gpu.apply(_t(u)).cpu().numpy().reshape(mesh.shape)
         l = gpu.lop(_t(u)).cpu().numpy().reshape(mesh.shape)
@@ -59,7 +59,7 @@ def test_pcg_kernel_families_ragged_phi(np_, uniform):
     b, x0 = rng.uniform(-1, 1, mesh.shape), rng.standard_normal(mesh.shape)
     for variant, tile, xfuse, qrec, persistent in [(0, 0, 0, 0, 0), (1, 0, 0, 0, 0), (1, 3, 0, 0, 0), (2, 0, 0, 0, 0),
                                                    (2, 0, 1, 0, 0), (2, 2, 1, 0, 0), (2, 5, 1, 0, 0), (2, 0, 1, 1, 0),
-                                                   (2, 0, 1, 0, 1)]:
+                                                   (2, 0, 1, 0, 1), (3, 0, 1, 0, 0), (3, 1, 1, 0, 0), (3, 2, 1, 0, 0), (3, 5, 1, 0, 0)]:
         for name, val in (("persistent", persistent), ("variant", variant), ("tile", tile), ("xfuse", xfuse),
                           ("qrecompute", qrec)):
             gpu.set_option(name, val)
@@ -74,7 +74,7 @@ def test_sts_ragged_theta(nt):
     tau = 40.0 / gpu.lambda_max()
     s = gpu.sts_stages(tau)
     y_ref = oref.sts(u, tau, s)
-    for tile in (0, 1, 3, 4, 6, 7):
+    for tile in (0, 1, 3, 4, 6, 7, 9, 10):
         gpu.set_option("stencil_tile", tile)
         ud = _t(u)
         gpu.sts_advance(ud, tau, s)
