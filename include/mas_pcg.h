@@ -108,15 +108,18 @@ int mas_pcg_mix_probe(mas_pcg_t *h, int which, int reps, void *stream, double *m
  *   [0] kernels launched inside the iteration loop, [1] kernels launched outside it,
  *   [2] loop mode used (1 = CUDA-graph WHILE node, 0 = host-driven chunks, 2 = one persistent cooperative kernel),
  *   [3] algorithmic bytes per cell per iteration of the kernels in use,
- *   [4] doubles per cell K1 moves, [5] doubles per cell K2 moves, [6..7] reserved (0). */
+ *   [4] doubles per cell K1 moves, [5] doubles per cell K2 moves,
+ *   [6] grid size of the persistent kernel (0 if not used), [7] 1 if the loop body used programmatic (PDL) edges. */
 int mas_pcg_stats(const mas_pcg_t *h, long long *out);
 
 /* Tuning / debugging knob, takes effect at the next solve.  name in
  *   "loop_mode" (0 host chunks, 1 graph while), "variant" (K1: 0 baseline, 1 marching, 2 wide marching with cp.async,
  *   3 wide marching with TMA bulk copies + mbarriers = default),
  *   "tile" (tile configuration of the variant), "ci" (r-chunk length, 0 = automatic),
- *   "xfuse" (1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B), "serpentine" (K2 sweeps
- *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile", "qrecompute" (64 B),
+ *   "xfuse" (variant 2 only; 1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B; variant 3 is always
+ *   fused), "serpentine" (K2 sweeps
+ *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile" (0..5 cp.async, 6..11 TMA),
+ *   "qrecompute" (variant 2 only: 64 B), "k2r_tile",
  *   "unroll" (PCG iterations per WHILE trip of the graph loop, 1..16), "pdl" (programmatic dependent launch
  *   edges inside the loop body; default 0: measured slower),
  *   "persistent" (small meshes: whole solve in one cooperative kernel; 0 off, 1 whenever it fits, 2 auto).
