@@ -696,7 +696,19 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     size_t psmem = 0;
     const void *pfunc = nullptr;
     const bool persistent = plan_persistent(h, &ppar, &pgrid, &psmem, &pfunc);
-    if (persistent) mode = 2;
+    long long launched_outside = 2, launched_loop = 0;
+    if (persistent) {                      // init + loop + finish in one cooperative kernel
+        OpDev op = h->op;
+        void *kargs[2] = {&op, &ppar};
+        if (cudaLaunchCooperativeKernel(pfunc, dim3(pgrid), dim3(PNT), kargs, psmem, s) == cudaSuccess) {
+            mode = 2;
+            launched_outside = 0;
+            launched_loop = 1;
+        } else {
+            cudaGetLastError();            // refused (e.g. co-residency limits): use the streaming loop instead
+            h->coop_ok = 0;
+        }
+    }
     if (mode == 1 && (h->graph_dirty || !h->exec)) {
         if (build_graph(h) != MAS_OK && h->pdl) {   // programmatic edges refused: plain edges
             h->pdl = 0;
@@ -707,13 +719,8 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
             mode = 0;
         }
     }
-    long long launched_outside = 2, launched_loop = 0;
-    if (mode == 2) {                       // init + loop + finish in one cooperative kernel
-        OpDev op = h->op;
-        void *kargs[2] = {&op, &ppar};
-        CK(cudaLaunchCooperativeKernel(pfunc, dim3(pgrid), dim3(PNT), kargs, psmem, s));
-        launched_outside = 0;
-        launched_loop = 1;
+    if (mode == 2) {
+        // launched above
     } else if (mode == 1) {
         CK(cudaGraphLaunch(h->exec, s));
     } else {
