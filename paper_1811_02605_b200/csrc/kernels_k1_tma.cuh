@@ -61,25 +61,7 @@ k1_tma(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int use
     const int kl = k0 == 0 ? op.np - 1 : k0 - 1;           // odd
     const int kr = k0 + tkeff >= op.np ? 0 : k0 + tkeff;   // even
 
-    // ---- operator-only prologue: coefficient columns, phi factors, zero-fill, barrier init ----
-    for (int e = tid; e < nsteps * NW; e += NT) {
-        const int pl = e / NW, wr = e - pl * NW;
-        const int ii = first + pl, jj = jt * TJ + wr - 1;
-        const bool in = ii >= 0 && ii < op.nr && jj >= 0 && jj < op.nt;
-        const int row = ii * op.nt + jj;
-        sm.cE[pl][wr] = in ? __ldg(op.E + row) : 0.0;
-        sm.cF[pl][wr] = in ? __ldg(op.F + row) : 0.0;
-        sm.cD[pl][wr] = in ? __ldg(op.Dinv + row) : 0.0;
-        sm.cAR[pl][wr] = (ii >= 0 && ii <= op.nr && jj >= 0 && jj < op.nt) ? __ldg(op.AR + row) : 0.0;
-        sm.cAT[pl][wr] = (ii >= 0 && ii < op.nr && jj >= 0 && jj <= op.nt) ? __ldg(op.AT + ii * (op.nt + 1) + jj) : 0.0;
-    }
-    if (!UNIFORM)
-        for (int e = tid; e < WIDE_TK + 2; e += NT) {
-            int kk = k0 - 1 + e;
-            kk = kk < 0 ? kk + op.np : (kk >= op.np ? kk - op.np : kk);
-            kk = kk >= op.np ? kk % op.np : kk;
-            sm.phv[e] = __ldg(op.vp + kk); sm.phw[e] = __ldg(op.wp + kk); sm.phi[e] = __ldg(op.ip + kk);
-        }
+    // ---- zero-fill and barrier init first, so that the first bulk copies can be issued as early as possible ----
     const double2 zero2 = make_double2(0.0, 0.0);
 #pragma unroll
     for (int s = 0; s < DEPTH; s++) {
@@ -147,6 +129,27 @@ k1_tma(OpDev op, Work w, WideParams mp, cudaGraphConditionalHandle cond, int use
     };
     if (lane == 0)
         for (int pl = 0; pl < DEPTH && pl < nsteps; pl++) produce(pl);
+
+    // ---- coefficient columns and phi factors, staged while the first planes are already in flight ----
+    for (int e = tid; e < nsteps * NW; e += NT) {
+        const int pl = e / NW, wr = e - pl * NW;
+        const int ii = first + pl, jj = jt * TJ + wr - 1;
+        const bool in = ii >= 0 && ii < op.nr && jj >= 0 && jj < op.nt;
+        const int row = ii * op.nt + jj;
+        sm.cE[pl][wr] = in ? __ldg(op.E + row) : 0.0;
+        sm.cF[pl][wr] = in ? __ldg(op.F + row) : 0.0;
+        sm.cD[pl][wr] = in ? __ldg(op.Dinv + row) : 0.0;
+        sm.cAR[pl][wr] = (ii >= 0 && ii <= op.nr && jj >= 0 && jj < op.nt) ? __ldg(op.AR + row) : 0.0;
+        sm.cAT[pl][wr] = (ii >= 0 && ii < op.nr && jj >= 0 && jj <= op.nt) ? __ldg(op.AT + ii * (op.nt + 1) + jj) : 0.0;
+    }
+    if (!UNIFORM)
+        for (int e = tid; e < WIDE_TK + 2; e += NT) {
+            int kk = k0 - 1 + e;
+            kk = kk < 0 ? kk + op.np : (kk >= op.np ? kk - op.np : kk);
+            kk = kk >= op.np ? kk % op.np : kk;
+            sm.phv[e] = __ldg(op.vp + kk); sm.phw[e] = __ldg(op.wp + kk); sm.phi[e] = __ldg(op.ip + kk);
+        }
+    __syncthreads();                            // coefficient columns visible
 
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
