@@ -54,7 +54,7 @@ def parse():
     ap.add_argument("--opt", action="append", default=[], help="name=value passed to mas_pcg_set_option (tuning)")
     ap.add_argument("--k2r-tile", type=int, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--chain-steps", type=int, default=20,
+    ap.add_argument("--chain-steps", type=int, default=100,
                     help="--workload c5: consecutive solves timed (BASELINE.json config 5 has 100)")
     return ap.parse_args()
 
@@ -210,32 +210,47 @@ def run_reference(args, rank, world):
 
 
 def run_chain(args):
-    """BASELINE.json config 5, time-step proxy: consecutive warm-started solves on 192x256x384, dt varying
+    """BASELINE.json config 5, time-step proxy: 100 consecutive warm-started solves on 192x256x384, dt varying
     +-20 % per step, RHS(k+1) = x(k) + 0.05 N(0,1).  Timed per solve with CUDA events (set_dt + solve);
-    RHS construction and its H2D copy are outside the timed regions."""
+    RHS construction and its H2D copy are outside the timed regions.  `e2e` is the same chain
+    through mas_pcg_solve_host (pinned host RHS and x; the copies are inside the timed call), run in lock-step
+    with the device-resident chain so that one noise draw per step serves both."""
     import numpy as np
     import torch
     from mas_inputs import configs
     from paper_1811_02605_b200 import MasPcg
     torch.cuda.set_device(0)
     prob = configs.make("c5")
+    nsteps = max(args.chain_steps, 1)
     dt0 = prob.dt_for(prob.stiffness[-1])
-    chain = configs.Chain(prob, max(args.chain_steps, 1))
+    chain = configs.Chain(prob, 100)
     gpu = MasPcg(prob.mesh, dt0, prob.nu_kind, prob.nu, prob.bc)
+    for kv in args.opt:
+        name, val = kv.split("=")
+        gpu.set_option(name, int(val))
     stream = torch.cuda.current_stream()
+    n = prob.mesh.ncells
     x = torch.zeros(prob.mesh.shape, dtype=torch.float64, device="cuda")
-    rhs = torch.from_numpy(chain.state0 + chain.noise()).cuda()
-    # warm-up on a scratch vector (graph build, clocks)
+    rhs_host = torch.from_numpy(chain.state0 + chain.noise()).pin_memory()
+    x_host = torch.zeros(prob.mesh.shape, dtype=torch.float64).pin_memory()
+    rhs = rhs_host.cuda()
+    rhs0_np = rhs_host.numpy().copy()
+    # warm-up on scratch vectors (graph build, staging buffers, clocks)
     xs = torch.zeros_like(x)
     for _ in range(max(args.warmup, 3)):
         xs.zero_()
         gpu.solve(rhs, xs, prob.rtol, prob.maxit, want_hist=False)
-    total_ms, iters, launches = 0.0, [], 0
-    for step in range(args.chain_steps):
+    gpu.solve_host(rhs_host, x_host, prob.rtol, prob.maxit, want_hist=False)
+    x_host.zero_()
+    sampler = ClockSampler(gpu_selector(torch))
+    sampler.start()
+    total_ms, e2e_s, iters, launches = 0.0, 0.0, [], 0
+    for step in range(nsteps):
+        dt = dt0 * chain.dt_factor[step]
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record(stream)
-        gpu.set_dt(dt0 * chain.dt_factor[step])
+        gpu.set_dt(dt)
         st, k, _ = gpu.solve(rhs, x, prob.rtol, prob.maxit, want_hist=False)      # x: warm start, in place
         e1.record(stream)
         torch.cuda.synchronize()
@@ -245,20 +260,55 @@ def run_chain(args):
         launches += sstat["loop_launches"] + sstat["other_launches"] + 1
         if st != 0:
             raise SystemExit(f"chain step {step}: status {st}")
-        rhs = x + torch.from_numpy(chain.noise()).cuda()                           # untimed
-    n = prob.mesh.ncells
+        t0 = time.perf_counter()                                                   # end to end: host buffers
+        gpu.set_dt(dt)
+        st2, k2, _ = gpu.solve_host(rhs_host, x_host, prob.rtol, prob.maxit, want_hist=False)
+        e2e_s += time.perf_counter() - t0
+        if (st2, k2) != (st, k):
+            raise SystemExit(f"chain step {step}: host-buffer solve differs ({st2}, {k2}) vs ({st}, {k})")
+        if step + 1 < nsteps:                                                      # untimed: next right-hand side
+            rhs_host.copy_(x_host + torch.from_numpy(chain.noise()))
+            rhs.copy_(rhs_host)
+    clocks = sampler.stop()
     bpc = gpu.stats()["bytes_per_cell_iter"]
-    line = {"metric": "pcg_solves_per_s_192x256x384_timestep_proxy", "value": args.chain_steps / (total_ms * 1e-3),
-            "unit": "solves/s", "n_gpus": 1, "steps": args.chain_steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": total_ms / args.chain_steps, "higher_is_better": True, "scaling": "weak",
+    peak, peak_src = hbm_peak()
+    its = float(np.sum(iters))
+    gbs = bpc * n * its / (total_ms * 1e-3) / 1e9
+    line = {"metric": "pcg_solves_per_s_192x256x384_timestep_proxy", "value": nsteps / (total_ms * 1e-3),
+            "unit": "solves/s", "n_gpus": 1, "steps": nsteps, "warmup": max(args.warmup, 3),
+            "ms_per_step": total_ms / nsteps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"c5: 192x256x384 fp64, s=100 at dt0, dt +-20 %/step, warm start, rtol 1e-9, "
-                                   f"first {args.chain_steps} of 100 chained solves",
-                       "mean_iters_per_solve": float(np.mean(iters)), "iters": iters,
-                       "bytes_per_cell_iter": bpc},
-            "iterations_per_s": float(np.sum(iters)) / (total_ms * 1e-3),
-            "model_gbs": bpc * n * float(np.sum(iters)) / (total_ms * 1e-3) / 1e9,
-            "gpu_launches": int(launches)}
+                                   f"{'all' if nsteps == 100 else 'first ' + str(nsteps) + ' of'} 100 chained solves",
+                       "l2": "inputs larger than L2 (5 live vectors x 151 MB vs 126 MB)",
+                       "mean_iters_per_solve": float(np.mean(iters)), "iters": iters, "bytes_per_cell_iter": bpc},
+            "iterations_per_s": its / (total_ms * 1e-3),
+            "clocks": clocks,
+            "e2e": {"value": nsteps / e2e_s, "unit": "solves/s", "h2d_bytes_per_step": 2 * 8 * n,
+                    "d2h_bytes_per_step": 8 * n},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "kernel": "whole solve (init + iterations + tail), model bytes = "
+                                                   f"{bpc} B/cell/iteration x iterations",
+                         "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                         "peak_source": peak_src}}
+    if not args.no_cpu_baseline:
+        from oracle import ref
+        op = ref.RefOperator(prob.mesh, dt0, prob.nu_kind, prob.nu, prob.bc)
+        ch = configs.Chain(prob, 100)
+        b, xo, t_or, k_or = rhs0_np, None, 0.0, []
+        ch.noise()                                          # the draw that made rhs0
+        for step in range(3):
+            op.set_dt(dt0 * ch.dt_factor[step])
+            t0 = time.perf_counter()
+            st_o, k_o, xo, _ = op.pcg(b, xo, prob.rtol, prob.maxit)
+            t_or += time.perf_counter() - t0
+            k_or.append(k_o)
+            b = xo + ch.noise()
+        op.close()
+        line["cpu_baseline"] = {"value": 3 / t_or, "unit": "solves/s", "cores": 1, "kind": "oracle",
+                                "sample": f"3-solve prefix of the chain (x100/3 extrapolates to the 100 solves), "
+                                          f"iterations {k_or} vs GPU {iters[:3]}, one thread of {os.cpu_count()} "
+                                          f"host cores, gcc -O2"}
     print(json.dumps(line), flush=True)
 
 
@@ -519,7 +569,18 @@ def main():
                           "frac_of_peak": bpc * n / (it_ms * 1e-3) / 1e9 / peak,
                           "frac_of_nominal_8000": bpc * n / (it_ms * 1e-3) / 1e9 / 8000.0},
         }
-        if world == 1 and not args.no_cpu_baseline:
+        if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
+            from oracle import ref                      # config 3 = the oracle's FULL solve
+            op = ref.RefOperator(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)
+            t0 = time.perf_counter()
+            st_o, k_o, _, _ = op.pcg(b_np, None, rtol, maxit)
+            t_o = time.perf_counter() - t0
+            op.close()
+            line["cpu_baseline"] = {
+                "value": k_o / t_o, "unit": UNIT, "cores": 1, "kind": "oracle",
+                "sample": f"full solve of the same workload: {k_o} iterations (GPU {k}) in {t_o:.1f} s including setup "
+                          f"and the initial residual, one thread of {os.cpu_count()} host cores, gcc -O2"}
+        elif world == 1 and not args.no_cpu_baseline:
             nit = CPU_BASELINE_ITERS if args.workload in ("c4", "c5") else 40
             t_a, _ = time_oracle(prob, dt, b_np, 2)
             t_b, _ = time_oracle(prob, dt, b_np, 2 + nit)

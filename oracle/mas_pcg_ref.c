@@ -232,6 +232,10 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
     mas_ref_volume(op, z);                       /* z used as scratch for V */
     for (size_t c = 0; c < n; c++) r[c] = z[c] * b_phys[c];     /* b_s = V.b */
     const double bb = dot(n, r, r);
+    if (!isfinite(bb)) {                         /* a non-finite scalar is a breakdown; x untouched */
+        if (hist) hist[0] = bb;
+        *iters = 0; status = REF_EBREAKDOWN; goto done;
+    }
     if (bb == 0.0) {                             /* zero right-hand side: x = 0 */
         memset(x, 0, n * sizeof(double));
         if (hist) hist[0] = 0.0;
@@ -245,6 +249,7 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
     double h = sqrt(rr / bb);
     if (hist) hist[0] = h;
     status = REF_OK;
+    if (!isfinite(rho) || !isfinite(rr)) { *iters = 0; status = REF_EBREAKDOWN; goto done; }
     while (k < maxit && h > rtol && rho != 0.0) {
         mas_ref_apply(op, p, q);
         const double sigma = dot(n, p, q);
@@ -258,6 +263,7 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
         k += 1;
         h = sqrt(rr / bb);
         if (hist) hist[k] = h;
+        if (!isfinite(rho1) || !isfinite(rr)) { status = REF_EBREAKDOWN; break; }   /* iterate k is kept */
         const double beta = rho1 / rho;
         rho = rho1;
         for (size_t c = 0; c < n; c++) p[c] = z[c] + beta * p[c];
@@ -267,6 +273,28 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
 done:
     free(d); free(r); free(z); free(p); free(q);
     return status;
+}
+
+/*
+ * NEXT-2: several right-hand sides that share one operator -- the three components of v in
+ * PAPER.md:50 eq. (1) "share one coefficient set".  By definition this is nrhs INDEPENDENT textbook solves,
+ * each with its own alpha, beta, iteration count, status and history: nothing is coupled across right-hand
+ * sides.  b, x: nrhs vectors stored back to back (nrhs * N doubles); hist: NULL or nrhs * (maxit + 1) doubles,
+ * right-hand side j's history starting at hist + j * (maxit + 1); iters, status: nrhs ints.
+ * Returns the most severe status (negative before MAXIT before OK).
+ */
+int mas_ref_pcg_multi(const ref_op *op, int nrhs, const double *b_phys, double *x, double rtol, int maxit,
+                      int *iters, int *status, double *hist)
+{
+    if (!op || nrhs < 1 || !b_phys || !x || !iters || !status) return REF_EINVAL;
+    const size_t n = (size_t)op->nr * op->nt * op->np;
+    int worst = REF_OK;
+    for (int j = 0; j < nrhs; j++) {
+        status[j] = mas_ref_pcg(op, b_phys + (size_t)j * n, x + (size_t)j * n, rtol, maxit, &iters[j],
+                                hist ? hist + (size_t)j * ((size_t)maxit + 1) : NULL);
+        if (status[j] < 0 ? (worst >= 0 || status[j] < worst) : (worst >= 0 && status[j] > worst)) worst = status[j];
+    }
+    return worst;
 }
 
 /* ==============================================================================================

@@ -50,6 +50,9 @@ def lib():
         L.mas_ref_pcg.restype = ctypes.c_int
         L.mas_ref_pcg.argtypes = [ctypes.c_void_p, _dp, _dp, ctypes.c_double, ctypes.c_int,
                                   ctypes.POINTER(ctypes.c_int), _dp]
+        L.mas_ref_pcg_multi.restype = ctypes.c_int
+        L.mas_ref_pcg_multi.argtypes = [ctypes.c_void_p, ctypes.c_int, _dp, _dp, ctypes.c_double, ctypes.c_int,
+                                        ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int), _dp]
         L.mas_ref_lop.argtypes = [ctypes.c_void_p, _dp, _dp]
         L.mas_ref_lambda_max_bound.restype = ctypes.c_double
         L.mas_ref_lambda_max_bound.argtypes = [ctypes.c_void_p]
@@ -118,6 +121,19 @@ class RefOperator:
         it = ctypes.c_int(0)
         st = lib().mas_ref_pcg(self._h, _p(b), _p(x), float(rtol), int(maxit), ctypes.byref(it), _p(hist))
         return st, it.value, x, hist[: it.value + 1].copy()
+
+    def pcg_multi(self, b_phys: np.ndarray, x0: np.ndarray | None, rtol: float, maxit: int):
+        """nrhs independent solves sharing the operator; b_phys has shape (nrhs, nr, nt, np).
+        Returns (worst status, [status_j], [iters_j], x (nrhs, ...), [hist_j[0..iters_j]])."""
+        b = np.ascontiguousarray(b_phys, dtype=np.float64)
+        nrhs = b.shape[0]
+        assert b.shape[1:] == self.shape
+        x = np.zeros_like(b) if x0 is None else np.array(x0, dtype=np.float64, order="C").reshape(b.shape)
+        hist = np.full((nrhs, maxit + 1), np.nan)
+        it = (ctypes.c_int * nrhs)()
+        st = (ctypes.c_int * nrhs)()
+        worst = lib().mas_ref_pcg_multi(self._h, nrhs, _p(b), _p(x), float(rtol), int(maxit), it, st, _p(hist))
+        return worst, list(st), list(it), x, [hist[j, : it[j] + 1].copy() for j in range(nrhs)]
 
     # ---- NEXT-1: explicit operator and RKL2 super time stepping ----
     def lop(self, u: np.ndarray) -> np.ndarray:

@@ -150,7 +150,11 @@ def _solve(fn, where, handle, b_ptr, x_ptr, rtol, maxit, stream, want_hist):
     st = fn(handle, b_ptr, x_ptr, float(rtol), int(maxit), stream, ctypes.byref(it),
             hist.ctypes.data_as(_dp) if want_hist else None)
     if st < 0:
-        raise MasError(st, where)
+        err = MasError(st, where)
+        if st == MAS_EBREAKDOWN:                 # x holds the last iterate; the count and history are meaningful
+            err.iters = it.value
+            err.hist = hist[: it.value + 1].copy() if want_hist else None
+        raise err
     return st, it.value, (hist[: it.value + 1].copy() if want_hist else None)
 
 

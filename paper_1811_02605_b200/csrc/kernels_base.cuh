@@ -177,7 +177,10 @@ __global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditio
         st->beta = 0.0; st->alpha = 0.0; st->sigma = 0.0;
         st->k = 0; st->launches = 0;
         int active = 0, status = ST_OK;
-        if (bb == 0.0) {
+        if (!isfinite(bb) || !isfinite(rr) || !isfinite(rho)) {
+            w.hist[0] = sqrt(rr / bb);          // a non-finite scalar (NaN / Inf in b or x0): breakdown, x untouched
+            status = ST_BREAKDOWN;
+        } else if (bb == 0.0) {
             w.hist[0] = 0.0;                    // zero RHS: x = 0 (host zeroes x), 0 iterations
         } else {
             const double h = sqrt(rr / bb);
@@ -208,8 +211,11 @@ __device__ __forceinline__ void k2_finish(State *st, const Work &w, double rho1,
     st->rr = rr;
     st->k = k;
     st->launches += 1;
-    const int active = (k < w.args->maxit) && (h > w.args->rtol) && (rho1 != 0.0);
-    if (!active) st->status = (h <= w.args->rtol || rho1 == 0.0) ? ST_OK : ST_MAXIT;
+    int active = (k < w.args->maxit) && (h > w.args->rtol) && (rho1 != 0.0);
+    if (!isfinite(rho1) || !isfinite(rr)) {            // iterate k is kept (the pending x-update is applied by the tail)
+        active = 0;
+        st->status = ST_BREAKDOWN;
+    } else if (!active) st->status = (h <= w.args->rtol || rho1 == 0.0) ? ST_OK : ST_MAXIT;
     st->active = active;
     set_cond(cond, use_cond, active);
 }

@@ -151,7 +151,10 @@ __global__ void __launch_bounds__(PNT, 1) k_pcg_persistent(OpDev op, PersistPara
     double rho = acc3[2], rr = acc3[1], beta = 0.0, alpha = 0.0;
     int k = 0, status = ST_OK, active = 0;
     double h = 0.0;
-    if (bb != 0.0) {
+    if (!isfinite(bb) || !isfinite(rr) || !isfinite(rho)) {
+        h = sqrt(rr / bb);
+        status = ST_BREAKDOWN;
+    } else if (bb != 0.0) {
         h = sqrt(rr / bb);
         active = (0 < maxit) && (h > rtol) && (rho != 0.0);
         if (!active) status = (h <= rtol || rho == 0.0) ? ST_OK : ST_MAXIT;
@@ -209,7 +212,8 @@ __global__ void __launch_bounds__(PNT, 1) k_pcg_persistent(OpDev op, PersistPara
         beta = rho1 / rho;
         rho = rho1;
         active = (k < maxit) && (h > rtol) && (rho1 != 0.0);
-        if (!active) status = (h <= rtol || rho1 == 0.0) ? ST_OK : ST_MAXIT;
+        if (!isfinite(rho1) || !isfinite(rr)) { active = 0; status = ST_BREAKDOWN; }
+        else if (!active) status = (h <= rtol || rho1 == 0.0) ? ST_OK : ST_MAXIT;
     }
     // ---- finish ----
     for (int m = 0; m < M; m++) {

@@ -25,3 +25,25 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+def pytest_terminal_summary(terminalreporter):
+    """Observed GPU-vs-oracle gaps (VERDICT r1 #7/#8: print what is seen, not only that the gate held)."""
+    from tests import helpers
+    if not helpers.GAPS:
+        return
+    tr = terminalreporter
+    tr.write_sep("-", "observed GPU-vs-oracle gaps")
+    worst = {}
+    for label, kw in helpers.GAPS:
+        for k, v in kw.items():
+            if k.startswith("k_"):
+                continue
+            if k not in worst or v > worst[k][0]:
+                worst[k] = (v, label)
+    for k, (v, label) in sorted(worst.items()):
+        tr.write_line(f"max {k:6s} = {v:.3e}   ({label})")
+    big = [(l, kw) for l, kw in helpers.GAPS if any(t in l for t in ("c3", "c4", "c5")) and "x_l2" in kw]
+    for label, kw in big:
+        tr.write_line(f"{label}: hist {kw['hist']:.2e}  x_l2 {kw['x_l2']:.2e}  x_max {kw['x_max']:.2e}  "
+                      f"k {kw['k_gpu']}/{kw['k_ref']}")

@@ -15,6 +15,21 @@ X_RTOL = 1e-9          # final x, relative L2, compared at EQUAL iteration count
 APPLY_RTOL = 1e-13     # single matvec, relative to max |A u| (pure rounding-order difference)
 
 
+# observed GPU-vs-oracle gaps, collected per test and printed by conftest.pytest_terminal_summary
+GAPS = []
+
+
+def record_gap(label, **kw):
+    GAPS.append((label, kw))
+
+
+def apply_gap(y, y_ref, label):
+    """max |y - y_ref| / max |y_ref| of a single matvec; recorded, returned for the assertion."""
+    g = float(np.abs(y - y_ref).max() / max(np.abs(y_ref).max(), 1e-300))
+    record_gap(label, apply=g)
+    return g
+
+
 def oracle_s1(mesh, nu_kind, nu, bc=(0, 0)) -> float:
     op = ref.RefOperator(mesh, 1.0, nu_kind, nu, bc)
     s1 = op.stiffness_max()
@@ -54,5 +69,10 @@ def check_parity(gpu, oref, b, x0, rtol, maxit, *, label=""):
         assert k_g2 == k_r
     xg = xd.cpu().numpy().reshape(x_r.shape)
     err = np.linalg.norm(xg - x_r) / np.linalg.norm(x_r)
+    # element-wise: the largest single-cell gap relative to max |x| (a localised error in a few boundary
+    # rows would hide under the L2 gate on a large mesh); reported, and gated at 100x the L2 tolerance
+    emax = float(np.abs(xg - x_r).max() / np.abs(x_r).max())
+    record_gap(label, hist=float(rel.max()), x_l2=float(err), x_max=emax, k_ref=k_r, k_gpu=k_g)
     assert err <= X_RTOL, f"{label}: x gap {err:.3e}"
+    assert emax <= 100 * X_RTOL, f"{label}: element-wise x gap {emax:.3e}"
     return k_r, k_g

@@ -24,7 +24,7 @@ def test_apply_matches_oracle_general_mesh(shape, bc):
     u = np.random.default_rng(1).standard_normal(mesh.shape)
     y_ref = oref.apply(u)
     y = gpu.apply(_t(u)).cpu().numpy().reshape(mesh.shape)
-    assert np.abs(y - y_ref).max() <= H.APPLY_RTOL * np.abs(y_ref).max()
+    assert H.apply_gap(y, y_ref, f"apply {shape} bc{bc}") <= H.APPLY_RTOL
 
 
 def test_apply_matches_oracle_uniform_phi_config1():
@@ -33,7 +33,19 @@ def test_apply_matches_oracle_uniform_phi_config1():
     u = configs.rhs_uniform(prob)
     y_ref = oref.apply(u)
     y = gpu.apply(_t(u)).cpu().numpy().reshape(prob.mesh.shape)
-    assert np.abs(y - y_ref).max() <= H.APPLY_RTOL * np.abs(y_ref).max()
+    assert H.apply_gap(y, y_ref, "apply c1") <= H.APPLY_RTOL
+
+
+@pytest.mark.parametrize("name,s", [("c3", 1e4), ("c5", 100.0)])
+def test_apply_matches_oracle_full_size_stiff(name, s):
+    """The standalone matvec at a BASELINE.json size and stiffness (coefficient form on the GPU against the
+    oracle's flux-difference form: the cancellation in d*u - sum(c*u_nb) grows with s)."""
+    prob = configs.make(name)
+    oref, gpu = H.both_ops(prob.mesh, prob.dt_for(s), prob.nu_kind, prob.nu)
+    u = np.random.default_rng(11).standard_normal(prob.mesh.shape)
+    y_ref = oref.apply(u)
+    y = gpu.apply(_t(u)).cpu().numpy().reshape(prob.mesh.shape)
+    assert H.apply_gap(y, y_ref, f"apply {name} s={s:g}") <= H.APPLY_RTOL
 
 
 def test_gpu_operator_symmetric_and_constant_closed_form():
@@ -183,6 +195,108 @@ def test_config5_chain_first_3_solves():
         H.check_parity(gpu, oref, rhs, x_prev, prob.rtol, prob.maxit, label=f"c5 step {step}")
         _, _, x_prev, _ = oref.pcg(rhs, x_prev, prob.rtol, prob.maxit)
         rhs = x_prev + chain.noise()
+
+
+def test_config5_full_size_first_3_solves():
+    """BASELINE.json configs[4] at its stated size, 192x256x384 (18.9 M cells), with the calibrated dt0
+    (s = 100): set_dt per step, warm start, the first 3 of the 100 chained solves,
+    gates unchanged.  Both sides get the SAME right-hand sides, built from the oracle's x_k."""
+    prob = configs.make("c5")
+    dt0 = prob.dt_for(100.0)
+    oref, gpu = H.both_ops(prob.mesh, dt0, prob.nu_kind, prob.nu)
+    chain = configs.Chain(prob, 100)
+    rhs = chain.state0 + chain.noise()
+    x_prev = None
+    for step in range(3):
+        dt = dt0 * chain.dt_factor[step]
+        oref.set_dt(dt)
+        gpu.set_dt(dt)
+        k_r, k_g = H.check_parity(gpu, oref, rhs, x_prev, prob.rtol, prob.maxit, label=f"c5 full step {step}")
+        assert 30 <= k_r <= 120                      # the paper's "easy" regime, ~70 iterations (PAPER.md:74)
+        _, _, x_prev, _ = oref.pcg(rhs, x_prev, prob.rtol, prob.maxit)
+        rhs = x_prev + chain.noise()
+
+
+# ------------------------------------------------------------------ breakdown and argument errors
+def _modes(gpu, mode):
+    """mode: 'persistent' (one cooperative kernel), 'graph' (CUDA-graph WHILE loop), 'host' (host chunks)."""
+    gpu.set_option("persistent", 1 if mode == "persistent" else 0)
+    gpu.set_option("loop_mode", 0 if mode == "host" else 1)
+
+
+@pytest.mark.parametrize("mode", ["persistent", "graph", "host"])
+def test_breakdown_nonfinite_rhs_at_init(mode):
+    """A NaN in b makes bb non-finite: MAS_EBREAKDOWN with k = 0 on every loop path, as in the oracle
+    ("non-finite scalar"); x is left as x0."""
+    import torch
+    from paper_1811_02605_b200 import MasError
+    mesh, dt, nu_kind, nu = H.general_case(12, 10, 66, s=50.0)
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    _modes(gpu, mode)
+    rng = np.random.default_rng(9)
+    b, x0 = rng.uniform(-1, 1, mesh.shape), rng.standard_normal(mesh.shape)
+    b[3, 4, 5] = np.nan
+    st_r, k_r, x_r, _ = oref.pcg(b, x0, 1e-10, 100)
+    assert (st_r, k_r) == (ref.REF_EBREAKDOWN, 0) and np.array_equal(x_r, x0)
+    xd = _t(x0)
+    with pytest.raises(MasError) as e:
+        gpu.solve(_t(b), xd, 1e-10, 100)
+    assert e.value.status == -4 and e.value.iters == 0
+    assert np.array_equal(xd.cpu().numpy(), x0)
+    # the handle stays usable: a clean solve afterwards
+    b[3, 4, 5] = 0.25
+    H.check_parity(gpu, oref, b, x0, 1e-10, 500, label=f"after breakdown {mode}")
+
+
+@pytest.mark.parametrize("mode", ["persistent", "graph", "host"])
+def test_breakdown_sigma_overflow_in_first_matvec(mode):
+    """p.Ap overflows to +Inf in the first K1 while bb, rr and rho are still finite: MAS_EBREAKDOWN raised by the
+    matvec kernel's scalar step (S3) at k = 0, and x must still be x0 (nothing pending for the deferred x-update)."""
+    import torch
+    from paper_1811_02605_b200 import MasError
+    mesh = grids.wobbly_phi_mesh(grids.radial_faces_pack(12, 4.0, 1.0, 1.3), 10, 66, 21)   # thin shell: every d < 1,
+    nu = 0.5 + np.random.default_rng(22).uniform(0.0, 1.0, (12, 10))                        # so rr stays below rho
+    dt, nu_kind = 50.0 / H.oracle_s1(mesh, 1, nu), 1
+    oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    assert oref.diag().max() < 1.0
+    _modes(gpu, mode)
+    # a right-hand side whose Jacobi-scaled residual D^-1/2 V b is a 3-D checkerboard: every neighbour has the
+    # opposite sign, so the Rayleigh quotient sigma/rho of D^-1/2 A D^-1/2 is well above 1
+    i, j, k = np.ogrid[:mesh.shape[0], :mesh.shape[1], :mesh.shape[2]]
+    d, V = oref.diag(), oref.volume()
+    b = np.where((i + j + k) % 2 == 0, 1.0, -1.0) * np.sqrt(d) / V
+    b *= 1.0 + 0.1 * np.random.default_rng(3).uniform(-1, 1, mesh.shape)
+    r0 = V * b
+    z0 = r0 / d
+    rho0, sigma0 = float(np.sum(r0 * z0)), float(np.sum(z0 * oref.apply(z0)))
+    assert sigma0 > 1.1 * rho0
+    scale = np.sqrt(np.finfo(np.float64).max / np.sqrt(rho0 * sigma0))      # rho finite, sigma = Inf
+    b *= scale
+    st_r, k_r, x_r, h_r = oref.pcg(b, None, 1e-10, 100)
+    assert (st_r, k_r) == (ref.REF_EBREAKDOWN, 0) and not x_r.any() and np.isfinite(h_r[0])   # the sigma branch
+    xd = torch.zeros(mesh.shape, dtype=torch.float64, device="cuda")
+    with pytest.raises(MasError) as e:
+        gpu.solve(_t(b), xd, 1e-10, 100)
+    assert e.value.status == -4 and e.value.iters == 0
+    assert e.value.hist[0] == pytest.approx(h_r[0], rel=1e-12)
+    assert not xd.any()
+
+
+def test_misaligned_and_aliased_vectors_are_einval():
+    import torch
+    from paper_1811_02605_b200 import binding as B
+    mesh, dt, nu_kind, nu = H.general_case(4, 4, 8)
+    _, gpu = H.both_ops(mesh, dt, nu_kind, nu)
+    n = mesh.shape[0] * mesh.shape[1] * mesh.shape[2]
+    buf = torch.zeros(2 * n + 2, dtype=torch.float64, device="cuda")
+    base = buf.data_ptr()
+    L = B.lib()
+    for b_ptr, x_ptr in [(base + 8, base + 8 * (n + 2)), (base, base + 8 * (n + 1)), (base, base)]:
+        assert L.mas_pcg_solve(gpu._h, b_ptr, x_ptr, 1e-10, 10, None, None, None) == B.MAS_EINVAL
+    assert L.mas_pcg_apply(gpu._h, base, base, None) == B.MAS_EINVAL
+    assert L.mas_pcg_apply(gpu._h, base + 8, base + 8 * (n + 2), None) == B.MAS_EINVAL
+    assert L.mas_pcg_solve(gpu._h, base, base + 8 * (n + 2), -1.0, 10, None, None, None) == B.MAS_EINVAL
+    assert L.mas_pcg_solve(gpu._h, base, base + 8 * (n + 2), 1e-10, -1, None, None, None) == B.MAS_EINVAL
 
 
 # ------------------------------------------------------------------ edge and degenerate cases

@@ -303,3 +303,55 @@ def test_config1_diagonal_dominance_ratio_is_1p5():
     d, V = op.diag(), op.volume()
     offsum = d - V                      # Dirichlet rows have less off-diagonal mass, so >= holds
     assert (d / offsum).min() == pytest.approx(1.5, rel=1e-12)
+
+
+# ------------------------------------------------------------------ breakdown (SURVEY 8(b) MAS_EBREAKDOWN, C3)
+def test_breakdown_nonfinite_rhs_keeps_x0():
+    m, op = tiny_op(s=20.0)
+    rng = np.random.default_rng(9)
+    b, x0 = rng.uniform(-1, 1, m.shape), rng.standard_normal(m.shape)
+    for bad in (np.nan, np.inf):
+        bb = b.copy()
+        bb[1, 2, 3] = bad
+        st, k, x, hist = op.pcg(bb, x0, 1e-10, 50)
+        assert (st, k) == (ref.REF_EBREAKDOWN, 0) and np.array_equal(x, x0) and hist.size == 1
+    st, k, x, hist = op.pcg(b, np.where(np.arange(8) == 2, np.nan, x0), 1e-10, 50)     # NaN in x0: rr, rho non-finite
+    assert (st, k) == (ref.REF_EBREAKDOWN, 0)
+
+
+def test_breakdown_sigma_overflow_stops_before_any_update():
+    """p.Ap = +Inf with bb, rr, rho finite: C3's `!isfinite(sigma)` branch; no iteration is counted, x = x0.
+    (A thin shell r in [1, 1.2]: every d < 1, so rr = sum r^2 stays below rho = sum r^2/d.)"""
+    m, op = tiny_op(s=20.0, mesh=grids.full_sphere_mesh(grids.radial_faces_ratio(4, 1.02, 1.0, 1.2), 4, 8))
+    assert op.diag().max() < 1.0
+    i, j, k = np.ogrid[:4, :4, :8]
+    d, V = op.diag(), op.volume()
+    b = np.where((i + j + k) % 2 == 0, 1.0, -1.0) * np.sqrt(d) / V
+    r0 = V * b
+    z0 = r0 / d
+    rho0, sigma0 = float(np.sum(r0 * z0)), float(np.sum(z0 * op.apply(z0)))
+    assert sigma0 > 1.1 * rho0
+    b *= np.sqrt(np.finfo(np.float64).max / np.sqrt(rho0 * sigma0))
+    st, kk, x, hist = op.pcg(b, None, 1e-10, 50)
+    assert (st, kk) == (ref.REF_EBREAKDOWN, 0) and not x.any() and np.isfinite(hist[0])
+
+
+# ------------------------------------------------------------------ NEXT-2: several right-hand sides, one operator
+def test_pcg_multi_is_three_independent_textbook_solves():
+    """mas_ref_pcg_multi is DEFINED as nrhs single solves (v_r, v_theta, v_phi share one coefficient
+    set, nothing else): bit-equal x, history, count and status per right-hand side, including one that converges
+    at once (zero RHS) and one that hits the iteration cap."""
+    m, nu = varnu_wobbly()
+    _, op = tiny_op(s=300.0, nu_kind=1, nu=nu, mesh=m)
+    rng = np.random.default_rng(31)
+    b = rng.uniform(-1, 1, (3,) + m.shape)
+    b[1] = 0.0
+    x0 = rng.standard_normal((3,) + m.shape)
+    for maxit in (2000, 5):
+        worst, sts, its, x, hists = op.pcg_multi(b, x0, 1e-12, maxit)
+        for jr in range(3):
+            st1, k1, x1, h1 = op.pcg(b[jr], x0[jr], 1e-12, maxit)
+            assert (sts[jr], its[jr]) == (st1, k1)
+            assert np.array_equal(x[jr], x1) and np.array_equal(hists[jr], h1)
+        assert worst == max(sts)
+    assert op.pcg_multi(b, x0, 1e-12, 5)[1] == [ref.REF_MAXIT, ref.REF_OK, ref.REF_MAXIT]
