@@ -42,21 +42,22 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "sts", "visc"])
-    ap.add_argument("--variant", type=int, default=None)
-    ap.add_argument("--tile", type=int, default=None)
-    ap.add_argument("--loop-mode", type=int, default=None)
-    ap.add_argument("--xfuse", type=int, default=None)
-    ap.add_argument("--ci", type=int, default=None)
-    ap.add_argument("--serpentine", type=int, default=None)
-    ap.add_argument("--stencil-tile", type=int, default=None)
-    ap.add_argument("--qrecompute", type=int, default=None)
-    ap.add_argument("--persistent", type=int, default=None)
     ap.add_argument("--opt", action="append", default=[], help="name=value passed to mas_pcg_set_option (tuning)")
-    ap.add_argument("--k2r-tile", type=int, default=None)
+    ap.add_argument("--nrhs", type=int, default=1, help="right-hand sides per batched solve (1..3; NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chain-steps", type=int, default=100,
                     help="--workload c5: consecutive solves timed (BASELINE.json config 5 has 100)")
     return ap.parse_args()
+
+
+def workload_rhs(name, prob):
+    """the config's right-hand side from prob.seed"""
+    from mas_inputs import configs
+    if name in ("c1", "c4"):
+        return configs.rhs_uniform(prob)
+    if name == "c2":
+        return configs.field_manufactured(prob)   # used as a right-hand side here (bench only)
+    return configs.rhs_blob(prob)
 
 
 def workload(name, rank=0):
@@ -67,12 +68,7 @@ def workload(name, rank=0):
     prob.seed += 1000 * rank
     s = prob.stiffness[-1]
     dt = prob.dt_for(s)
-    if name in ("c1", "c4"):
-        b = configs.rhs_uniform(prob)
-    elif name == "c2":
-        b = configs.field_manufactured(prob)      # used as a right-hand side here (bench only)
-    else:
-        b = configs.rhs_blob(prob)
+    b = workload_rhs(name, prob)
     nr, nt, np_ = prob.mesh.shape
     rtol, maxit = (0.0, 500) if name == "c4" else (prob.rtol, prob.maxit)
     desc = (f"{name}: {nr}x{nt}x{np_} fp64, stiffness s={s:g}, rtol={rtol:g}, maxit={maxit}, "
@@ -148,16 +144,17 @@ def hbm_peak():
 
 
 def ncu_traffic(kernel_key):
-    """Per-launch DRAM bytes of the dominant kernel from the committed ncu --set full summary."""
+    """(per-launch DRAM bytes, provenance) of a kernel from the committed ncu --set full summary
+    (profiles/roofline_traffic.csv; each row names the commit and the capture it was taken from)."""
     try:
         import csv
         with open(os.path.join(ROOT, "profiles", "roofline_traffic.csv")) as f:
             for row in csv.DictReader(f):
                 if row["kernel"] == kernel_key:
-                    return int(row["dram_bytes_per_launch"])
+                    return int(row["dram_bytes_per_launch"]), f"{row.get('commit', '?')} {row.get('source', '')}".strip()
     except Exception:
         pass
-    return None
+    return None, None
 
 
 def time_oracle(prob, dt, b, iters):
@@ -324,8 +321,9 @@ def run_sts(args):
     prob = configs.make("c4")
     S = 200
     gpu = MasPcg(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
-    if args.stencil_tile is not None:
-        gpu.set_option("stencil_tile", args.stencil_tile)
+    for kv in args.opt:
+        name, val = kv.split("=")
+        gpu.set_option(name, int(val))
     tau = 0.9 * (S * S + S - 2.0) / 4.0 * 2.0 / gpu.lambda_max()
     u0 = torch.from_numpy(configs.rhs_uniform(prob)).cuda()
     u = u0.clone()
@@ -359,7 +357,8 @@ def run_sts(args):
                                    "tau = 0.9 tau_max", "l2": "inputs larger than L2"},
             "clocks": clocks, "gpu_launches": args.steps * S,
             "roofline": {"bound": "hbm", "kernel": "k_stencil<EPI_STS>", "achieved": gbs, "peak": peak, "unit": "GB/s",
-                         "frac": gbs / peak, "traffic": ncu_traffic("k_stencil_sts"), "peak_source": peak_src}}
+                         "frac": gbs / peak, "traffic": ncu_traffic("k_stencil_sts")[0],
+                         "traffic_source": ncu_traffic("k_stencil_sts")[1], "peak_source": peak_src}}
     if not args.no_cpu_baseline:
         from oracle import ref
         op = ref.RefOperator(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
@@ -452,41 +451,37 @@ def main():
 
     prob, dt, b_np, rtol, maxit, desc = workload(args.workload, rank)
     n = prob.mesh.ncells
+    nrhs = max(1, min(3, args.nrhs))
+    opts = [(kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt]
     gpu = MasPcg(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)
-    if args.variant is not None:
-        gpu.set_option("variant", args.variant)
-    if args.tile is not None:
-        gpu.set_option("tile", args.tile)
-    if args.loop_mode is not None:
-        gpu.set_option("loop_mode", args.loop_mode)
-    if args.xfuse is not None:
-        gpu.set_option("xfuse", args.xfuse)
-    if args.ci is not None:
-        gpu.set_option("ci", args.ci)
-    if args.serpentine is not None:
-        gpu.set_option("serpentine", args.serpentine)
-    if args.qrecompute is not None:
-        gpu.set_option("qrecompute", args.qrecompute)
-    if args.persistent is not None:
-        gpu.set_option("persistent", args.persistent)
-    for kv in args.opt:
-        name, val = kv.split("=")
-        gpu.set_option(name, int(val))
-    if args.k2r_tile is not None:
-        gpu.set_option("k2r_tile", args.k2r_tile)
-    b_host = torch.from_numpy(b_np).pin_memory()
+    for name, val in opts:
+        gpu.set_option(name, val)
+    # right-hand side j of a batched solve = the workload's b from seed + j (independent problems, one operator)
+    b_hosts = [torch.from_numpy(b_np).pin_memory()]
+    for j in range(1, nrhs):
+        pj = prob
+        pj.seed += 1
+        b_hosts.append(torch.from_numpy(np.ascontiguousarray(workload_rhs(args.workload, pj))).pin_memory())
     x_host = torch.zeros(prob.mesh.shape, dtype=torch.float64).pin_memory()
-    b = b_host.cuda()
-    x = torch.zeros_like(b)
+    bs = [bh.cuda() for bh in b_hosts]
+    xs = [torch.zeros_like(bs[0]) for _ in range(nrhs)]
+    b, x, b_host = bs[0], xs[0], b_hosts[0]
     stream = torch.cuda.current_stream()
 
     def step():
-        x.zero_()                                   # x0 = 0 (a 268 MB memset, outside the solver's kernels)
-        return gpu.solve(b, x, rtol, maxit, want_hist=False)
+        """one whole solve from x0 = 0 (the memsets are outside the solver's kernels); returns (status, iterations
+        summed over the right-hand sides)"""
+        for xv in xs:
+            xv.zero_()
+        if nrhs == 1:
+            st_, k_, _ = gpu.solve(b, x, rtol, maxit, want_hist=False)
+            return st_, k_
+        st_, sts_, its_, _ = gpu.solve_multi(bs, xs, rtol, maxit, want_hist=False)
+        return st_, int(sum(its_))
 
     # ---------------- device-resident timing (value) ----------------
     for _ in range(max(args.warmup, 3)):
-        st, k, _ = step()
+        st, k = step()
     barrier()
     sampler = ClockSampler(gpu_selector(torch))
     if rank == 0:
@@ -496,7 +491,7 @@ def main():
     barrier()
     e0.record(stream)
     for _ in range(args.steps):
-        st, k, _ = step()
+        st, k = step()
         iters_done += k
         s = gpu.stats()
         launches += s["loop_launches"] + s["other_launches"]
@@ -519,11 +514,18 @@ def main():
     barrier()
     e2e_s = time.perf_counter() - t0
 
-    # ---------------- per-kernel durations (CUDA events around each launch) ----------------
+    # ---------------- per-kernel durations: CUDA events around each launch (debug library, same source + probes) ----
+    from paper_1811_02605_b200.debug import MasPcgProbe
+    probe = MasPcgProbe(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc, options=[o for o in opts if o[0] != "persistent"])
     x.zero_()
-    prof = gpu.profile(b, x, 40)
+    prof = probe.profile(b, x, 40, int(stream.cuda_stream))
+    pstats = probe.stats()
     # what a trivial linear kernel with the same DRAM read/write mix sustains (context for the rooflines)
-    mix = {"k1_mix_ms": gpu.mix_probe(6, 100), "k2_mix_ms": gpu.mix_probe(3, 100)} if args.workload == "c4" else None
+    mix = None
+    if args.workload == "c4":
+        mix = {"k1_mix_ms": probe.mix_probe(pstats["k1_doubles_per_cell"], 100, int(stream.cuda_stream)),
+               "k2_mix_ms": probe.mix_probe(3, 100, int(stream.cuda_stream))}
+    probe.close()
     barrier()
 
     ms, iters_all, launches_all = reduce_over_ranks(ms, float(iters_done), float(launches), world)
@@ -531,44 +533,50 @@ def main():
 
     if rank == 0:
         value = iters_all / (ms * 1e-3)
-        bpc = stats["bytes_per_cell_iter"]
+        bpc = stats["bytes_per_cell_iter"] if loop_mode != 2 else pstats["bytes_per_cell_iter"]
         peak, peak_src = hbm_peak()
-        stats = gpu.stats()                               # after profile(): per-kernel doubles per cell
-        k1_bytes, k2_bytes = stats["k1_doubles_per_cell"] * 8 * n, stats["k2_doubles_per_cell"] * 8 * n
+        k1_bytes, k2_bytes = pstats["k1_doubles_per_cell"] * 8 * n, pstats["k2_doubles_per_cell"] * 8 * n
         k1_gbs = k1_bytes / (prof["k1_ms"] * 1e-3) / 1e9
         k2_gbs = k2_bytes / (prof["k2_ms"] * 1e-3) / 1e9
-        dom = "k1_fused_matvec" if prof["k1_ms"] >= prof["k2_ms"] else "k2_fused_vector"
-        dom_gbs = k1_gbs if dom.startswith("k1") else k2_gbs
+        k1_name = "k1_tma_noq" if pstats["k1_doubles_per_cell"] == 5 else "k1_tma"
+        k2_name = "k2r_stencil_tma" if pstats["k1_doubles_per_cell"] == 5 else "k2_vec"
+        dom = k1_name if prof["k1_ms"] >= prof["k2_ms"] else k2_name
+        dom_gbs = k1_gbs if dom == k1_name else k2_gbs
+        traffic, traffic_src = ncu_traffic(dom)
         it_ms = ms / (iters_all / world) if iters_all else float("nan")
+        nr_, nt_, np__ = prob.mesh.shape
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "metric": METRIC if args.workload == "c4" else f"fp64_pcg_iterations_per_s_{nr_}x{nt_}x{np__}",
+            "value": value, "unit": UNIT if nrhs == 1 else "rhs-iterations/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": desc, "parallelism": "replicas only" if world > 1 else "1 gpu",
-                       "l2": "inputs larger than L2 (5 live vectors x %.0f MB vs 126 MB)" % (8 * n / 1e6),
+                       "l2": "inputs larger than L2 (%d live vectors x %.0f MB vs 126 MB)" % (4 * nrhs, 8 * n / 1e6),
                        "loop_mode": {0: "host chunks", 1: "cuda-graph while", 2: "persistent cooperative kernel"}[loop_mode],
-                       "bytes_per_cell_iter": bpc, "status": st, "iters_per_step": k},
+                       "bytes_per_cell_iter": bpc, "status": st, "iters_per_step": k, "nrhs": nrhs,
+                       "options": dict(opts)},
             "clocks": clocks,
             "e2e": {"value": e2e_iters_all / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": 2 * 8 * n, "d2h_bytes_per_step": 8 * n},
             "gpu_launches": int(launches_all),
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": dom_gbs, "peak": peak, "unit": "GB/s",
-                         "frac": dom_gbs / peak, "traffic": ncu_traffic(dom), "peak_source": peak_src,
-                         "frac_of_nominal_8000": dom_gbs / 8000.0},
-            "kernels": {"k1_fused_matvec": {"ms": prof["k1_ms"], "min_ms": prof["k1_min_ms"],
-                                            "alg_bytes": k1_bytes, "gbs": k1_gbs},
-                        "k2_fused_vector": {"ms": prof["k2_ms"], "min_ms": prof["k2_min_ms"],
-                                            "alg_bytes": k2_bytes, "gbs": k2_gbs}},
+                         "frac": dom_gbs / peak, "traffic": traffic, "traffic_source": traffic_src,
+                         "peak_source": peak_src, "frac_of_nominal_8000": dom_gbs / 8000.0},
+            "kernels": {k1_name: {"ms": prof["k1_ms"], "min_ms": prof["k1_min_ms"], "alg_bytes": k1_bytes, "gbs": k1_gbs},
+                        k2_name: {"ms": prof["k2_ms"], "min_ms": prof["k2_min_ms"], "alg_bytes": k2_bytes, "gbs": k2_gbs}},
             "mix_ceiling": None if mix is None else {
-                "what": "trivial linear kernels with the same DRAM mix (K1: 3 vectors read + 3 written, K2: 2 read + 1 "
-                        "written in place), best grid size, 100 back-to-back launches",
+                "what": "trivial linear kernels with the same DRAM mix (K1: r, p, x read; p, x (, q) written; K2: 2 read + "
+                        "1 written in place), best grid size, 100 back-to-back launches",
                 "k1_mix_gbs": k1_bytes / (mix["k1_mix_ms"] * 1e-3) / 1e9,
                 "k2_mix_gbs": k2_bytes / (mix["k2_mix_ms"] * 1e-3) / 1e9,
                 "k1_frac_of_mix": mix["k1_mix_ms"] / prof["k1_ms"], "k2_frac_of_mix": mix["k2_mix_ms"] / prof["k2_ms"]},
             "iteration": {"ms": it_ms, "model_gbs": bpc * n / (it_ms * 1e-3) / 1e9,
                           "frac_of_peak": bpc * n / (it_ms * 1e-3) / 1e9 / peak,
-                          "frac_of_nominal_8000": bpc * n / (it_ms * 1e-3) / 1e9 / 8000.0},
+                          "frac_of_nominal_8000": bpc * n / (it_ms * 1e-3) / 1e9 / 8000.0,
+                          "kernel_sum_ms": prof["k1_ms"] + prof["k2_ms"]},
         }
+        if nrhs > 1:
+            line["iteration"]["note"] = "per right-hand-side iteration"
         if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
             from oracle import ref                      # config 3 = the oracle's FULL solve
             op = ref.RefOperator(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)

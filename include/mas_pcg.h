@@ -19,6 +19,10 @@
  * All vectors are fp64, C-contiguous [nr][nt][np] with phi fastest, 16-byte aligned.
  * Every entry point returns an int status (below); no exceptions, no aborts, no output.
  * There is no CPU fallback: without a CUDA device every call that needs one returns MAS_ECUDA.
+ * A handle remembers the device it was created on; every call switches to that device for its own
+ * duration, whatever the caller's current device is.
+ *
+ * Measurement probes used by bench.py are NOT here: see mas_pcg_debug.h (a separate library).
  */
 #ifndef MAS_PCG_H
 #define MAS_PCG_H
@@ -55,10 +59,14 @@ enum {
     MAS_MAXIT = 1,       /* ran maxit iterations without meeting rtol; x is the last iterate.  The
                             normal return of fixed-iteration runs (rtol = 0)                            */
     MAS_EINVAL = -1,     /* bad dimension / null pointer / non-positive width / dt < 0 / nu <= 0 /
-                            rtol < 0 / maxit < 0 / misaligned vector                                    */
+                            rtol < 0 / maxit < 0 / misaligned or aliased vector                         */
     MAS_ENOMEM = -2,     /* host or device allocation failed                                            */
-    MAS_ECUDA = -3,      /* a CUDA runtime call failed (no device, launch error, ...)                   */
-    MAS_EBREAKDOWN = -4  /* p.Ap <= 0 or a non-finite scalar: the operator is not SPD for these inputs  */
+    MAS_ECUDA = -3,      /* a CUDA runtime call failed (no device, launch error, ...), or a kernel
+                            reported a protocol fault (an mbarrier wait that timed out)                 */
+    MAS_EBREAKDOWN = -4  /* p.Ap <= 0, or a non-finite scalar (||V.b||^2, ||r||^2, r.z, p.Ap): the
+                            operator is not SPD for these inputs, or b / x0 hold NaN / Inf.  x is the
+                            last iterate (x0 if no iteration completed); iters_out and the history
+                            are valid                                                                   */
 };
 
 /* Build the operator for (grid, metric, dt, nu, boundary kinds) and allocate all workspaces
@@ -89,40 +97,43 @@ int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, double rtol,
 int mas_pcg_solve_host(mas_pcg_t *h, const double *b_host, double *x_host, double rtol, int maxit,
                        void *stream, int *iters_out, double *reshist_host);
 
+/* Batched solve: nrhs <= 3 right-hand sides that share the operator -- PAPER.md:50 eq. (1):
+ * the implicit terms act on the vector v, whose three components share one coefficient set.  By definition these
+ * are nrhs INDEPENDENT textbook solves (own alpha, beta, iteration count, status and history each; bit-identical to
+ * nrhs calls of mas_pcg_solve), run by ONE set of kernel launches per iteration: the right-hand side is the second
+ * grid dimension, a right-hand side that has converged drops out, the loop ends when all have.
+ *   b_dev, x_dev  : HOST arrays of nrhs DEVICE pointers (N doubles each; all distinct).
+ *   iters_out     : HOST, nrhs ints (may be NULL);  status_out: HOST, nrhs ints (MAS_OK / MAS_MAXIT /
+ *                   MAS_EBREAKDOWN per right-hand side; may be NULL).
+ *   reshist_host  : HOST, NULL or nrhs * (maxit + 1) doubles; right-hand side j's history starts at
+ *                   reshist_host + j * (maxit + 1).
+ * Returns the most severe per-right-hand-side status (negative before MAS_MAXIT before MAS_OK), or an error. */
+int mas_pcg_solve_multi(mas_pcg_t *h, int nrhs, const double *const *b_dev, double *const *x_dev, double rtol,
+                        int maxit, void *stream, int *iters_out, int *status_out, double *reshist_host);
+
 /* y = A_sym x (the matrix-free stencil alone; asynchronous on `stream`).  x_dev != y_dev. */
 int mas_pcg_apply(mas_pcg_t *h, const double *x_dev, double *y_dev, void *stream);
-
-/* Measurement aid (bench.py roofline): runs `nit` PCG iterations (rtol = 0) from x0 = x_dev with the
- * kernels launched one by one and CUDA events recorded around each on `stream`; synchronises.
- * ms_out (HOST, 4 doubles) = { mean K1, mean K2, min K1, min K2 } kernel durations in milliseconds
- * (K1 = fused matvec, K2 = fused vector kernel).  1 <= nit <= 256.  x_dev is overwritten. */
-int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev, int nit, void *stream, double *ms_out);
-
-/* Measurement aid (bench.py): *ms_out (HOST) = best sustained time per launch, over `reps` back-to-back
- * launches, of a trivial LINEAR kernel with the DRAM read/write mix of K1 (which = 6: three N-vectors read,
- * three written, one of them in place) or K2 (which = 3: two read, one written in place) and none of their
- * structure: what the memory system sustains for that mix.  Clobbers the handle's workspaces. */
-int mas_pcg_mix_probe(mas_pcg_t *h, int which, int reps, void *stream, double *ms_out);
 
 /* Fills HOST array out[8] with counters of the last solve:
  *   [0] kernels launched inside the iteration loop, [1] kernels launched outside it,
  *   [2] loop mode used (1 = CUDA-graph WHILE node, 0 = host-driven chunks, 2 = one persistent cooperative kernel),
  *   [3] algorithmic bytes per cell per iteration of the kernels in use,
  *   [4] doubles per cell K1 moves, [5] doubles per cell K2 moves,
- *   [6] grid size of the persistent kernel (0 if not used), [7] 1 if the loop body used programmatic (PDL) edges. */
+ *   [6] grid size of the persistent kernel (0 if not used; slab groups: the number of slabs),
+ *   [7] 1 if a cooperative launch was refused and the handle fell back to the streaming loop. */
 int mas_pcg_stats(const mas_pcg_t *h, long long *out);
 
-/* Tuning / debugging knob, takes effect at the next solve.  name in
- *   "loop_mode" (0 host chunks, 1 graph while), "variant" (K1: 0 baseline, 1 marching, 2 wide marching with cp.async,
- *   3 wide marching with TMA bulk copies + mbarriers = default),
- *   "tile" (tile configuration of the variant), "ci" (r-chunk length, 0 = automatic),
- *   "xfuse" (variant 2 only; 1: x-update fused into K1, 72 B/cell/iteration; 0: in K2, 80 B; variant 3 is always
- *   fused), "serpentine" (K2 sweeps
- *   backward), "apply_variant" (1 marching stencil kernel, 0 baseline), "stencil_tile" (0..5 cp.async, 6..11 TMA),
- *   "qrecompute" (variant 2 only: 64 B), "k2r_tile",
- *   "unroll" (PCG iterations per WHILE trip of the graph loop, 1..16), "pdl" (programmatic dependent launch
- *   edges inside the loop body; default 0: measured slower),
- *   "persistent" (small meshes: whole solve in one cooperative kernel; 0 off, 1 whenever it fits, 2 auto).
+/* Tuning knob, takes effect at the next solve.  name in
+ *   "loop_mode"   0 host-driven chunks of 16 iterations, 1 CUDA-graph WHILE loop (default);
+ *   "persistent"  1 (default): meshes whose per-cell state fits in the SMs' shared memory are solved by ONE
+ *                 cooperative kernel, whatever loop_mode says; 0: always the streaming loop;
+ *   "qrecompute"  1 (default): 64 B/cell/iteration -- K1 does not store q, K2 recomputes it; 0: 72 B, q stored;
+ *   "tile"        K1 tile configuration (0..6), "k2r_tile" / "stencil_tile" (0..5) the stencil kernel's tile for
+ *                 K2R / for apply and RKL2 stages, "ci" r-chunk length of the marching kernels (0 = automatic, else 2..32);
+ *   "serpentine"  1 (default): K2 sweeps the mesh backward (L2 reuse across K1 -> K2 -> K1);
+ *   "unroll"      PCG iterations per WHILE trip of the graph loop (1..16, default 4);
+ *   "l2_keep_r", "l2_keep_p"  number of leading r-planes of r / p whose accesses carry the L2 evict_last priority
+ *                 (0 = no hints), "l2_first_x" 1: x is streamed with evict_first.
  * Unknown name or value: MAS_EINVAL. */
 int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value);
 
@@ -149,6 +160,31 @@ int mas_sts_advance(mas_pcg_t *h, double *u_dev, double tau, int s, void *stream
 void mas_pcg_destroy(mas_pcg_t *h);            /* NULL is allowed                                 */
 
 const char *mas_pcg_strerror(int status);      /* static string, never NULL                       */
+
+/* ---- NEXT-3: r-slab decomposition (Sec. 4.3: domain split, one rank per GPU; PAPER.md:177, 183:
+ * the scaling loss past one node came from host-staged halo exchange).  The mesh is split along r into nslab slabs,
+ * slab s owning the planes [i_split[s], i_split[s+1]); each slab has its own vectors, as one rank per GPU would.
+ * The kernels read the neighbour slab's boundary plane of r, p and x0 straight through a pointer (a peer mapping
+ * over NVLink on a real node): per matvec one plane of nt*np doubles per neighbour, no halo kernel or staging
+ * buffer; the two scalar reductions per iteration add the slabs' partial sums in slab order.  The undivided solve
+ * is the definition: iterates agree with mas_pcg_solve up to the rounding order of the sums.
+ * This library drives all slabs from ONE process on ONE device; that is the form that can be tested with one GPU,
+ * and it is unmeasured on multi-GPU hardware. ---- */
+typedef struct mas_pcg_slabs mas_pcg_slabs_t;
+
+/* grid, metric, nu, bc describe the WHOLE mesh.  i_split: HOST, nslab + 1 increasing plane indices, i_split[0] = 0,
+ * i_split[nslab] = nr; 1 <= nslab <= 16. */
+int mas_pcg_slabs_create(const mas_grid_t *grid, const mas_metric_t *metric, double dt, const mas_nu_t *nu,
+                         const mas_bc_t *bc, int nslab, const int *i_split, mas_pcg_slabs_t **out);
+int mas_pcg_slabs_set_dt(mas_pcg_slabs_t *g, double dt, void *stream);
+/* same names as mas_pcg_set_option (except "persistent") */
+int mas_pcg_slabs_set_option(mas_pcg_slabs_t *g, const char *name, int value);
+/* b_dev, x_dev: HOST arrays of nslab DEVICE pointers; slab s's vectors hold its own planes only,
+ * (i_split[s+1] - i_split[s]) * nt * np doubles.  Other arguments as mas_pcg_solve. */
+int mas_pcg_slabs_solve(mas_pcg_slabs_t *g, const double *const *b_dev, double *const *x_dev, double rtol, int maxit,
+                        void *stream, int *iters_out, double *reshist_host);
+int mas_pcg_slabs_stats(const mas_pcg_slabs_t *g, long long *out);
+void mas_pcg_slabs_destroy(mas_pcg_slabs_t *g);
 
 #ifdef __cplusplus
 }

@@ -5,4 +5,4 @@ torch CUDA tensors (device memory + streams only).  No CPU fallback exists.
 """
 from .binding import (MAS_OK, MAS_MAXIT, MAS_EINVAL, MAS_ENOMEM, MAS_ECUDA, MAS_EBREAKDOWN,  # noqa: F401
                       MAS_BC_DIRICHLET, MAS_BC_NEUMANN, MasError)
-from .solver import MasPcg  # noqa: F401
+from .solver import MasPcg, MasPcgSlabs  # noqa: F401

@@ -16,8 +16,11 @@ from . import build as _build
 
 MAS_OK, MAS_MAXIT, MAS_EINVAL, MAS_ENOMEM, MAS_ECUDA, MAS_EBREAKDOWN = 0, 1, -1, -2, -3, -4
 MAS_BC_DIRICHLET, MAS_BC_NEUMANN = 0, 1
+MAX_RHS = 3
 
 _dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int)
+_vpp = ctypes.POINTER(ctypes.c_void_p)
 
 
 class mas_grid_t(ctypes.Structure):
@@ -37,6 +40,40 @@ class mas_nu_t(ctypes.Structure):
     _fields_ = [("kind", ctypes.c_int), ("v", _dp)]
 
 
+def _prototypes(L):
+    """argtypes / restype of every include/mas_pcg.h entry point on a loaded library."""
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    create_args = [ctypes.POINTER(mas_grid_t), ctypes.POINTER(mas_metric_t), cd, ctypes.POINTER(mas_nu_t),
+                   ctypes.POINTER(mas_bc_t)]
+    sig = {
+        "mas_pcg_create": (ci, create_args + [_vpp]),
+        "mas_pcg_set_dt": (ci, [vp, cd, vp]),
+        "mas_pcg_solve": (ci, [vp, vp, vp, cd, ci, vp, _ip, _dp]),
+        "mas_pcg_solve_host": (ci, [vp, vp, vp, cd, ci, vp, _ip, _dp]),
+        "mas_pcg_solve_multi": (ci, [vp, ci, _vpp, _vpp, cd, ci, vp, _ip, _ip, _dp]),
+        "mas_pcg_apply": (ci, [vp, vp, vp, vp]),
+        "mas_pcg_lop": (ci, [vp, vp, vp, vp]),
+        "mas_pcg_lambda_max": (ci, [vp, _dp]),
+        "mas_sts_stages": (ci, [vp, cd, _ip]),
+        "mas_sts_advance": (ci, [vp, vp, cd, ci, vp]),
+        "mas_pcg_stats": (ci, [vp, ctypes.POINTER(ctypes.c_longlong)]),
+        "mas_pcg_set_option": (ci, [vp, ctypes.c_char_p, ci]),
+        "mas_pcg_destroy": (None, [vp]),
+        "mas_pcg_strerror": (ctypes.c_char_p, [ci]),
+        "mas_pcg_slabs_create": (ci, create_args + [ci, _ip, _vpp]),
+        "mas_pcg_slabs_set_dt": (ci, [vp, cd, vp]),
+        "mas_pcg_slabs_set_option": (ci, [vp, ctypes.c_char_p, ci]),
+        "mas_pcg_slabs_solve": (ci, [vp, _vpp, _vpp, cd, ci, vp, _ip, _dp]),
+        "mas_pcg_slabs_stats": (ci, [vp, ctypes.POINTER(ctypes.c_longlong)]),
+        "mas_pcg_slabs_destroy": (None, [vp]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(L, name)
+        f.restype = res
+        f.argtypes = args
+    return L
+
+
 def _load():
     path = _build.LIB
     if not _build.up_to_date():
@@ -45,40 +82,7 @@ def _load():
         except Exception as e:  # no nvcc on this machine: use the shipped .so if there is one
             if not os.path.exists(path):
                 raise ImportError(f"libmas_pcg.so is missing and could not be built: {e}") from e
-    L = ctypes.CDLL(path)
-    vp = ctypes.c_void_p
-    L.mas_pcg_create.restype = ctypes.c_int
-    L.mas_pcg_create.argtypes = [ctypes.POINTER(mas_grid_t), ctypes.POINTER(mas_metric_t), ctypes.c_double,
-                                 ctypes.POINTER(mas_nu_t), ctypes.POINTER(mas_bc_t), ctypes.POINTER(vp)]
-    L.mas_pcg_set_dt.restype = ctypes.c_int
-    L.mas_pcg_set_dt.argtypes = [vp, ctypes.c_double, vp]
-    for name in ("mas_pcg_solve", "mas_pcg_solve_host"):
-        f = getattr(L, name)
-        f.restype = ctypes.c_int
-        f.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_int, vp, ctypes.POINTER(ctypes.c_int), _dp]
-    L.mas_pcg_apply.restype = ctypes.c_int
-    L.mas_pcg_apply.argtypes = [vp, vp, vp, vp]
-    L.mas_pcg_profile.restype = ctypes.c_int
-    L.mas_pcg_profile.argtypes = [vp, vp, vp, ctypes.c_int, vp, _dp]
-    L.mas_pcg_lop.restype = ctypes.c_int
-    L.mas_pcg_lop.argtypes = [vp, vp, vp, vp]
-    L.mas_pcg_lambda_max.restype = ctypes.c_int
-    L.mas_pcg_lambda_max.argtypes = [vp, _dp]
-    L.mas_sts_stages.restype = ctypes.c_int
-    L.mas_sts_stages.argtypes = [vp, ctypes.c_double, ctypes.POINTER(ctypes.c_int)]
-    L.mas_sts_advance.restype = ctypes.c_int
-    L.mas_sts_advance.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp]
-    L.mas_pcg_mix_probe.restype = ctypes.c_int
-    L.mas_pcg_mix_probe.argtypes = [vp, ctypes.c_int, ctypes.c_int, vp, _dp]
-    L.mas_pcg_stats.restype = ctypes.c_int
-    L.mas_pcg_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_longlong)]
-    L.mas_pcg_set_option.restype = ctypes.c_int
-    L.mas_pcg_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_int]
-    L.mas_pcg_destroy.restype = None
-    L.mas_pcg_destroy.argtypes = [vp]
-    L.mas_pcg_strerror.restype = ctypes.c_char_p
-    L.mas_pcg_strerror.argtypes = [ctypes.c_int]
-    return L
+    return _prototypes(ctypes.CDLL(path))
 
 
 _lib = None
@@ -105,25 +109,30 @@ def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
 
 
-def mas_pcg_create(grid, metric_arrays, dt, nu_kind, nu, bc=(0, 0)) -> int:
-    """grid = (nr, nt, np); metric_arrays = the ten HOST arrays of mas_metric_t in declaration order.
-    Returns the opaque handle (an int); raises MasError on a negative status."""
+def _create_args(grid, metric_arrays, dt, nu_kind, nu, bc):
     arrs = [_f64(a) for a in metric_arrays]
     nu_h = _f64(nu)
     g = mas_grid_t(*[int(v) for v in grid])
     m = mas_metric_t(*[a.ctypes.data_as(_dp) for a in arrs])
     n = mas_nu_t(int(nu_kind), nu_h.ctypes.data_as(_dp))
     b = mas_bc_t(int(bc[0]), int(bc[1]))
+    keep = (arrs, nu_h, g, m, n, b)              # alive until the call returns
+    return keep, (ctypes.byref(g), ctypes.byref(m), float(dt), ctypes.byref(n), ctypes.byref(b))
+
+
+def mas_pcg_create(grid, metric_arrays, dt, nu_kind, nu, bc=(0, 0), L=None) -> int:
+    """grid = (nr, nt, np); metric_arrays = the ten HOST arrays of mas_metric_t in declaration order.
+    Returns the opaque handle (an int); raises MasError on a negative status."""
+    keep, args = _create_args(grid, metric_arrays, dt, nu_kind, nu, bc)
     out = ctypes.c_void_p()
-    st = lib().mas_pcg_create(ctypes.byref(g), ctypes.byref(m), float(dt), ctypes.byref(n), ctypes.byref(b),
-                              ctypes.byref(out))
+    st = (L or lib()).mas_pcg_create(*args, ctypes.byref(out))
     if st != MAS_OK:
         raise MasError(st, "mas_pcg_create")
     return out.value
 
 
-def mas_pcg_destroy(handle):
-    lib().mas_pcg_destroy(handle)
+def mas_pcg_destroy(handle, L=None):
+    (L or lib()).mas_pcg_destroy(handle)
 
 
 def mas_pcg_set_dt(handle, dt, stream=0):
@@ -132,8 +141,8 @@ def mas_pcg_set_dt(handle, dt, stream=0):
         raise MasError(st, "mas_pcg_set_dt")
 
 
-def mas_pcg_set_option(handle, name: str, value: int):
-    st = lib().mas_pcg_set_option(handle, name.encode(), int(value))
+def mas_pcg_set_option(handle, name: str, value: int, L=None):
+    st = (L or lib()).mas_pcg_set_option(handle, name.encode(), int(value))
     if st != MAS_OK:
         raise MasError(st, f"mas_pcg_set_option({name}={value})")
 
@@ -144,17 +153,20 @@ def mas_pcg_apply(handle, x_ptr, y_ptr, stream=0):
         raise MasError(st, "mas_pcg_apply")
 
 
+def _raise(st, where, iters=None, hist=None):
+    err = MasError(st, where)
+    if st == MAS_EBREAKDOWN:                     # x holds the last iterate; the count and history are meaningful
+        err.iters, err.hist = iters, hist
+    raise err
+
+
 def _solve(fn, where, handle, b_ptr, x_ptr, rtol, maxit, stream, want_hist):
     it = ctypes.c_int(0)
     hist = np.empty(maxit + 1) if want_hist else None
     st = fn(handle, b_ptr, x_ptr, float(rtol), int(maxit), stream, ctypes.byref(it),
             hist.ctypes.data_as(_dp) if want_hist else None)
     if st < 0:
-        err = MasError(st, where)
-        if st == MAS_EBREAKDOWN:                 # x holds the last iterate; the count and history are meaningful
-            err.iters = it.value
-            err.hist = hist[: it.value + 1].copy() if want_hist else None
-        raise err
+        _raise(st, where, it.value, hist[: it.value + 1].copy() if want_hist else None)
     return st, it.value, (hist[: it.value + 1].copy() if want_hist else None)
 
 
@@ -169,13 +181,23 @@ def mas_pcg_solve_host(handle, b_ptr, x_ptr, rtol, maxit, stream=0, want_hist=Tr
                   want_hist)
 
 
-def mas_pcg_profile(handle, b_ptr, x_ptr, nit, stream=0):
-    """Per-kernel CUDA-event timing of nit iterations: {k1_ms, k2_ms, k1_min_ms, k2_min_ms}."""
-    out = np.zeros(4)
-    st = lib().mas_pcg_profile(handle, b_ptr, x_ptr, int(nit), stream, out.ctypes.data_as(_dp))
-    if st != MAS_OK:
-        raise MasError(st, "mas_pcg_profile")
-    return {"k1_ms": out[0], "k2_ms": out[1], "k1_min_ms": out[2], "k2_min_ms": out[3]}
+def _ptr_array(ptrs):
+    return (ctypes.c_void_p * len(ptrs))(*[int(p) for p in ptrs])
+
+
+def mas_pcg_solve_multi(handle, b_ptrs, x_ptrs, rtol, maxit, stream=0, want_hist=True):
+    """nrhs = len(b_ptrs) <= 3 DEVICE pointers each.  Returns (worst status, [status_j], [iters_j], [hist_j]);
+    raises MasError only on argument / runtime errors (a per-right-hand-side breakdown is reported in status_j)."""
+    nrhs = len(b_ptrs)
+    it = (ctypes.c_int * nrhs)()
+    sj = (ctypes.c_int * nrhs)()
+    hist = np.empty((nrhs, maxit + 1)) if want_hist else None
+    st = lib().mas_pcg_solve_multi(handle, nrhs, _ptr_array(b_ptrs), _ptr_array(x_ptrs), float(rtol), int(maxit),
+                                   stream, it, sj, hist.ctypes.data_as(_dp) if want_hist else None)
+    if st < 0 and st != MAS_EBREAKDOWN:
+        raise MasError(st, "mas_pcg_solve_multi")
+    hists = [hist[j, : it[j] + 1].copy() for j in range(nrhs)] if want_hist else None
+    return st, list(sj), list(it), hists
 
 
 def mas_pcg_lop(handle, u_ptr, y_ptr, stream=0):
@@ -206,19 +228,60 @@ def mas_sts_advance(handle, u_ptr, tau, s, stream=0):
         raise MasError(st, "mas_sts_advance")
 
 
-def mas_pcg_mix_probe(handle, which, reps, stream=0) -> float:
-    """ms per launch of a trivial linear kernel with K1's (which=6) or K2's (which=3) DRAM read/write mix."""
-    out = ctypes.c_double(0.0)
-    st = lib().mas_pcg_mix_probe(handle, int(which), int(reps), stream, ctypes.byref(out))
+def _stats_dict(out):
+    return {"loop_launches": out[0], "other_launches": out[1], "loop_mode": out[2], "bytes_per_cell_iter": out[3],
+            "k1_doubles_per_cell": out[4], "k2_doubles_per_cell": out[5], "persistent_grid_or_slabs": out[6],
+            "coop_refused": out[7]}
+
+
+def mas_pcg_stats(handle, L=None):
+    out = (ctypes.c_longlong * 8)()
+    st = (L or lib()).mas_pcg_stats(handle, out)
     if st != MAS_OK:
-        raise MasError(st, "mas_pcg_mix_probe")
+        raise MasError(st, "mas_pcg_stats")
+    return _stats_dict(out)
+
+
+# ---- NEXT-3: r-slab groups ----
+def mas_pcg_slabs_create(grid, metric_arrays, dt, nu_kind, nu, bc, i_split) -> int:
+    keep, args = _create_args(grid, metric_arrays, dt, nu_kind, nu, bc)
+    split = (ctypes.c_int * len(i_split))(*[int(v) for v in i_split])
+    out = ctypes.c_void_p()
+    st = lib().mas_pcg_slabs_create(*args, len(i_split) - 1, split, ctypes.byref(out))
+    if st != MAS_OK:
+        raise MasError(st, "mas_pcg_slabs_create")
     return out.value
 
 
-def mas_pcg_stats(handle):
-    out = (ctypes.c_longlong * 8)()
-    st = lib().mas_pcg_stats(handle, out)
+def mas_pcg_slabs_destroy(handle):
+    lib().mas_pcg_slabs_destroy(handle)
+
+
+def mas_pcg_slabs_set_dt(handle, dt, stream=0):
+    st = lib().mas_pcg_slabs_set_dt(handle, float(dt), stream)
     if st != MAS_OK:
-        raise MasError(st, "mas_pcg_stats")
-    return {"loop_launches": out[0], "other_launches": out[1], "loop_mode": out[2], "bytes_per_cell_iter": out[3],
-            "k1_doubles_per_cell": out[4], "k2_doubles_per_cell": out[5]}
+        raise MasError(st, "mas_pcg_slabs_set_dt")
+
+
+def mas_pcg_slabs_set_option(handle, name: str, value: int):
+    st = lib().mas_pcg_slabs_set_option(handle, name.encode(), int(value))
+    if st != MAS_OK:
+        raise MasError(st, f"mas_pcg_slabs_set_option({name}={value})")
+
+
+def mas_pcg_slabs_solve(handle, b_ptrs, x_ptrs, rtol, maxit, stream=0, want_hist=True):
+    it = ctypes.c_int(0)
+    hist = np.empty(maxit + 1) if want_hist else None
+    st = lib().mas_pcg_slabs_solve(handle, _ptr_array(b_ptrs), _ptr_array(x_ptrs), float(rtol), int(maxit), stream,
+                                   ctypes.byref(it), hist.ctypes.data_as(_dp) if want_hist else None)
+    if st < 0:
+        _raise(st, "mas_pcg_slabs_solve", it.value, hist[: it.value + 1].copy() if want_hist else None)
+    return st, it.value, (hist[: it.value + 1].copy() if want_hist else None)
+
+
+def mas_pcg_slabs_stats(handle):
+    out = (ctypes.c_longlong * 8)()
+    st = lib().mas_pcg_slabs_stats(handle, out)
+    if st != MAS_OK:
+        raise MasError(st, "mas_pcg_slabs_stats")
+    return _stats_dict(out)

@@ -1,4 +1,8 @@
-"""Builds csrc/mas_pcg.cu into lib/libmas_pcg.so for sm_100a (in-tree, so the .so travels with gpurun).
+"""Builds csrc/mas_pcg.cu for sm_100a, in-tree (so the .so files travel with gpurun):
+
+    lib/libmas_pcg.so      the product library (include/mas_pcg.h)
+    lib/libmas_pcg_dbg.so  the same source with -DMAS_PCG_DEBUG_PROBES: adds the measurement probes of
+                           include/mas_pcg_debug.h (per-kernel CUDA-event timing, traffic-mix probe) for bench.py
 
     python -m paper_1811_02605_b200.build [--force]
 """
@@ -13,6 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "lib", "libmas_pcg.so")
+LIB_DBG = os.path.join(_HERE, "lib", "libmas_pcg_dbg.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
@@ -20,14 +25,17 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
 
 def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))
-                  + glob.glob(os.path.join(INCLUDE, "*.h")))
+                  + glob.glob(os.path.join(CSRC, "*.inc")) + glob.glob(os.path.join(INCLUDE, "*.h")))
 
 
 def up_to_date() -> bool:
-    if not os.path.exists(LIB):
-        return False
-    t = os.path.getmtime(LIB)
-    return all(os.path.getmtime(s) <= t for s in sources())
+    for lib in (LIB, LIB_DBG):
+        if not os.path.exists(lib):
+            return False
+        t = os.path.getmtime(lib)
+        if not all(os.path.getmtime(s) <= t for s in sources()):
+            return False
+    return True
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -35,16 +43,22 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(os.path.dirname(LIB), exist_ok=True)
-    tmp = f"{LIB}.{os.getpid()}.tmp"
-    cmd = [nvcc, *NVCC_FLAGS, "-o", tmp, os.path.join(CSRC, "mas_pcg.cu")]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
-    os.replace(tmp, LIB)
+    jobs = []
+    for lib, extra in ((LIB, []), (LIB_DBG, ["-DMAS_PCG_DEBUG_PROBES"])):
+        tmp = f"{lib}.{os.getpid()}.tmp"
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", tmp, os.path.join(CSRC, "mas_pcg.cu")]
+        jobs.append((lib, tmp, cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
+    logs = []
+    for lib, tmp, cmd, proc in jobs:
+        out, err = proc.communicate()
+        if proc.returncode != 0:
+            raise RuntimeError("nvcc failed:\n" + out + err)
+        os.replace(tmp, lib)
+        logs.append(" ".join(cmd) + "\n" + err)
     with open(os.path.join(os.path.dirname(LIB), "ptxas.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + res.stderr)
+        f.write(logs[0])
     if verbose:
-        print(res.stderr)
+        print(logs[0])
     return LIB
 
 

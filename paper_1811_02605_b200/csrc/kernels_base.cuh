@@ -1,7 +1,7 @@
-// kernels_base.cuh -- set_dt plane scaling, plain matvec (mas_pcg_apply / init), init, the fused
-// vector kernel K2, and the straightforward fused matvec K1 "variant 0" (neighbours through
-// L1/L2, p_new recomputed per neighbour).  Variant 0 is the in-library correctness baseline for
-// the tiled kernels in kernels_march.cuh.
+// kernels_base.cuh -- set_dt plane scaling, init (S1), the fused vector kernel K2 (S4), the x tail, the scalar
+// steps S3 / S5 run by the last-arriving block of the reducing kernels, and the slab combine step.
+// Every kernel takes the right-hand side index from blockIdx.y (batched solves: the three
+// components of v share one coefficient set); a single solve is gridDim.y = 1.
 #pragma once
 #include "common.cuh"
 
@@ -34,61 +34,6 @@ __global__ void k_scale_planes(PlaneSet ps, double dt)
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// the 7-point stencil on one double2 (cells k = 2kv, k+1 of row (i,j)), coefficient form:
-//   (A u)_c = d_c u_c - vp[k] (ARm u_im + ARp u_ip + ATm u_jm + ATp u_jp) - F (ip[k] u_kp + ip[k-1] u_km)
-// ---------------------------------------------------------------------------------------------
-struct RowCoef {
-    double E, F, ARm, ARp, ATm, ATp;
-};
-
-__device__ __forceinline__ RowCoef load_coef(const OpDev &op, int i, int j)
-{
-    RowCoef c;
-    const int row = i * op.nt + j;
-    c.E = __ldg(op.E + row);
-    c.F = __ldg(op.F + row);
-    c.ARm = __ldg(op.AR + row);
-    c.ARp = __ldg(op.AR + row + op.nt);
-    c.ATm = __ldg(op.AT + i * (op.nt + 1) + j);
-    c.ATp = __ldg(op.AT + i * (op.nt + 1) + j + 1);
-    return c;
-}
-
-struct PhiCoef {            // phi factors of the two cells of a vector and their outer faces
-    double vp0, vp1, wp0, wp1, ipm, ip0, ip1;   // ipm = ip[k-1], ip0 = ip[k], ip1 = ip[k+1]
-    int km, kp;                                 // wrapped neighbour cells k-1 and k+2
-};
-
-__device__ __forceinline__ PhiCoef load_phi(const OpDev &op, int kv)
-{
-    PhiCoef c;
-    const int k = 2 * kv;
-    c.km = k == 0 ? op.np - 1 : k - 1;
-    c.kp = k + 2 >= op.np ? 0 : k + 2;
-    c.vp0 = __ldg(op.vp + k);
-    c.vp1 = __ldg(op.vp + k + 1);
-    c.wp0 = __ldg(op.wp + k);
-    c.wp1 = __ldg(op.wp + k + 1);
-    c.ipm = __ldg(op.ip + c.km);
-    c.ip0 = __ldg(op.ip + k);
-    c.ip1 = __ldg(op.ip + k + 1);
-    return c;
-}
-
-__device__ __forceinline__ double2 stencil(const RowCoef &c, const PhiCoef &f, double2 u, double2 uim,
-                                           double2 uip, double2 ujm, double2 ujp, double ukm, double ukp)
-{
-    const double d0 = fma(f.vp0, c.E, c.F * f.wp0);
-    const double d1 = fma(f.vp1, c.E, c.F * f.wp1);
-    const double sx = c.ARm * uim.x + c.ARp * uip.x + c.ATm * ujm.x + c.ATp * ujp.x;
-    const double sy = c.ARm * uim.y + c.ARp * uip.y + c.ATm * ujm.y + c.ATp * ujp.y;
-    double2 q;
-    q.x = d0 * u.x - f.vp0 * sx - c.F * (f.ip0 * u.y + f.ipm * ukm);
-    q.y = d1 * u.y - f.vp1 * sy - c.F * (f.ip1 * ukp + f.ip0 * u.x);
-    return q;
-}
-
 __device__ __forceinline__ double2 ld2(const double *p, size_t cell)
 {
     return *reinterpret_cast<const double2 *>(p + cell);
@@ -99,113 +44,86 @@ __device__ __forceinline__ void st2(double *p, size_t cell, double2 v)
 }
 
 // ---------------------------------------------------------------------------------------------
-// y = A_sym u   (mas_pcg_apply; also A x0 for the initial residual).  u = xin, or args->x if null.
-// ---------------------------------------------------------------------------------------------
-template <int NT>
-__global__ void __launch_bounds__(NT) k_apply(OpDev op, const double *xin, const SolveArgs *args, double *y)
-{
-    const double *u = xin ? xin : args->x;
-    const RowMap m = row_map<NT>(op.nv);
-    if (m.idle) return;
-    const double2 zero = make_double2(0.0, 0.0);
-    for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
-        const int row = rowbase + m.rl;
-        if (row >= op.nrows) break;
-        const int i = row / op.nt, j = row - i * op.nt;
-        const RowCoef c = load_coef(op, i, j);
-        const size_t base = (size_t)row * op.np;
-        const size_t sr = (size_t)op.nt * op.np;
-        for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
-            const PhiCoef f = load_phi(op, kv);
-            const size_t cell = base + 2 * kv;
-            const double2 uc = ld2(u, cell);
-            const double2 uim = i > 0 ? ld2(u, cell - sr) : zero;
-            const double2 uip = i < op.nr - 1 ? ld2(u, cell + sr) : zero;
-            const double2 ujm = j > 0 ? ld2(u, cell - op.np) : zero;
-            const double2 ujp = j < op.nt - 1 ? ld2(u, cell + op.np) : zero;
-            const double ukm = u[base + f.km], ukp = u[base + f.kp];
-            st2(y, cell, stencil(c, f, uc, uim, uip, ujm, ujp, ukm, ukp));
-        }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// init (S1): r = V.b - q (q = A x0), p_in = 0, bb = |V.b|^2, rr = |r|^2, rho = r.(r/d); then the
-// last block sets hist[0], k = 0, beta = 0 and the loop condition.
+// loop control: the graph's WHILE condition (and the flag the host-chunk loop polls) = "some right-hand
+// side is still active".  Every right-hand side reports once per voting kernel (init, K2): through its
+// last-arriving block when it did work, through block 0 when it was already inactive.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ void set_cond(cudaGraphConditionalHandle cond, int use_cond, int v)
 {
     if (use_cond) cudaGraphSetConditional(cond, v ? 1u : 0u);
 }
 
-template <int NT, bool UNIFORM>
-__global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond)
+__device__ __forceinline__ void loop_vote(const Work &w, int active, int nvoters, cudaGraphConditionalHandle cond,
+                                          int use_cond)
 {
-    __shared__ double sh[32];
-    const double *b = w.args->b;
-    const RowMap m = row_map<NT>(op.nv);
-    double acc[3] = {0.0, 0.0, 0.0};   // bb, rr, rho
-    if (!m.idle)
-        for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
-            const int row = rowbase + m.rl;
-            if (row >= op.nrows) break;
-            const double E = __ldg(op.E + row), F = __ldg(op.F + row), V2 = __ldg(op.V2 + row);
-            const double dinv = __ldg(op.Dinv + row);
-            const size_t base = (size_t)row * op.np;
-            for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
-                const int k = 2 * kv;
-                const double vp0 = __ldg(op.vp + k), vp1 = __ldg(op.vp + k + 1);
-                const double d0 = fma(vp0, E, F * __ldg(op.wp + k)), d1 = fma(vp1, E, F * __ldg(op.wp + k + 1));
-                const size_t cell = base + k;
-                const double2 bv = ld2(b, cell), qv = ld2(w.q, cell);
-                const double bs0 = V2 * vp0 * bv.x, bs1 = V2 * vp1 * bv.y;
-                double2 r;
-                r.x = bs0 - qv.x;
-                r.y = bs1 - qv.y;
-                st2(w.r, cell, r);
-                st2(w.p0, cell, make_double2(0.0, 0.0));
-                acc[0] += bs0 * bs0 + bs1 * bs1;
-                acc[1] += r.x * r.x + r.y * r.y;
-                acc[2] += UNIFORM ? r.x * (r.x * dinv) + r.y * (r.y * dinv)      // same z as K1/K2 use
-                                  : r.x * (r.x / d0) + r.y * (r.y / d1);
-            }
-        }
-    if (grid_sum<NT, 3>(acc, w.partials, &w.st->ticket[0], sh) && threadIdx.x == 0) {
-        State *st = w.st;
-        const double bb = acc[0], rr = acc[1], rho = acc[2];
-        st->bb = bb; st->rr = rr; st->rho = rho;
-        st->beta = 0.0; st->alpha = 0.0; st->sigma = 0.0;
-        st->k = 0; st->launches = 0;
-        int active = 0, status = ST_OK;
-        if (!isfinite(bb) || !isfinite(rr) || !isfinite(rho)) {
-            w.hist[0] = sqrt(rr / bb);          // a non-finite scalar (NaN / Inf in b or x0): breakdown, x untouched
-            status = ST_BREAKDOWN;
-        } else if (bb == 0.0) {
-            w.hist[0] = 0.0;                    // zero RHS: x = 0 (host zeroes x), 0 iterations
-        } else {
-            const double h = sqrt(rr / bb);
-            w.hist[0] = h;
-            active = (0 < w.args->maxit) && (h > w.args->rtol) && (rho != 0.0);
-            if (!active) status = (h <= w.args->rtol || rho == 0.0) ? ST_OK : ST_MAXIT;
-        }
-        st->active = active;
-        st->status = status;
+    Ctl *c = w.ctl;
+    if (nvoters == 1) {
+        c->loop = active;
         set_cond(cond, use_cond, active);
+        return;
+    }
+    if (active) atomicAdd(&c->any, 1);
+    __threadfence();
+    if (atomicAdd(&c->votes, 1) == nvoters - 1) {
+        __threadfence();
+        const int any = atomicExch(&c->any, 0);
+        c->votes = 0;                          // re-arm for the next voting kernel (stream order separates them)
+        c->loop = any > 0;
+        set_cond(cond, use_cond, any > 0);
     }
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2 (S4+S5): x += alpha p; r -= alpha q; z = r/d; rho' = r.z; rr = r.r; last block: k++,
-// hist[k], beta, convergence test, graph conditional.  6N doubles of traffic.
+// scalar steps (SURVEY 8(a) S1 tail, S3, S5), run by ONE thread once a reduction is complete
 // ---------------------------------------------------------------------------------------------
-// XF = true: the x-update lives in K1 (deferred one iteration), K2 only touches r and q: 3N doubles.
-// the last block of every K2 variant ends with this (S5): k++, hist[k], beta, convergence test
-__device__ __forceinline__ void k2_finish(State *st, const Work &w, double rho1, double rr,
+__device__ __forceinline__ void init_finish(const Work &w, int rhs, int nvoters, double bb, double rr, double rho,
+                                            cudaGraphConditionalHandle cond, int use_cond)
+{
+    State *st = w.st + rhs;
+    double *hist = w.hist + (size_t)rhs * w.hstride;
+    st->bb = bb; st->rr = rr; st->rho = rho;
+    st->beta = 0.0; st->alpha = 0.0; st->sigma = 0.0;
+    st->k = 0; st->launches = 0;
+    int active = 0, status = ST_OK;
+    if (!isfinite(bb) || !isfinite(rr) || !isfinite(rho)) {
+        hist[0] = sqrt(rr / bb);                // a non-finite scalar (NaN / Inf in b or x0): breakdown, x untouched
+        status = ST_BREAKDOWN;
+    } else if (bb == 0.0) {
+        hist[0] = 0.0;                          // zero RHS: x = 0 (host zeroes x), 0 iterations
+    } else {
+        const double h = sqrt(rr / bb);
+        hist[0] = h;
+        active = (0 < w.args->maxit) && (h > w.args->rtol) && (rho != 0.0);
+        if (!active) status = (h <= w.args->rtol || rho == 0.0) ? ST_OK : ST_MAXIT;
+    }
+    st->active = active;
+    st->status = status;
+    loop_vote(w, active, nvoters, cond, use_cond);
+}
+
+// S3: sigma -> alpha, breakdown test.  (No vote: K2 of the same iteration reports for this right-hand side.)
+__device__ __forceinline__ void k1_finish(const Work &w, int rhs, double sigma)
+{
+    State *st = w.st + rhs;
+    st->sigma = sigma;
+    st->launches += 1;
+    if (!(sigma > 0.0) || isinf(sigma)) {
+        st->status = ST_BREAKDOWN;
+        st->active = 0;
+        st->alpha = 0.0;                 // nothing pending for the x tail
+    } else {
+        st->alpha = st->rho / sigma;
+    }
+}
+
+// S5: k++, hist[k], beta, convergence test, loop condition
+__device__ __forceinline__ void k2_finish(const Work &w, int rhs, int nvoters, double rho1, double rr,
                                           cudaGraphConditionalHandle cond, int use_cond)
 {
+    State *st = w.st + rhs;
     const int k = st->k + 1;
     const double h = sqrt(rr / st->bb);
-    w.hist[k] = h;
+    w.hist[(size_t)rhs * w.hstride + k] = h;
     st->beta = rho1 / st->rho;
     st->rho = rho1;
     st->rr = rr;
@@ -217,37 +135,120 @@ __device__ __forceinline__ void k2_finish(State *st, const Work &w, double rho1,
         st->status = ST_BREAKDOWN;
     } else if (!active) st->status = (h <= w.args->rtol || rho1 == 0.0) ? ST_OK : ST_MAXIT;
     st->active = active;
-    set_cond(cond, use_cond, active);
+    loop_vote(w, active, nvoters, cond, use_cond);
 }
 
+// What the last block of a reducing kernel does with its totals: finish the scalar step, or (slab mode)
+// leave them for k_slab_combine, which adds the slabs' sums in slab order.
+enum { ROLE_INIT = 0, ROLE_K1 = 1, ROLE_K2 = 2 };
+template <int ROLE, int NQ>
+__device__ __forceinline__ void reduction_done(const Work &w, int rhs, const double (&tot)[NQ],
+                                               cudaGraphConditionalHandle cond, int use_cond)
+{
+    if (w.slab_sums) {
+#pragma unroll
+        for (int q = 0; q < NQ; q++) w.slab_sums[(ROLE * 3 + q) * MAX_SLABS + w.slab] = tot[q];
+        return;
+    }
+    if (ROLE == ROLE_INIT) init_finish(w, rhs, gridDim.y, tot[0], tot[NQ > 1 ? 1 : 0], tot[NQ > 2 ? 2 : 0], cond, use_cond);
+    else if (ROLE == ROLE_K1) k1_finish(w, rhs, tot[0]);
+    else k2_finish(w, rhs, gridDim.y, tot[0], tot[NQ > 1 ? 1 : 0], cond, use_cond);
+}
+
+// Slab combine ("the two scalar reductions combine per-slab partials in fixed slab order").
+// One thread; on a multi-GPU node every rank would run this on its own copy of the state after the slabs' sums
+// have been exchanged, and all ranks would obtain identical scalars.
+__global__ void k_slab_combine(Work w, int role, int nslab, cudaGraphConditionalHandle cond, int use_cond)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (role != ROLE_INIT && !w.st->active) {
+        if (role == ROLE_K2) loop_vote(w, 0, 1, cond, use_cond);
+        return;
+    }
+    double t[3] = {0.0, 0.0, 0.0};
+    for (int q = 0; q < 3; q++)
+        for (int s = 0; s < nslab; s++) t[q] += w.slab_sums[(role * 3 + q) * MAX_SLABS + s];
+    if (role == ROLE_INIT) init_finish(w, 0, 1, t[0], t[1], t[2], cond, use_cond);
+    else if (role == ROLE_K1) k1_finish(w, 0, t[0]);
+    else k2_finish(w, 0, 1, t[0], t[1], cond, use_cond);
+}
+
+// ---------------------------------------------------------------------------------------------
+// init (S1): r = V.b - q (q = A x0), p_in = 0, bb = |V.b|^2, rr = |r|^2, rho = r.(r/d); then the
+// last block sets hist[0], k = 0, beta = 0 and the loop condition.
+// ---------------------------------------------------------------------------------------------
+template <int NT, bool UNIFORM>
+__global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond)
+{
+    __shared__ double sh[32];
+    const int rhs = blockIdx.y;
+    const double *b = w.args->b[rhs];
+    double *rv = w.r + rhs * w.vstride, *p0 = w.p0 + rhs * w.vstride;
+    const double *qv0 = w.q + rhs * w.vstride;
+    const int crow0 = op.i_lo * op.nt;
+    const RowMap m = row_map<NT>(op.nv);
+    double acc[3] = {0.0, 0.0, 0.0};   // bb, rr, rho
+    if (!m.idle)
+        for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
+            const int row = rowbase + m.rl;
+            if (row >= op.nrows) break;
+            const int crow = row + crow0;
+            const double E = __ldg(op.E + crow), F = __ldg(op.F + crow), V2 = __ldg(op.V2 + crow);
+            const double dinv = __ldg(op.Dinv + crow);
+            const size_t base = (size_t)row * op.np;
+            for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
+                const int k = 2 * kv;
+                const double vp0 = __ldg(op.vp + k), vp1 = __ldg(op.vp + k + 1);
+                const double d0 = fma(vp0, E, F * __ldg(op.wp + k)), d1 = fma(vp1, E, F * __ldg(op.wp + k + 1));
+                const size_t cell = base + k;
+                const double2 bv = ld2(b, cell), qv = ld2(qv0, cell);
+                const double bs0 = V2 * vp0 * bv.x, bs1 = V2 * vp1 * bv.y;
+                double2 r;
+                r.x = bs0 - qv.x;
+                r.y = bs1 - qv.y;
+                st2(rv, cell, r);
+                st2(p0, cell, make_double2(0.0, 0.0));
+                acc[0] += bs0 * bs0 + bs1 * bs1;
+                acc[1] += r.x * r.x + r.y * r.y;
+                acc[2] += UNIFORM ? r.x * (r.x * dinv) + r.y * (r.y * dinv)      // same z as K1/K2 use
+                                  : r.x * (r.x / d0) + r.y * (r.y / d1);
+            }
+        }
+    if (grid_sum<NT, 3>(acc, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 0], sh) && threadIdx.x == 0)
+        reduction_done<ROLE_INIT, 3>(w, rhs, acc, cond, use_cond);
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2 (S4+S5): r -= alpha q; z = r/d (not stored); rho' = r.z; rr = r.r; last block: k++, hist[k], beta,
+// convergence test, loop condition.  3N doubles of traffic: the x-update lives in K1 (deferred one iteration).
 // `reverse`: sweep the rows from the last to the first (serpentine: K1 marches forward in r, so the
 // planes it touched last -- q, r -- are still in L2 when K2 starts there, and K2's last rows are in L2
 // when the next K1 starts at i = 0).  The row -> block -> partial mapping stays fixed, so determinism holds.
-template <int NT, bool UNIFORM, bool XF>
+// ---------------------------------------------------------------------------------------------
+template <int NT, bool UNIFORM>
 __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond,
                                              int reverse)
 {
     __shared__ double sh[32];
-    cudaGridDependencySynchronize();                  // PDL edge from K1 (no-op for a plain launch)
-    State *st = w.st;
-    if (!st->active) return;
+    const int rhs = blockIdx.y;
+    State *st = w.st + rhs;
+    if (!st->active) {                                // this right-hand side is done: report, nothing else
+        if (blockIdx.x == 0 && threadIdx.x == 0 && !w.slab_sums) loop_vote(w, 0, gridDim.y, cond, use_cond);
+        return;
+    }
     const double alpha = st->alpha;
-    const double *p = (st->k & 1) ? w.p0 : w.p1;      // written by K1 of this iteration
-    double *x = w.args->x;
+    double *rvec = w.r + rhs * w.vstride;
+    const double *qvec = w.q + rhs * w.vstride;
+    const int crow0 = op.i_lo * op.nt;
     const RowMap m = row_map<NT>(op.nv);
     double acc[2] = {0.0, 0.0};   // rho', rr
     // Two row groups per trip (A and B, one grid stride apart): their loads are issued together, which
     // doubles the bytes in flight per thread -- K2 has no other latency hiding than memory parallelism.
-    auto body = [&](int row, int kv, double2 rv, double2 qv, double2 xv, double2 pv, double E, double F, double dinv) {
+    auto body = [&](int row, int kv, double2 rv, double2 qv, double E, double F, double dinv) {
         const size_t cell = (size_t)row * op.np + 2 * kv;
-        if (!XF) {
-            xv.x = fma(alpha, pv.x, xv.x);
-            xv.y = fma(alpha, pv.y, xv.y);
-            st2(x, cell, xv);
-        }
         rv.x = fma(-alpha, qv.x, rv.x);
         rv.y = fma(-alpha, qv.y, rv.y);
-        st2(w.r, cell, rv);
+        st2(rvec, cell, rv);
         double z0, z1;
         if (UNIFORM) { z0 = rv.x * dinv; z1 = rv.y * dinv; }
         else {
@@ -267,40 +268,36 @@ __global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditio
             if (!okA) break;
             if (reverse) { rowA = op.nrows - 1 - rowA; rowB = op.nrows - 1 - rowB; }
             double EA = 0, FA = 0, dA = 0, EB = 0, FB = 0, dB = 0;
-            if (UNIFORM) { dA = __ldg(op.Dinv + rowA); if (okB) dB = __ldg(op.Dinv + rowB); }
+            if (UNIFORM) { dA = __ldg(op.Dinv + crow0 + rowA); if (okB) dB = __ldg(op.Dinv + crow0 + rowB); }
             else {
-                EA = __ldg(op.E + rowA); FA = __ldg(op.F + rowA);
-                if (okB) { EB = __ldg(op.E + rowB); FB = __ldg(op.F + rowB); }
+                EA = __ldg(op.E + crow0 + rowA); FA = __ldg(op.F + crow0 + rowA);
+                if (okB) { EB = __ldg(op.E + crow0 + rowB); FB = __ldg(op.F + crow0 + rowB); }
             }
             const size_t baseA = (size_t)rowA * op.np, baseB = okB ? (size_t)rowB * op.np : 0;
             for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
                 const size_t cA = baseA + 2 * kv, cB = baseB + 2 * kv;
-                const double2 rA = ld2(w.r, cA), qA = ld2(w.q, cA);
-                const double2 rB = okB ? ld2(w.r, cB) : zero, qB = okB ? ld2(w.q, cB) : zero;
-                double2 xA = zero, pA = zero, xB = zero, pB = zero;
-                if (!XF) {
-                    xA = ld2(x, cA); pA = ld2(p, cA);
-                    if (okB) { xB = ld2(x, cB); pB = ld2(p, cB); }
-                }
-                body(rowA, kv, rA, qA, xA, pA, EA, FA, dA);
-                if (okB) body(rowB, kv, rB, qB, xB, pB, EB, FB, dB);
+                const double2 rA = ld2(rvec, cA), qA = ld2(qvec, cA);
+                const double2 rB = okB ? ld2(rvec, cB) : zero, qB = okB ? ld2(qvec, cB) : zero;
+                body(rowA, kv, rA, qA, EA, FA, dA);
+                if (okB) body(rowB, kv, rB, qB, EB, FB, dB);
             }
         }
     }
-    cudaTriggerProgrammaticLaunchCompletion();        // PDL: K1 of the next iteration may start its prologue
-    if (grid_sum<NT, 2>(acc, w.partials, &st->ticket[2], sh) && threadIdx.x == 0)
-        k2_finish(st, w, acc[0], acc[1], cond, use_cond);
+    if (grid_sum<NT, 2>(acc, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 2], sh) && threadIdx.x == 0)
+        reduction_done<ROLE_K2, 2>(w, rhs, acc, cond, use_cond);
 }
 
-// XF tail (after the loop): the one x-update still pending, x += alpha_{k-1} p_{k-1}.  alpha is 0 when
+// x tail (after the loop): the one x-update still pending, x += alpha_{k-1} p_{k-1}.  alpha is 0 when
 // nothing is pending (no iteration ran, or K1 broke down after applying the previous update).
 template <int NT>
 __global__ void __launch_bounds__(NT) k_xtail(OpDev op, Work w)
 {
-    const State *st = w.st;
+    const int rhs = blockIdx.y;
+    const State *st = w.st + rhs;
     const double alpha = st->alpha;
-    const double *p = (st->k & 1) ? w.p1 : w.p0;
-    double *x = w.args->x;
+    if (alpha == 0.0) return;
+    const double *p = ((st->k & 1) ? w.p1 : w.p0) + rhs * w.vstride;
+    double *x = w.args->x[rhs];
     const RowMap m = row_map<NT>(op.nv);
     if (m.idle) return;
     for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
@@ -315,105 +312,6 @@ __global__ void __launch_bounds__(NT) k_xtail(OpDev op, Work w)
             xv.y = fma(alpha, pv.y, xv.y);
             st2(x, cell, xv);
         }
-    }
-}
-
-// the last block of every K1 variant ends with this: sigma -> alpha, breakdown test (S3)
-__device__ __forceinline__ void k1_finish(State *st, double sigma, cudaGraphConditionalHandle cond, int use_cond)
-{
-    st->sigma = sigma;
-    st->launches += 1;
-    if (!(sigma > 0.0) || isinf(sigma)) {
-        st->status = ST_BREAKDOWN;
-        st->active = 0;
-        st->alpha = 0.0;                 // nothing pending for the XF tail
-        set_cond(cond, use_cond, 0);
-    } else {
-        st->alpha = st->rho / sigma;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// K1 variant 0 (S2): p_new = r/d + beta p_old at the cell and at each of its 6 neighbours
-// (recomputed), q = A p_new, sigma = p_new.q.  Neighbour rows come through L1/L2.
-// ---------------------------------------------------------------------------------------------
-template <bool UNIFORM>
-__device__ __forceinline__ double pn1(double r, double p, double beta, double E, double F, double dinv, double vp,
-                                      double wp)
-{
-    return fma(beta, p, UNIFORM ? r * dinv : r / fma(vp, E, F * wp));   // same z as K2 computes
-}
-
-template <int NT, bool UNIFORM>
-__global__ void __launch_bounds__(NT) k1_v0(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond)
-{
-    __shared__ double sh[32];
-    State *st = w.st;
-    if (!st->active) return;
-    const double beta = st->beta;
-    const double *pin = (st->k & 1) ? w.p1 : w.p0;
-    double *pout = (st->k & 1) ? w.p0 : w.p1;
-    const double *r = w.r;
-    const RowMap m = row_map<NT>(op.nv);
-    const double2 zero = make_double2(0.0, 0.0);
-    double acc[1] = {0.0};
-    if (!m.idle)
-        for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
-            const int row = rowbase + m.rl;
-            if (row >= op.nrows) break;
-            const int i = row / op.nt, j = row - i * op.nt;
-            const RowCoef c = load_coef(op, i, j);
-            const size_t base = (size_t)row * op.np;
-            const size_t sr = (size_t)op.nt * op.np;
-            for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
-                const PhiCoef f = load_phi(op, kv);
-                const size_t cell = base + 2 * kv;
-                auto pnv = [&](size_t cl, int rw) {
-                    const double2 rv = ld2(r, cl), pv = ld2(pin, cl);
-                    const double E = __ldg(op.E + rw), F = __ldg(op.F + rw), di = __ldg(op.Dinv + rw);
-                    return make_double2(pn1<UNIFORM>(rv.x, pv.x, beta, E, F, di, f.vp0, f.wp0),
-                                        pn1<UNIFORM>(rv.y, pv.y, beta, E, F, di, f.vp1, f.wp1));
-                };
-                const double2 u = pnv(cell, row);
-                const double2 uim = i > 0 ? pnv(cell - sr, row - op.nt) : zero;
-                const double2 uip = i < op.nr - 1 ? pnv(cell + sr, row + op.nt) : zero;
-                const double2 ujm = j > 0 ? pnv(cell - op.np, row - 1) : zero;
-                const double2 ujp = j < op.nt - 1 ? pnv(cell + op.np, row + 1) : zero;
-                const double di = __ldg(op.Dinv + row);
-                const double ukm = pn1<UNIFORM>(r[base + f.km], pin[base + f.km], beta, c.E, c.F, di,
-                                                __ldg(op.vp + f.km), __ldg(op.wp + f.km));
-                const double ukp = pn1<UNIFORM>(r[base + f.kp], pin[base + f.kp], beta, c.E, c.F, di,
-                                                __ldg(op.vp + f.kp), __ldg(op.wp + f.kp));
-                const double2 q = stencil(c, f, u, uim, uip, ujm, ujp, ukm, ukp);
-                st2(pout, cell, u);
-                st2(w.q, cell, q);
-                acc[0] += u.x * q.x + u.y * q.y;
-            }
-        }
-    if (grid_sum<NT, 1>(acc, w.partials, &st->ticket[1], sh) && threadIdx.x == 0)
-        k1_finish(st, acc[0], cond, use_cond);
-}
-
-// ---------------------------------------------------------------------------------------------
-// Measurement aids (mas_pcg_mix_probe): trivial LINEAR kernels with the DRAM read/write mix of K1 and K2 and
-// none of their structure -- what the memory system sustains for that mix, as context for the rooflines.
-// ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_mix6(const double2 *a, const double2 *b, double2 *x, double2 *p, double2 *q,
-                                              size_t n2)        // K1 (xfuse): reads a, b, x; writes p, q, x
-{
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x) {
-        const double2 av = a[i], bv = b[i], xv = x[i];
-        p[i] = make_double2(av.x + bv.x, av.y + bv.y);
-        q[i] = make_double2(av.x - bv.x, av.y - bv.y);
-        x[i] = make_double2(xv.x + 0.5 * av.x, xv.y + 0.5 * av.y);
-    }
-}
-
-__global__ void __launch_bounds__(256) k_mix3(double2 *r, const double2 *q, size_t n2)   // K2: reads r, q; writes r
-{
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x) {
-        const double2 rv = r[i], qv = q[i];
-        r[i] = make_double2(rv.x - 0.5 * qv.x, rv.y - 0.5 * qv.y);
     }
 }
 

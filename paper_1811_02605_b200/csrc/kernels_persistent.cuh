@@ -21,12 +21,68 @@ namespace mas {
 
 namespace cg = cooperative_groups;
 
+// ---------------------------------------------------------------------------------------------
+// the 7-point stencil on one double2 (cells k = 2kv, k+1 of row (i,j)), coefficient form, operands from global memory:
+//   (A u)_c = d_c u_c - vp[k] (ARm u_im + ARp u_ip + ATm u_jm + ATp u_jp) - F (ip[k] u_kp + ip[k-1] u_km)
+// ---------------------------------------------------------------------------------------------
+struct RowCoef {
+    double E, F, ARm, ARp, ATm, ATp;
+};
+
+__device__ __forceinline__ RowCoef load_coef(const OpDev &op, int i, int j)
+{
+    RowCoef c;
+    const int row = i * op.nt + j;
+    c.E = __ldg(op.E + row);
+    c.F = __ldg(op.F + row);
+    c.ARm = __ldg(op.AR + row);
+    c.ARp = __ldg(op.AR + row + op.nt);
+    c.ATm = __ldg(op.AT + i * (op.nt + 1) + j);
+    c.ATp = __ldg(op.AT + i * (op.nt + 1) + j + 1);
+    return c;
+}
+
+struct PhiCoef {            // phi factors of the two cells of a vector and their outer faces
+    double vp0, vp1, wp0, wp1, ipm, ip0, ip1;   // ipm = ip[k-1], ip0 = ip[k], ip1 = ip[k+1]
+    int km, kp;                                 // wrapped neighbour cells k-1 and k+2
+};
+
+__device__ __forceinline__ PhiCoef load_phi(const OpDev &op, int kv)
+{
+    PhiCoef c;
+    const int k = 2 * kv;
+    c.km = k == 0 ? op.np - 1 : k - 1;
+    c.kp = k + 2 >= op.np ? 0 : k + 2;
+    c.vp0 = __ldg(op.vp + k);
+    c.vp1 = __ldg(op.vp + k + 1);
+    c.wp0 = __ldg(op.wp + k);
+    c.wp1 = __ldg(op.wp + k + 1);
+    c.ipm = __ldg(op.ip + c.km);
+    c.ip0 = __ldg(op.ip + k);
+    c.ip1 = __ldg(op.ip + k + 1);
+    return c;
+}
+
+__device__ __forceinline__ double2 stencil(const RowCoef &c, const PhiCoef &f, double2 u, double2 uim,
+                                           double2 uip, double2 ujm, double2 ujp, double ukm, double ukp)
+{
+    const double d0 = fma(f.vp0, c.E, c.F * f.wp0);
+    const double d1 = fma(f.vp1, c.E, c.F * f.wp1);
+    const double sx = c.ARm * uim.x + c.ARp * uip.x + c.ATm * ujm.x + c.ATp * ujp.x;
+    const double sy = c.ARm * uim.y + c.ARp * uip.y + c.ATm * ujm.y + c.ATp * ujp.y;
+    double2 q;
+    q.x = d0 * u.x - f.vp0 * sx - c.F * (f.ip0 * u.y + f.ipm * ukm);
+    q.y = d1 * u.y - f.vp1 * sy - c.F * (f.ip1 * ukp + f.ip0 * u.x);
+    return q;
+}
+
 constexpr int PNT = 512;         // threads per block, one block per SM
 constexpr int PMAX_SMEM = 226 * 1024;   // dynamic shared memory available to the one block per SM
 
 struct PersistParams {
     double *Z, *P0, *P1;         // handle-owned N-vectors (the streaming path's r, p0, p1 workspaces)
-    double *partials;            // [6][MAX_PARTIALS]: regions 0 (sigma), 1-2 (rho', rr), 3-5 (init)
+    double *partials;            // [6][pstride]: regions 0 (sigma), 1-2 (rho', rr), 3-5 (init)
+    int pstride;                 // >= gridDim.x
     double *hist;
     State *st;
     const SolveArgs *args;
@@ -38,20 +94,20 @@ inline size_t persist_smem(int M) { return (size_t)M * PNT * (4 * sizeof(double2
 
 // fixed-order sum of NP partial arrays written by all blocks; result identical in every block
 template <int NP>
-__device__ __forceinline__ void all_sum(double (&v)[NP], double *partials, double *sh, cg::grid_group &grid)
+__device__ __forceinline__ void all_sum(double (&v)[NP], double *partials, int pstride, double *sh, cg::grid_group &grid)
 {
     const int G = gridDim.x;
 #pragma unroll
     for (int q = 0; q < NP; q++) {
         const double t = block_sum<PNT>(v[q], sh);
-        if (threadIdx.x == 0) partials[q * MAX_PARTIALS + blockIdx.x] = t;
+        if (threadIdx.x == 0) partials[(size_t)q * pstride + blockIdx.x] = t;
     }
     grid.sync();
 #pragma unroll
     for (int q = 0; q < NP; q++) {
         double a = 0.0;
         if (threadIdx.x < 32) {
-            for (int i = threadIdx.x; i < G; i += 32) a += __ldcg(&partials[q * MAX_PARTIALS + i]);
+            for (int i = threadIdx.x; i < G; i += 32) a += __ldcg(&partials[(size_t)q * pstride + i]);
             a = warp_sum(a);
         }
         if (threadIdx.x == 0) sh[q] = a;
@@ -68,8 +124,8 @@ __global__ void __launch_bounds__(PNT, 1) k_pcg_persistent(OpDev op, PersistPara
     __shared__ double sh[32];
     extern __shared__ __align__(16) unsigned char psm[];
     cg::grid_group grid = cg::this_grid();
-    const double *__restrict__ b = pp.args->b;
-    double *__restrict__ xg = pp.args->x;
+    const double *__restrict__ b = pp.args->b[0];
+    double *__restrict__ xg = pp.args->x[0];
     const double rtol = pp.args->rtol;
     const int maxit = pp.args->maxit;
     const int M = pp.M, tid = threadIdx.x;
@@ -146,7 +202,7 @@ __global__ void __launch_bounds__(PNT, 1) k_pcg_persistent(OpDev op, PersistPara
         acc3[1] += rv.x * rv.x + rv.y * rv.y;
         acc3[2] += rv.x * z.x + rv.y * z.y;
     }
-    all_sum<3>(acc3, pp.partials + 3 * MAX_PARTIALS, sh, grid);      // barrier: Z, P1 visible
+    all_sum<3>(acc3, pp.partials + 3 * (size_t)pp.pstride, pp.pstride, sh, grid);      // barrier: Z, P1 visible
     const double bb = acc3[0];
     double rho = acc3[2], rr = acc3[1], beta = 0.0, alpha = 0.0;
     int k = 0, status = ST_OK, active = 0;
@@ -180,7 +236,7 @@ __global__ void __launch_bounds__(PNT, 1) k_pcg_persistent(OpDev op, PersistPara
             SQ[m * PNT + tid] = q;
             a1[0] += pv.x * q.x + pv.y * q.y;
         }
-        all_sum<1>(a1, pp.partials, sh, grid);            // barrier A: all reads of Z (= z_k) are done
+        all_sum<1>(a1, pp.partials, pp.pstride, sh, grid);            // barrier A: all reads of Z (= z_k) are done
         const double sigma = a1[0];
         if (!(sigma > 0.0) || isinf(sigma)) { status = ST_BREAKDOWN; break; }
         alpha = rho / sigma;
@@ -203,7 +259,7 @@ __global__ void __launch_bounds__(PNT, 1) k_pcg_persistent(OpDev op, PersistPara
             a2[0] += rv.x * z.x + rv.y * z.y;
             a2[1] += rv.x * rv.x + rv.y * rv.y;
         }
-        all_sum<2>(a2, pp.partials + MAX_PARTIALS, sh, grid);   // barrier B: Z (= z_{k+1}) and P[k&1] visible
+        all_sum<2>(a2, pp.partials + (size_t)pp.pstride, pp.pstride, sh, grid);   // barrier B: Z (= z_{k+1}) and P[k&1] visible
         const double rho1 = a2[0];
         rr = a2[1];
         k += 1;

@@ -1,61 +1,55 @@
-// kernels_stencil_tma.cuh -- k_stencil with the TMA engine as the loader: every tile row of a plane is ONE
-// bulk copy (cp.async.bulk.shared::cluster.global, SASS UBLKCP) that signals an mbarrier with complete_tx, and
-// the per-plane __syncthreads of k_stencil is replaced by a full/empty mbarrier pair per ring slot:
+// kernels_stencil_tma.cuh -- the matrix-free 7-point stencil applied to a STORED vector, as a 2.5-D marching kernel
+// (tiling: tile.cuh) with a fused epilogue.  Used by
+//   * mas_pcg_apply and the initial residual (EPI_APPLY:  out = S u,  S = A_sym with the dt-scaled planes),
+//   * the RKL2 super-time-stepping stages of NEXT-1 (EPI_STS: S = L_sym from the dt-independent planes,
+//     M u = -S u / V,  out = c_u u + c_a1 a1 + c_a2 a2 + c_L M u + c_a3 a3,  optionally out2 = M u)
+//     -- PAPER.md:65 "Runge-Kutta Legendre super time-stepping (STS) scheme [21]", "explicit
+//     finite difference algorithms (such as ... the STS algorithm)",
+//   * K2R, the fused vector kernel of the 64 B/cell/iteration PCG (EPI_K2R: u = p written by K1 of this iteration,
+//     q = A_sym p recomputed instead of read, r -= alpha q in place, rho' = r.z, rr = r.r, then the scalar step S5).
+// The TMA engine is the loader: every tile row of a plane is ONE bulk copy (cp.async.bulk.shared::cluster.global,
+// SASS UBLKCP) that signals an mbarrier with complete_tx; a full/empty mbarrier pair per ring slot replaces the
+// per-plane block barrier:
 //   full[s]  : count NW; lane 0 of every warp arrives with expect_tx(bytes of its row: the 1 KB row segment, the two
 //              16-byte phi-halo pairs, and for interior rows the epilogue's extra streams); it completes when all rows
 //              of the plane have landed, which also makes them visible to every waiting thread;
 //   empty[s] : count NW; a warp arrives once it no longer needs the plane in slot s (its theta-neighbours' rows were
 //              read); lane 0 of a warp waits on it before refilling ITS row of slot s (planes are DEPTH+2 apart).
 // Warps therefore drift by up to one plane instead of meeting at a block barrier every plane.
-// Same tiling, arithmetic and epilogues (EPI_APPLY, EPI_STS) as k_stencil; selected by stencil tiles 6 and 7.
 #pragma once
-#include "kernels_stencil.cuh"
+#include "kernels_base.cuh"
+#include "tile.cuh"
 
 namespace mas {
 
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, unsigned parity)
-{
-    unsigned ok;
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    return ok != 0;
-}
-// bounded wait: a protocol mistake must abort the kernel, not hang the GPU
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
-{
-    for (unsigned spin = 0; !mbar_try_wait(bar, parity); ++spin)
-        if (spin > (1u << 24)) __trap();
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
+enum { EPI_APPLY = 0, EPI_STS = 1, EPI_K2R = 2 };
 
-template <int TJ, int DEPTH, int NX>      // NX = 3 extra streams (EPI_STS) or 0
+struct StencilParams {
+    TileParams t;
+    PlaneSetDev ps;                       // plane set: A_sym (dt-scaled) or L_sym (base); ps.D = Vinv (STS) / Dinv (K2R)
+    const double *u, *u_lo, *u_hi;        // the vector the stencil is applied to (null: args->x[rhs]) and its slab halos
+    long long ustride;                    // right-hand side j of u / out at + j * ustride
+    const SolveArgs *args;
+    double *out, *out2;
+    const double *a1, *a2, *a3;           // EPI_STS: Y_{j-2}, Y_0, M Y_0 (null = absent)
+    double c_u, c_a1, c_a2, c_L, c_a3;
+    int *fault;
+    // EPI_K2R
+    Work w;
+    cudaGraphConditionalHandle cond;
+    int use_cond;
+};
+
+template <int TJ, int DEPTH, int NX, bool UNIFORM>      // NX extra streams: 3 (EPI_STS), 1 (EPI_K2R: r), 0
 struct StencilTmaSmem {
     static constexpr int NW = TJ + 2;
     static constexpr int NT = NW * 32;
     static constexpr int R = DEPTH + 2;
-    static constexpr int NPL = MARCH_CI_MAX + 2;
     alignas(16) double2 ring[R][NW][64];                 // [slot][row][128 cells]
     alignas(16) double2 halo[R][NW][2];                  // [slot][row][left pair (kl-1, kl) | right pair (kr, kr+1)]
-    alignas(16) double2 xf[NX ? DEPTH : 1][NX ? NX : 1][NX ? TJ : 1][NX ? 64 : 1];   // [stage][a1 a2 a3][interior row][128 cells]
-    double cE[NPL][NW], cF[NPL][NW], cAR[NPL][NW], cAT[NPL][NW], cV[NPL][NW];
-    double phv[WIDE_TK + 2], phw[WIDE_TK + 2], phi[WIDE_TK + 2];
+    alignas(16) double2 xf[NX ? DEPTH : 1][NX ? NX : 1][NX ? TJ : 1][NX ? 64 : 1];   // [stage][stream][interior row][128 cells]
+    TileCoefs<NW, UNIFORM> c;
+    double red[32];
     alignas(8) uint64_t full[R], empty[R];
 };
 
@@ -63,52 +57,42 @@ template <int TJ, int DEPTH, bool UNIFORM, int MINB, int EPI>
 __global__ void __launch_bounds__((TJ + 2) * 32, MINB)
 k_stencil_tma(OpDev op, StencilParams mp)
 {
-    static_assert(EPI == EPI_APPLY || EPI == EPI_STS, "TMA variant: apply and STS epilogues");
-    using Smem = StencilTmaSmem<TJ, DEPTH, EPI == EPI_STS ? 3 : 0>;
+    constexpr int NX = EPI == EPI_STS ? 3 : (EPI == EPI_K2R ? 1 : 0);
+    using Smem = StencilTmaSmem<TJ, DEPTH, NX, UNIFORM>;
     constexpr int NT = Smem::NT, NW = Smem::NW, R = Smem::R;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     Smem &sm = *reinterpret_cast<Smem *>(smem_raw);
 
-    const double *__restrict__ uvec = mp.u ? mp.u : mp.args->x;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, tid = threadIdx.x;
-    int b = blockIdx.x;
-    const int kt = b % mp.nkt; b /= mp.nkt;
-    const int jt = b % mp.njt;
-    const int it = b / mp.njt;
-    const int i0 = it * mp.ci, i1 = min(i0 + mp.ci, op.nr);
-    const int first = i0 - 1, nsteps = i1 - i0 + 2;
-    const int j = jt * TJ + warp - 1;
-    const int k0 = kt * WIDE_TK;
-    const int tkeff = min(WIDE_TK, op.np - k0);
-    const bool row_ok = (j >= 0) && (j < op.nt);
-    const bool vA = row_ok && (2 * lane < tkeff), vB = row_ok && (64 + 2 * lane < tkeff);
-    const bool interior = (warp >= 1) && (warp <= TJ);
-    const bool qA = interior && vA, qB = interior && vB;
-    const bool left_edge = qA && (lane == 0);
-    const bool right_A = qA && (2 * lane + 2 == tkeff), right_B = qB && (64 + 2 * lane + 2 == tkeff);
-    const bool right_edge = right_A || right_B;
-    const int kl = k0 == 0 ? op.np - 1 : k0 - 1;           // odd (k0 and np are even)
-    const int kr = k0 + tkeff >= op.np ? 0 : k0 + tkeff;   // even
+    const int rhs = blockIdx.y;
+    const TileGeom g = tile_geom<TJ>(op, mp.t);
+    const int lane = g.lane, warp = g.warp, tid = g.tid;
 
-    // ---- stage coefficient columns and phi factors; zero the ring; init the barriers ----
-    for (int e = tid; e < nsteps * NW; e += NT) {
-        const int pl = e / NW, wr = e - pl * NW;
-        const int ii = first + pl, jj = jt * TJ + wr - 1;
-        const bool in = ii >= 0 && ii < op.nr && jj >= 0 && jj < op.nt;
-        const int row = ii * op.nt + jj;
-        sm.cE[pl][wr] = in ? __ldg(mp.E + row) : 0.0;
-        sm.cF[pl][wr] = in ? __ldg(mp.F + row) : 0.0;
-        sm.cV[pl][wr] = (in && EPI == EPI_STS) ? __ldg(mp.Vinv + row) : 0.0;
-        sm.cAR[pl][wr] = (ii >= 0 && ii <= op.nr && jj >= 0 && jj < op.nt) ? __ldg(mp.AR + row) : 0.0;
-        sm.cAT[pl][wr] = (ii >= 0 && ii < op.nr && jj >= 0 && jj <= op.nt) ? __ldg(mp.AT + ii * (op.nt + 1) + jj) : 0.0;
-    }
-    if (!UNIFORM)
-        for (int e = tid; e < WIDE_TK + 2; e += NT) {
-            int kk = k0 - 1 + e;
-            kk = kk < 0 ? kk + op.np : (kk >= op.np ? kk - op.np : kk);
-            kk = kk >= op.np ? kk % op.np : kk;
-            sm.phv[e] = __ldg(op.vp + kk); sm.phw[e] = __ldg(op.wp + kk); sm.phi[e] = __ldg(op.ip + kk);
+    // ---- which vectors ----
+    double alpha = 0.0;
+    VecHalo uV;
+    double *rvec = nullptr;
+    if (EPI == EPI_K2R) {                            // u = p written by K1 of this iteration; r updated in place
+        const State *st = mp.w.st + rhs;
+        if (!st->active) {                           // this right-hand side is done: report, nothing else
+            if (blockIdx.x == 0 && tid == 0 && !mp.w.slab_sums) loop_vote(mp.w, 0, gridDim.y, mp.cond, mp.use_cond);
+            return;
         }
+        alpha = st->alpha;
+        const int par = st->k & 1;                   // K1 wrote p[(k+1)&1]
+        const long long voff = rhs * mp.w.vstride;
+        uV.own = (par ? mp.w.p0 : mp.w.p1) + voff;
+        uV.lo = par ? mp.w.lo_p0 : mp.w.lo_p1;
+        uV.hi = par ? mp.w.hi_p0 : mp.w.hi_p1;
+        rvec = mp.w.r + voff;
+    } else {
+        if (mp.u) { uV.own = mp.u + rhs * mp.ustride; uV.lo = mp.u_lo; uV.hi = mp.u_hi; }
+        else { uV.own = mp.args->x[rhs]; uV.lo = mp.args->x_lo; uV.hi = mp.args->x_hi; }
+    }
+    double *out = EPI == EPI_K2R ? rvec : mp.out + rhs * mp.ustride;
+    const double *x1p = EPI == EPI_K2R ? rvec : mp.a1;           // K2R: the one extra stream is r
+    int *fault = mp.fault;
+
+    // ---- zero the ring, init the barriers, start the first planes, then stage the coefficient columns ----
 #pragma unroll
     for (int s = 0; s < R; s++) {
         sm.ring[s][warp][lane] = make_double2(0.0, 0.0);
@@ -124,117 +108,118 @@ k_stencil_tma(OpDev op, StencilParams mp)
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
     __syncthreads();
 
+    const PhiFac<UNIFORM, TileCoefs<NW, UNIFORM>> ph = {sm.c, mp.t.vp, mp.t.wp, mp.t.ip};
     const int ea = 2 * lane + 1, eb = 2 * lane + 65;
-    auto VP = [&](int e) { return UNIFORM ? mp.vp : sm.phv[e]; };
-    auto WP = [&](int e) { return UNIFORM ? mp.wp : sm.phw[e]; };
-    auto IP = [&](int e) { return UNIFORM ? mp.ip : sm.phi[e]; };
-
     const long long plane = (long long)op.nt * op.np;
-    const long long rowbase0 = (long long)first * plane + (row_ok ? (long long)j * op.np : 0);
-    const int ka = k0 + 2 * lane, kb = ka + 64;
+    const long long rowbase0 = (long long)g.first * plane + (g.row_ok ? (long long)g.j * op.np : 0);
     long long orow = rowbase0 + plane;                      // row base of plane i0: outputs
-    const bool has1 = EPI == EPI_STS && mp.a1 != nullptr, has2 = EPI == EPI_STS && mp.a2 != nullptr,
-               has3 = EPI == EPI_STS && mp.a3 != nullptr;
-    const unsigned rowbytes = (unsigned)tkeff * 8u;
+    const bool has1 = (EPI == EPI_STS && mp.a1 != nullptr) || EPI == EPI_K2R,
+               has2 = EPI == EPI_STS && mp.a2 != nullptr, has3 = EPI == EPI_STS && mp.a3 != nullptr;
+    const unsigned rowbytes = (unsigned)g.tkeff * 8u;
+    const bool hints = EPI == EPI_K2R && (mp.t.l2.keep_r | mp.t.l2.keep_p) != 0;
+    const uint64_t pol_last = hints ? l2_policy_evict_last() : 0;
 
     // lane 0 of each warp: load THIS warp's row of plane index pl (ring plane first+pl) and, for interior rows,
     // the extras of the plane whose outputs are formed when that ring plane is consumed (first+pl-1).
     auto produce = [&](int pl) {
-        const int slot = pl % R, ii = first + pl;
+        const int slot = pl % R, ii = g.first + pl;
         uint64_t *bar = &sm.full[slot];
         unsigned bytes = 0;
-        const long long rb = rowbase0 + (long long)pl * plane;
-        const bool plane_in = (unsigned)ii < (unsigned)op.nr;
-        if (row_ok && plane_in) bytes += rowbytes + (interior ? 32u : 0u);
-        const bool xin = EPI == EPI_STS && interior && row_ok && (ii - 1 >= i0) && (ii - 1 < i1);
+        const double *urow = g.row_ok ? plane_row(uV, op, ii, g.j) : nullptr;
+        if (urow) bytes += rowbytes + (g.interior ? 32u : 0u);
+        const bool xin = NX > 0 && g.interior && g.row_ok && (ii - 1 >= g.i0) && (ii - 1 < g.i1);
         if (xin) bytes += rowbytes * ((has1 ? 1u : 0u) + (has2 ? 1u : 0u) + (has3 ? 1u : 0u));
         if (bytes == 0) { mbar_arrive(bar); return; }
         mbar_arrive_expect_tx(bar, bytes);
-        if (row_ok && plane_in) {
-            bulk_g2s(&sm.ring[slot][warp][0], uvec + rb + k0, rowbytes, bar);
-            if (interior) {
-                bulk_g2s(&sm.halo[slot][warp][0], uvec + rb + (kl - 1), 16u, bar);
-                bulk_g2s(&sm.halo[slot][warp][1], uvec + rb + kr, 16u, bar);
+        if (urow) {
+            if (hints && ii < mp.t.l2.keep_p) bulk_g2s_hint(&sm.ring[slot][warp][0], urow + g.k0, rowbytes, bar, pol_last);
+            else bulk_g2s(&sm.ring[slot][warp][0], urow + g.k0, rowbytes, bar);
+            if (g.interior) {
+                bulk_g2s(&sm.halo[slot][warp][0], urow + (g.kl - 1), 16u, bar);
+                bulk_g2s(&sm.halo[slot][warp][1], urow + g.kr, 16u, bar);
             }
         }
         if (xin) {
             const int xs = pl % DEPTH;
-            const long long xb = rb - plane + k0;
-            if (has1) bulk_g2s(&sm.xf[xs][0][warp - 1][0], mp.a1 + xb, rowbytes, bar);
-            if (has2) bulk_g2s(&sm.xf[xs][1][warp - 1][0], mp.a2 + xb, rowbytes, bar);
-            if (has3) bulk_g2s(&sm.xf[xs][2][warp - 1][0], mp.a3 + xb, rowbytes, bar);
+            const long long xb = (long long)(ii - 1) * plane + (long long)g.j * op.np + g.k0;
+            if (has1) {
+                if (hints && ii - 1 < mp.t.l2.keep_r) bulk_g2s_hint(&sm.xf[xs][0][warp - 1][0], x1p + xb, rowbytes, bar, pol_last);
+                else bulk_g2s(&sm.xf[xs][0][warp - 1][0], x1p + xb, rowbytes, bar);
+            }
+            if (has2) bulk_g2s(&sm.xf[xs][NX > 1 ? 1 : 0][warp - 1][0], mp.a2 + xb, rowbytes, bar);
+            if (has3) bulk_g2s(&sm.xf[xs][NX > 2 ? 2 : 0][warp - 1][0], mp.a3 + xb, rowbytes, bar);
         }
     };
     if (lane == 0)
-        for (int pl = 0; pl < DEPTH && pl < nsteps; pl++) produce(pl);
+        for (int pl = 0; pl < DEPTH && pl < g.nsteps; pl++) produce(pl);
+
+    stage_coefs<TJ, UNIFORM>(sm.c, g, op, mp.ps);
+    __syncthreads();                                        // coefficient columns visible
 
     const double2 zero2 = make_double2(0.0, 0.0);
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
-    const int lm = (lane + 31) & 31, lp = (lane + 1) & 31;
+    double acc[2] = {0.0, 0.0};                             // K2R: rho', rr
 
-    for (int t = 0; t < nsteps; t++) {
+    for (int t = 0; t < g.nsteps; t++) {
         const int slot = t % R, slot_prev = (t + R - 1) % R;
-        const int ii = first + t;
-        const bool plane_ok = (unsigned)ii < (unsigned)op.nr;
-        mbar_wait(&sm.full[slot], (unsigned)(t / R) & 1u);          // plane ii: every row has landed
+        const int ii = g.first + t;
+        const bool plane_ok = (unsigned)(op.i_lo + ii) < (unsigned)op.nr_glob;
+        mbar_wait(&sm.full[slot], (unsigned)(t / R) & 1u, fault);   // plane ii: every row has landed
         double2 an = zero2, bn = zero2;
         double hl_n = 0.0, hr_n = 0.0;
         if (plane_ok) {
             an = sm.ring[slot][warp][lane];
             bn = sm.ring[slot][warp][lane + 32];
-            if (left_edge) hl_n = sm.halo[slot][warp][0].y;
-            if (right_edge) hr_n = sm.halo[slot][warp][1].x;
+            if (g.left_edge) hl_n = sm.halo[slot][warp][0].y;
+            if (g.right_edge) hr_n = sm.halo[slot][warp][1].x;
         }
-        const double mA = __shfl_sync(0xffffffffu, ac.y, lm), mB = __shfl_sync(0xffffffffu, bc.y, lm);
-        const double pA = __shfl_sync(0xffffffffu, ac.x, lp), pB = __shfl_sync(0xffffffffu, bc.x, lp);
-        if (t >= 2 && interior && row_ok) {
-            const double Ec = sm.cE[t - 1][warp], Fc = sm.cF[t - 1][warp];
-            const double ARm = sm.cAR[t - 1][warp], ARp = sm.cAR[t][warp];
-            const double ATm = sm.cAT[t - 1][warp], ATp = sm.cAT[t - 1][warp + 1];
-            const double vinv = EPI == EPI_STS ? sm.cV[t - 1][warp] : 0.0;
+        const PhiNb nb = phi_neighbours(ac, bc, lane);
+        if (t >= 2 && g.interior && g.row_ok) {
+            const RowCoefs rc = row_coefs(sm.c, t, warp);
+            const double dsc = EPI != EPI_APPLY ? sm.c.cD[t - 1][warp] : 0.0;      // 1/V2 (STS) or Dinv (K2R)
             const int xs = t % DEPTH;
             auto finish = [&](double2 s, double2 uc, int half, int e, int kcell) {
                 double2 o;
+                const int xi = lane + 32 * half;
+                const bool keep = hints && (ii - 1) < mp.t.l2.keep_r;
                 if (EPI == EPI_APPLY) {
                     o = s;
+                } else if (EPI == EPI_K2R) {                     // s = q = A p;  stream 0 = r
+                    const double2 rv = sm.xf[xs][0][warp - 1][xi];
+                    o.x = fma(-alpha, s.x, rv.x);
+                    o.y = fma(-alpha, s.y, rv.y);
+                    double z0, z1;
+                    if (UNIFORM) { z0 = o.x * dsc; z1 = o.y * dsc; }
+                    else { z0 = o.x / fma(ph.VP(e), rc.Ec, rc.Fc * ph.WP(e)); z1 = o.y / fma(ph.VP(e + 1), rc.Ec, rc.Fc * ph.WP(e + 1)); }
+                    acc[0] += o.x * z0 + o.y * z1;
+                    acc[1] += o.x * o.x + o.y * o.y;
                 } else {
-                    double2 mu;
-                    mu.x = UNIFORM ? -(s.x * vinv) * (1.0 / mp.vp) : -(s.x * vinv) / VP(e);
-                    mu.y = UNIFORM ? -(s.y * vinv) * (1.0 / mp.vp) : -(s.y * vinv) / VP(e + 1);
-                    if (mp.out2) st2(mp.out2, orow + kcell, mu);
+                    double2 mu;                                  // M u = -S u / (V2 vp)
+                    mu.x = UNIFORM ? -(s.x * dsc) * (1.0 / mp.t.vp) : -(s.x * dsc) / ph.VP(e);
+                    mu.y = UNIFORM ? -(s.y * dsc) * (1.0 / mp.t.vp) : -(s.y * dsc) / ph.VP(e + 1);
+                    if (mp.out2) st2g(mp.out2, orow + kcell, mu);
                     o.x = mp.c_u * uc.x + mp.c_L * mu.x;
                     o.y = mp.c_u * uc.y + mp.c_L * mu.y;
-                    const int xi = lane + 32 * half;
                     if (has1) { const double2 x1 = sm.xf[xs][0][warp - 1][xi]; o.x = fma(mp.c_a1, x1.x, o.x); o.y = fma(mp.c_a1, x1.y, o.y); }
-                    if (has2) { const double2 x2 = sm.xf[xs][1][warp - 1][xi]; o.x = fma(mp.c_a2, x2.x, o.x); o.y = fma(mp.c_a2, x2.y, o.y); }
-                    if (has3) { const double2 x3 = sm.xf[xs][2][warp - 1][xi]; o.x = fma(mp.c_a3, x3.x, o.x); o.y = fma(mp.c_a3, x3.y, o.y); }
+                    if (has2) { const double2 x2 = sm.xf[xs][NX > 1 ? 1 : 0][warp - 1][xi]; o.x = fma(mp.c_a2, x2.x, o.x); o.y = fma(mp.c_a2, x2.y, o.y); }
+                    if (has3) { const double2 x3 = sm.xf[xs][NX > 2 ? 2 : 0][warp - 1][xi]; o.x = fma(mp.c_a3, x3.x, o.x); o.y = fma(mp.c_a3, x3.y, o.y); }
                 }
-                st2(mp.out, orow + kcell, o);
+                if (keep) st2_hint(out, orow + kcell, o, pol_last); else st2g(out, orow + kcell, o);
             };
-            if (qA) {
-                const double ukm = left_edge ? hl_c : mA;
-                const double ukp = right_A ? hr_c : (lane == 31 ? pB : pA);
-                const double2 ujm = sm.ring[slot_prev][warp - 1][lane], ujp = sm.ring[slot_prev][warp + 1][lane];
-                const double d0 = fma(VP(ea), Ec, Fc * WP(ea)), d1 = fma(VP(ea + 1), Ec, Fc * WP(ea + 1));
-                const double sx = ARm * am.x + ARp * an.x + ATm * ujm.x + ATp * ujp.x;
-                const double sy = ARm * am.y + ARp * an.y + ATm * ujm.y + ATp * ujp.y;
-                double2 s;
-                s.x = d0 * ac.x - VP(ea) * sx - Fc * (IP(ea) * ac.y + IP(ea - 1) * ukm);
-                s.y = d1 * ac.y - VP(ea + 1) * sy - Fc * (IP(ea + 1) * ukp + IP(ea) * ac.x);
-                finish(s, ac, 0, ea, ka);
+            if (g.qA) {
+                const double ukm = g.left_edge ? hl_c : nb.mA;
+                const double ukp = g.right_A ? hr_c : (lane == 31 ? nb.pB : nb.pA);
+                const double2 s = stencil_half(ph, ea, rc, am, ac, an, sm.ring[slot_prev][warp - 1][lane],
+                                               sm.ring[slot_prev][warp + 1][lane], ukm, ukp);
+                finish(s, ac, 0, ea, g.ka);
             }
-            if (qB) {
-                const double ukm = lane == 0 ? mA : mB;
-                const double ukp = right_B ? hr_c : pB;
-                const double2 ujm = sm.ring[slot_prev][warp - 1][lane + 32], ujp = sm.ring[slot_prev][warp + 1][lane + 32];
-                const double d0 = fma(VP(eb), Ec, Fc * WP(eb)), d1 = fma(VP(eb + 1), Ec, Fc * WP(eb + 1));
-                const double sx = ARm * bm.x + ARp * bn.x + ATm * ujm.x + ATp * ujp.x;
-                const double sy = ARm * bm.y + ARp * bn.y + ATm * ujm.y + ATp * ujp.y;
-                double2 s;
-                s.x = d0 * bc.x - VP(eb) * sx - Fc * (IP(eb) * bc.y + IP(eb - 1) * ukm);
-                s.y = d1 * bc.y - VP(eb + 1) * sy - Fc * (IP(eb + 1) * ukp + IP(eb) * bc.x);
-                finish(s, bc, 1, eb, kb);
+            if (g.qB) {
+                const double ukm = lane == 0 ? nb.mA : nb.mB;
+                const double ukp = g.right_B ? hr_c : nb.pB;
+                const double2 s = stencil_half(ph, eb, rc, bm, bc, bn, sm.ring[slot_prev][warp - 1][lane + 32],
+                                               sm.ring[slot_prev][warp + 1][lane + 32], ukm, ukp);
+                finish(s, bc, 1, eb, g.kb);
             }
         }
         if (t >= 2) orow += plane;
@@ -242,46 +227,52 @@ k_stencil_tma(OpDev op, StencilParams mp)
         if (lane == 0) {
             if (t >= 1) mbar_arrive(&sm.empty[slot_prev]);  // plane t-1 released by this warp
             const int pl = t + DEPTH;                       // refill: plane pl goes to the slot plane pl-R used
-            if (pl < nsteps) {
+            if (pl < g.nsteps) {
                 const int use = pl / R;                     // n-th use of that slot
-                if (use >= 1) mbar_wait(&sm.empty[pl % R], (unsigned)(use - 1) & 1u);
+                if (use >= 1) mbar_wait(&sm.empty[pl % R], (unsigned)(use - 1) & 1u, fault);
                 produce(pl);
             }
         }
         am = ac; ac = an; bm = bc; bc = bn;
         hl_c = hl_n; hr_c = hr_n;
     }
+    if (EPI == EPI_K2R) {
+        if (grid_sum<NT, 2>(acc, part_base(mp.w, rhs), mp.w.pstride, &mp.w.tickets[rhs * 4 + 2], sm.red) && threadIdx.x == 0)
+            reduction_done<ROLE_K2, 2>(mp.w, rhs, acc, mp.cond, mp.use_cond);
+    }
 }
 
+// ---------------------------------------------------------------------------------------------
+// host-side configuration
+// ---------------------------------------------------------------------------------------------
 template <int TJ, int DEPTH, int MINB>
 inline void stencil_tma_pick(bool uniform, int epi, const void **func, dim3 *block, size_t *smem)
 {
     if (epi == EPI_APPLY) {
         *func = uniform ? (const void *)k_stencil_tma<TJ, DEPTH, true, MINB, EPI_APPLY>
                         : (const void *)k_stencil_tma<TJ, DEPTH, false, MINB, EPI_APPLY>;
-        *smem = sizeof(StencilTmaSmem<TJ, DEPTH, 0>);
+        *smem = uniform ? sizeof(StencilTmaSmem<TJ, DEPTH, 0, true>) : sizeof(StencilTmaSmem<TJ, DEPTH, 0, false>);
+    } else if (epi == EPI_K2R) {
+        *func = uniform ? (const void *)k_stencil_tma<TJ, DEPTH, true, MINB, EPI_K2R>
+                        : (const void *)k_stencil_tma<TJ, DEPTH, false, MINB, EPI_K2R>;
+        *smem = uniform ? sizeof(StencilTmaSmem<TJ, DEPTH, 1, true>) : sizeof(StencilTmaSmem<TJ, DEPTH, 1, false>);
     } else {
         *func = uniform ? (const void *)k_stencil_tma<TJ, DEPTH, true, MINB, EPI_STS>
                         : (const void *)k_stencil_tma<TJ, DEPTH, false, MINB, EPI_STS>;
-        *smem = sizeof(StencilTmaSmem<TJ, DEPTH, 3>);
+        *smem = uniform ? sizeof(StencilTmaSmem<TJ, DEPTH, 3, true>) : sizeof(StencilTmaSmem<TJ, DEPTH, 3, false>);
     }
     *block = dim3((TJ + 2) * 32);
     cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);
 }
 
-// every stencil tile id: 0..5 = k_stencil (cp.async), 6..11 = k_stencil_tma (bulk copies + mbarriers)
-inline int stencil_num_tiles_any() { return stencil_num_tiles() + 6; }
+inline int stencil_num_tiles() { return 6; }
 
-inline void stencil_configure_any(int nr, int nt, int np, int uniform, int epi, int tile, int num_sms, StencilParams *mp,
-                                  const void **func, dim3 *grid, dim3 *block, size_t *smem)
+// tile ids: 0 = TJ 6 (2 blocks/SM), 1 = TJ 8 (2 blocks/SM; default), 2 = TJ 14, 3 = TJ 10, 4 = TJ 8 DEPTH 3, 5 = TJ 12 DEPTH 3
+inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int tile, int num_sms, int ci_force, int ny,
+                              StencilParams *mp, const void **func, dim3 *grid, dim3 *block, size_t *smem)
 {
-    if (tile < stencil_num_tiles() || epi == EPI_K2R) {
-        stencil_configure(nr, nt, np, uniform, epi, tile < stencil_num_tiles() ? tile : 1, num_sms, mp, func, grid, block,
-                          smem);
-        return;
-    }
     int tj;
-    switch (tile - stencil_num_tiles()) {
+    switch (tile) {
         case 0: tj = 6; stencil_tma_pick<6, 2, 2>(uniform, epi, func, block, smem); break;
         case 1: tj = 8; stencil_tma_pick<8, 2, 2>(uniform, epi, func, block, smem); break;
         case 2: tj = 14; stencil_tma_pick<14, 2, 1>(uniform, epi, func, block, smem); break;
@@ -289,7 +280,16 @@ inline void stencil_configure_any(int nr, int nt, int np, int uniform, int epi, 
         case 4: tj = 8; stencil_tma_pick<8, 3, 1>(uniform, epi, func, block, smem); break;
         default: tj = 12; stencil_tma_pick<12, 3, 1>(uniform, epi, func, block, smem); break;
     }
-    stencil_grid(nr, nt, np, epi, tj, num_sms, *func, *block, *smem, mp, grid);
+    mp->t.nkt = (np + TILE_TK - 1) / TILE_TK;
+    mp->t.njt = (nt + tj - 1) / tj;
+    int occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, *func, (int)block->x, *smem) != cudaSuccess || occ < 1) {
+        cudaGetLastError();
+        occ = 1;
+    }
+    mp->t.ci = tile_pick_ci(nr, (long long)mp->t.nkt * mp->t.njt, (long long)num_sms * occ, ny, ci_force);
+    mp->t.nit = (nr + mp->t.ci - 1) / mp->t.ci;
+    *grid = dim3((unsigned)(mp->t.nkt * mp->t.njt * mp->t.nit), (unsigned)ny);
 }
 
 }  // namespace mas

@@ -1,7 +1,7 @@
-// mas_pcg.cu -- C ABI (include/mas_pcg.h) of the B200-native MAS PCG path: handle, coefficient
-// planes, workspaces, the CUDA-graph WHILE loop and its host-chunk fallback.  Every step of the
-// numerical path runs in the kernels of kernels_base.cuh / kernels_march.cuh; this file only
-// marshals.  There is no CPU fallback.
+// mas_pcg.cu -- C ABI (include/mas_pcg.h) of the B200-native MAS PCG path: handle, coefficient planes, workspaces,
+// launch plans, the CUDA-graph WHILE loop and its host-chunk fallback, batched right-hand sides, r-slab groups.
+// Every step of the numerical path runs in the kernels of kernels_*.cuh; this file only marshals.
+// There is no CPU fallback.
 #include "../../include/mas_pcg.h"
 
 #include <cuda_runtime.h>
@@ -9,13 +9,13 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <memory>
 #include <new>
 #include <vector>
 
 #include "common.cuh"
 #include "kernels_base.cuh"
-#include "kernels_march.cuh"
-#include "kernels_stencil.cuh"
+#include "tile.cuh"
 #include "kernels_stencil_tma.cuh"
 #include "kernels_k1_tma.cuh"
 #include "kernels_persistent.cuh"
@@ -26,13 +26,13 @@ namespace {
 
 constexpr int NT_BASE = 256;
 constexpr int HOST_CHUNK = 16;       // iterations per poll in host-chunk mode
+constexpr int CI_FORCE_MIN = 2;      // smallest r-chunk an option may force (bounds the largest grid, see pstride)
 
 struct KLaunch {                     // one kernel launch, usable directly or as a graph node
     const void *func = nullptr;
     dim3 grid{1, 1, 1}, block{1, 1, 1};
     size_t smem = 0;
-    void *args[12] = {};
-    int nargs = 0;
+    void *args[8] = {};
 };
 
 template <typename T>
@@ -53,6 +53,21 @@ struct DevBuf {
     }
 };
 
+struct DeviceGuard {                 // entry points run on the handle's device, whatever the caller's current device is
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; cudaGetLastError(); return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) { ok = false; cudaGetLastError(); }
+        if (prev == dev) prev = -1;
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
 }  // namespace
 
 struct mas_pcg {
@@ -61,40 +76,38 @@ struct mas_pcg {
     int device = 0, num_sms = 0;
     double dt = 0.0;
     int uniform_phi = 0;
-    // device planes
+    // device planes (global mesh)
     DevBuf<double> V2, SD, CP, CRoff, CT, E, F, AR, AT, Dinv, vp, wp, ip, Vinv;
     double lambda_max = 0.0;         // Gershgorin bound on the spectral radius of M = -V^-1 L_sym
     double vp0 = 0, wp0 = 0, ip0 = 0;
-    // workspaces
+    // workspaces for `nrhs_cap` right-hand sides (vectors back to back, stride n)
+    int nrhs_cap = 0;
     DevBuf<double> r, p0, p1, q, partials, hist, bdev, xdev;
+    int pstride = 0;
     DevBuf<State> st;
     DevBuf<SolveArgs> args;
+    DevBuf<Ctl> ctl;
+    DevBuf<unsigned> tickets;
     // pinned staging
     SolveArgs *h_args = nullptr;
-    State *h_st = nullptr;
-    double *h_hist = nullptr;
+    State *h_st = nullptr;           // [MAX_RHS]
+    Ctl *h_ctl = nullptr;
+    double *h_hist = nullptr;        // [MAX_RHS][hist_cap]
     size_t hist_cap = 0;
-    // loop
+    // options
     int loop_mode = 1;               // requested: 1 graph-while, 0 host chunks
-    int loop_mode_used = 1;
-    int variant = 3;                 // K1 variant: 0 baseline, 1 marching tiles (64 wide), 2 wide marching tiles (cp.async),
-                                     // 3 wide marching tiles with TMA bulk copies + mbarriers (default)
-    int tile = 0;                    // tile configuration id of the variant
+    int tile = 0;                    // K1 tile configuration id
     int ci_force = 0;                // >0: override the r-chunk length (tuning)
-    int apply_variant = 1;           // 1: k_stencil marching kernel for A x (apply / initial residual); 0: k_apply
-    int stencil_tile = 7;            // 0..5 cp.async k_stencil, 6..11 TMA k_stencil_tma (7 = TJ 8, 2 blocks/SM: fastest)
-    int k2r_tile = 0;
-    int serpentine = 1;              // 1: K2 sweeps the rows backward (L2 reuse across K1 -> K2 -> K1)
-    int persistent = 2;              // one cooperative kernel for the whole solve: 0 off, 1 whenever it fits, 2 auto
-    int coop_ok = 0;
-    int pdl = 0;                     // programmatic dependent launch edges inside the loop body: measured 5 % SLOWER
-                                     // (early K1 blocks park their shared memory while K2 drains), so off
+    int stencil_tile = 1;            // k_stencil_tma tile for apply / STS
+    int k2r_tile = 1;                // k_stencil_tma tile for K2R
+    int serpentine = 1;              // 1: K2 sweeps backward (L2 reuse across K1 -> K2 -> K1)
+    int persistent = 1;              // 1: one cooperative kernel for the whole solve whenever the state fits on chip
+    int coop_ok = 0, coop_refused = 0;
     int unroll = 4;                  // PCG iterations per WHILE trip of the graph loop (measured: +1 % c4, +3 % c3)
-    int qrecompute = 0;              // 1 (needs xfuse, wide): q is not stored, K2 recomputes it: 64 B/cell/iteration
-    int xfuse = 1;                   // 1: x-update fused into K1 (72 B/cell/iteration), wide variant only
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t exec = nullptr;
-    bool graph_dirty = true;
+    int qrecompute = 1;              // 1: q is not stored, K2R recomputes it: 64 B/cell/iteration; 0: 72 B
+    L2Plan l2{0, 0, 0};
+    cudaGraph_t graph[MAX_RHS] = {};
+    cudaGraphExec_t exec[MAX_RHS] = {};
     long long stats[8] = {};
     OpDev op{};
     Work work{};
@@ -132,18 +145,33 @@ int upload(DevBuf<double> &d, const std::vector<double> &h)
     return MAS_OK;
 }
 
+void drop_graphs(mas_pcg *h)
+{
+    for (int j = 0; j < MAX_RHS; j++) {
+        if (h->exec[j]) cudaGraphExecDestroy(h->exec[j]);
+        if (h->graph[j]) cudaGraphDestroy(h->graph[j]);
+        h->exec[j] = nullptr;
+        h->graph[j] = nullptr;
+    }
+}
+
 void fill_op(mas_pcg *h)
 {
     OpDev &o = h->op;
     o.nr = h->nr; o.nt = h->nt; o.np = h->np; o.nv = h->np / 2;
     o.nrows = h->nr * h->nt;
     o.uniform_phi = h->uniform_phi;
+    o.i_lo = 0; o.nr_glob = h->nr;
     o.n = (long long)h->n;
     o.E = h->E.p; o.F = h->F.p; o.AR = h->AR.p; o.AT = h->AT.p; o.Dinv = h->Dinv.p;
     o.V2 = h->V2.p; o.vp = h->vp.p; o.wp = h->wp.p; o.ip = h->ip.p;
     Work &w = h->work;
+    memset(&w, 0, sizeof(w));
     w.r = h->r.p; w.p0 = h->p0.p; w.p1 = h->p1.p; w.q = h->q.p;
-    w.partials = h->partials.p; w.hist = h->hist.p; w.st = h->st.p; w.args = h->args.p;
+    w.vstride = (long long)h->n;
+    w.partials = h->partials.p; w.pstride = h->pstride;
+    w.hist = h->hist.p; w.hstride = (int)h->hist_cap;
+    w.st = h->st.p; w.tickets = h->tickets.p; w.ctl = h->ctl.p; w.args = h->args.p;
 }
 
 int scale_planes(mas_pcg *h, double dt, cudaStream_t s)
@@ -159,6 +187,34 @@ int scale_planes(mas_pcg *h, double dt, cudaStream_t s)
     return MAS_OK;
 }
 
+// Upper bound on gridDim.x of every reducing kernel any option can select: the marching kernels' smallest tile is
+// 6 theta-rows x 128 phi-cells x CI_FORCE_MIN planes; the row kernels launch at most 32 blocks per SM.
+int partials_stride(const mas_pcg *h)
+{
+    const long long nkt = (h->np + TILE_TK - 1) / TILE_TK, njt = (h->nt + 5) / 6, nit = (h->nr + CI_FORCE_MIN - 1) / CI_FORCE_MIN;
+    long long g = nkt * njt * nit;
+    if (g < 32LL * h->num_sms) g = 32LL * h->num_sms;
+    return (int)g;
+}
+
+// vectors for `nrhs` right-hand sides (grown on the first batched solve)
+int ensure_rhs_capacity(mas_pcg *h, int nrhs)
+{
+    if (nrhs <= h->nrhs_cap) return MAS_OK;
+    drop_graphs(h);
+    const size_t tot = h->n * (size_t)nrhs;
+    if (h->r.alloc(tot) || h->p0.alloc(tot) || h->p1.alloc(tot) || h->q.alloc(tot)) {
+        cudaGetLastError();
+        h->nrhs_cap = 0;
+        return MAS_ENOMEM;
+    }
+    CK(cudaMemset(h->p0.p, 0, tot * sizeof(double)));
+    CK(cudaMemset(h->p1.p, 0, tot * sizeof(double)));
+    h->nrhs_cap = nrhs;
+    fill_op(h);
+    return MAS_OK;
+}
+
 }  // namespace
 
 extern "C" const char *mas_pcg_strerror(int status)
@@ -168,8 +224,8 @@ extern "C" const char *mas_pcg_strerror(int status)
         case MAS_MAXIT: return "iteration cap reached before rtol";
         case MAS_EINVAL: return "invalid argument";
         case MAS_ENOMEM: return "out of memory";
-        case MAS_ECUDA: return "CUDA runtime error (no device, or a launch failed)";
-        case MAS_EBREAKDOWN: return "PCG breakdown: p.Ap <= 0 or non-finite";
+        case MAS_ECUDA: return "CUDA runtime error (no device, a launch failed, or a kernel reported a protocol fault)";
+        case MAS_EBREAKDOWN: return "PCG breakdown: p.Ap <= 0 or a non-finite scalar";
         default: return "unknown status";
     }
 }
@@ -177,23 +233,29 @@ extern "C" const char *mas_pcg_strerror(int status)
 extern "C" void mas_pcg_destroy(mas_pcg_t *h)
 {
     if (!h) return;
-    if (h->exec) cudaGraphExecDestroy(h->exec);
-    if (h->graph) cudaGraphDestroy(h->graph);
+    DeviceGuard dg(h->device);
+    drop_graphs(h);
     DevBuf<double> *bufs[] = {&h->V2, &h->SD, &h->CP, &h->CRoff, &h->CT, &h->E, &h->F, &h->AR, &h->AT, &h->Dinv,
                               &h->vp, &h->wp, &h->ip, &h->Vinv, &h->r, &h->p0, &h->p1, &h->q, &h->partials, &h->hist,
                               &h->bdev, &h->xdev};
     for (DevBuf<double> *b : bufs) b->release();
     h->st.release();
     h->args.release();
+    h->ctl.release();
+    h->tickets.release();
     if (h->h_args) cudaFreeHost(h->h_args);
     if (h->h_st) cudaFreeHost(h->h_st);
+    if (h->h_ctl) cudaFreeHost(h->h_ctl);
     if (h->h_hist) cudaFreeHost(h->h_hist);
     cudaGetLastError();
     delete h;
 }
 
-extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double dt, const mas_nu_t *nu,
-                              const mas_bc_t *bc, mas_pcg_t **out)
+namespace {
+
+// Everything of create except the per-cell workspaces: validation, planes, state, pinned staging.
+int create_operator(const mas_grid_t *g, const mas_metric_t *m, double dt, const mas_nu_t *nu, const mas_bc_t *bc,
+                    mas_pcg **out)
 {
     if (out) *out = nullptr;
     if (!g || !m || !nu || !bc || !out) return MAS_EINVAL;
@@ -230,38 +292,37 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
         cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess)
         return fail(h, MAS_ECUDA);
 
-    // ---- coefficient planes (R1; the paper prints no discrete operator) ----
+    // ---- coefficient planes (R1; the paper prints no discrete operator).  Face by face: the conductance
+    // of a face is formed once from (area / distance) and the face's nu, and enters both adjacent cells. ----
     const int nrows = nr * nt;
-    std::vector<double> V2(nrows), CP(nrows), SD(nrows), CRf((size_t)(nr + 1) * nt), CRoff((size_t)(nr + 1) * nt),
-        CT((size_t)nr * (nt + 1)), vp(np), ip(np), wp(np);
-    for (int i = 0; i < nr; i++)
+    std::vector<double> V2(nrows), CP(nrows), SD(nrows, 0.0), CRoff((size_t)(nr + 1) * nt, 0.0),
+        CT((size_t)nr * (nt + 1), 0.0), vp(np), ip(np), wp(np), Vinv(nrows);
+    for (int t = 0; t < nrows; t++) {
+        const int i = t / nt, j = t - i * nt;
+        const double solid = m->sin_c[j] * m->dth_c[j];                    // sin(theta) dtheta of the row
+        V2[t] = (m->r_c[i] * m->r_c[i]) * m->dr_c[i] * solid;
+        Vinv[t] = 1.0 / V2[t];
+        CP[t] = nu_at(nu, nt, i, j) * (m->dr_c[i] * m->dth_c[j]) / m->sin_c[j];
+    }
+    for (int f = 0; f <= nr; f++) {                                        // radial faces f = 0 .. nr
+        const bool inner = f == 0, outer = f == nr;
+        if ((inner && bc->r_inner == MAS_BC_NEUMANN) || (outer && bc->r_outer == MAS_BC_NEUMANN)) continue;
+        const double geom = (m->r_f[f] * m->r_f[f]) / m->dr_f[f];
         for (int j = 0; j < nt; j++) {
-            const double area_rt = m->sin_c[j] * m->dth_c[j];
-            V2[i * nt + j] = m->r_c[i] * m->r_c[i] * m->dr_c[i] * area_rt;
-            CP[i * nt + j] = nu_at(nu, nt, i, j) * m->dr_c[i] * m->dth_c[j] / m->sin_c[j];
+            const double nu_lo = nu_at(nu, nt, inner ? 0 : f - 1, j), nu_hi = nu_at(nu, nt, outer ? nr - 1 : f, j);
+            const double c = 0.5 * (nu_lo + nu_hi) * geom * (m->sin_c[j] * m->dth_c[j]);
+            if (!inner) SD[(size_t)(f - 1) * nt + j] += c;                 // the cell below the face
+            if (!outer) SD[(size_t)f * nt + j] += c;                       // the cell above it
+            if (!inner && !outer) CRoff[(size_t)f * nt + j] = c;           // a Dirichlet face has no off-diagonal partner
         }
-    for (int i = 0; i <= nr; i++)
-        for (int j = 0; j < nt; j++) {
-            const int il = i > 0 ? i - 1 : 0, ih = i < nr ? i : nr - 1;
-            const double nuf = 0.5 * (nu_at(nu, nt, il, j) + nu_at(nu, nt, ih, j));
-            double c = nuf * (m->r_f[i] * m->r_f[i]) * (m->sin_c[j] * m->dth_c[j]) / m->dr_f[i];
-            const bool boundary = (i == 0 || i == nr);
-            if (i == 0 && bc->r_inner == MAS_BC_NEUMANN) c = 0.0;
-            if (i == nr && bc->r_outer == MAS_BC_NEUMANN) c = 0.0;
-            CRf[(size_t)i * nt + j] = c;                        // enters the diagonal (Dirichlet face)
-            CRoff[(size_t)i * nt + j] = boundary ? 0.0 : c;     // no off-diagonal partner on a boundary
-        }
+    }
     for (int i = 0; i < nr; i++)
-        for (int j = 0; j <= nt; j++) {
-            double c = 0.0;                                     // polar faces: zero area
-            if (j > 0 && j < nt)
-                c = 0.5 * (nu_at(nu, nt, i, j - 1) + nu_at(nu, nt, i, j)) * m->dr_c[i] * m->sin_f[j] / m->dth_f[j];
-            CT[(size_t)i * (nt + 1) + j] = c;
+        for (int f = 1; f < nt; f++) {                                     // theta faces; the polar faces have zero area
+            const double c = 0.5 * (nu_at(nu, nt, i, f - 1) + nu_at(nu, nt, i, f)) * m->dr_c[i] * (m->sin_f[f] / m->dth_f[f]);
+            CT[(size_t)i * (nt + 1) + f] = c;
+            SD[(size_t)i * nt + f - 1] += c;
+            SD[(size_t)i * nt + f] += c;
         }
-    for (int i = 0; i < nr; i++)
-        for (int j = 0; j < nt; j++)
-            SD[i * nt + j] = CRf[(size_t)i * nt + j] + CRf[(size_t)(i + 1) * nt + j] + CT[(size_t)i * (nt + 1) + j] +
-                             CT[(size_t)i * (nt + 1) + j + 1];
     h->uniform_phi = 1;
     for (int k = 0; k < np; k++) {
         vp[k] = m->dph_c[k];
@@ -269,13 +330,9 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
         if (m->dph_c[k] != m->dph_c[0] || m->dph_f[k] != m->dph_f[0]) h->uniform_phi = 0;
     }
     for (int k = 0; k < np; k++) wp[k] = ip[k] + ip[(k + np - 1) % np];
-    std::vector<double> Vinv(nrows);
     double gmax = 0.0;                                      // max_k wp[k]/vp[k]
     for (int k = 0; k < np; k++) gmax = fmax(gmax, wp[k] / vp[k]);
-    for (int t = 0; t < nrows; t++) {
-        Vinv[t] = 1.0 / V2[t];
-        h->lambda_max = fmax(h->lambda_max, 2.0 * (SD[t] + CP[t] * gmax) / V2[t]);
-    }
+    for (int t = 0; t < nrows; t++) h->lambda_max = fmax(h->lambda_max, 2.0 * (SD[t] + CP[t] * gmax) / V2[t]);
     h->vp0 = vp[0];
     h->wp0 = wp[0];
     h->ip0 = ip[0];
@@ -285,21 +342,22 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
         (rc = upload(h->CRoff, CRoff)) || (rc = upload(h->CT, CT)) || (rc = upload(h->vp, vp)) ||
         (rc = upload(h->wp, wp)) || (rc = upload(h->ip, ip)) || (rc = upload(h->Vinv, Vinv)))
         return fail(h, rc);
+    h->pstride = partials_stride(h);
     if (h->E.alloc(nrows) || h->F.alloc(nrows) || h->Dinv.alloc(nrows) || h->AR.alloc((size_t)(nr + 1) * nt) ||
-        h->AT.alloc((size_t)nr * (nt + 1)) || h->r.alloc(h->n) || h->p0.alloc(h->n) || h->p1.alloc(h->n) ||
-        h->q.alloc(h->n) || h->partials.alloc(8 * (size_t)MAX_PARTIALS) || h->st.alloc(1) || h->args.alloc(1)) {
+        h->AT.alloc((size_t)nr * (nt + 1)) || h->partials.alloc((size_t)MAX_RHS * PART_REGIONS * h->pstride) ||
+        h->st.alloc(MAX_RHS) || h->args.alloc(1) || h->ctl.alloc(1) || h->tickets.alloc(MAX_RHS * 4)) {
         cudaGetLastError();
         return fail(h, MAS_ENOMEM);
     }
     h->hist_cap = 1 << 13;
-    if (h->hist.alloc(h->hist_cap) != cudaSuccess) return fail(h, MAS_ENOMEM);
+    if (h->hist.alloc(MAX_RHS * h->hist_cap) != cudaSuccess) return fail(h, MAS_ENOMEM);
     if (cudaMallocHost((void **)&h->h_args, sizeof(SolveArgs)) != cudaSuccess ||
-        cudaMallocHost((void **)&h->h_st, sizeof(State)) != cudaSuccess ||
-        cudaMallocHost((void **)&h->h_hist, h->hist_cap * sizeof(double)) != cudaSuccess)
+        cudaMallocHost((void **)&h->h_st, MAX_RHS * sizeof(State)) != cudaSuccess ||
+        cudaMallocHost((void **)&h->h_ctl, sizeof(Ctl)) != cudaSuccess ||
+        cudaMallocHost((void **)&h->h_hist, MAX_RHS * h->hist_cap * sizeof(double)) != cudaSuccess)
         return fail(h, MAS_ENOMEM);
-    if (cudaMemset(h->st.p, 0, sizeof(State)) != cudaSuccess) return fail(h, MAS_ECUDA);
-    if (cudaMemset(h->p0.p, 0, h->n * sizeof(double)) != cudaSuccess ||
-        cudaMemset(h->p1.p, 0, h->n * sizeof(double)) != cudaSuccess)
+    if (cudaMemset(h->st.p, 0, MAX_RHS * sizeof(State)) != cudaSuccess || cudaMemset(h->ctl.p, 0, sizeof(Ctl)) != cudaSuccess ||
+        cudaMemset(h->tickets.p, 0, MAX_RHS * 4 * sizeof(unsigned)) != cudaSuccess)
         return fail(h, MAS_ECUDA);
     fill_op(h);
     if (cudaDeviceGetAttribute(&h->coop_ok, cudaDevAttrCooperativeLaunch, h->device) != cudaSuccess) h->coop_ok = 0;
@@ -309,31 +367,43 @@ extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double
     return MAS_OK;
 }
 
+}  // namespace
+
+extern "C" int mas_pcg_create(const mas_grid_t *g, const mas_metric_t *m, double dt, const mas_nu_t *nu,
+                              const mas_bc_t *bc, mas_pcg_t **out)
+{
+    mas_pcg *h = nullptr;
+    int rc = create_operator(g, m, dt, nu, bc, &h);
+    if (rc != MAS_OK) return rc;
+    if ((rc = ensure_rhs_capacity(h, 1)) != MAS_OK) return fail(h, rc);
+    if (cudaDeviceSynchronize() != cudaSuccess) return fail(h, MAS_ECUDA);
+    *out = h;
+    return MAS_OK;
+}
+
 // =============================================================================================
-// launch descriptions
+// launch plans
 // =============================================================================================
 namespace {
 
-struct LoopCtx {                     // storage that kernel argument pointers refer to
+// One "part" = what a set of launches works on: the whole mesh, or one r-slab of a slab group.
+struct Plan {                        // storage that kernel argument pointers refer to + the launches
     OpDev op;
     Work work;
     cudaGraphConditionalHandle cond;
     int use_cond;
     int reverse;
-    const double *xin;
-    const SolveArgs *args;
-    double *y;
-    MarchParams mp;
-    WideParams wp;
-    StencilParams sp, sp2;
+    TileParams k1p;
+    StencilParams sp_apply, sp_k2;
+    KLaunch apply, init, k1, k2, xtail;
+    int max_grid = 0;
 };
 
-int base_grid(const mas_pcg *h, const void *func, int nt_block)
+int base_grid(const mas_pcg *h, const OpDev &op, const void *func, int nt_block)
 {
-    const int nv = h->np / 2;
-    const int nvc = nv < nt_block ? nv : nt_block;
+    const int nvc = op.nv < nt_block ? op.nv : nt_block;
     const int rb = nt_block / nvc;
-    const long long groups = ((long long)h->nr * h->nt + rb - 1) / rb;
+    const long long groups = ((long long)op.nrows + rb - 1) / rb;
     int occ = 1;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, func, nt_block, 0) != cudaSuccess || occ < 1) {
         cudaGetLastError();
@@ -341,124 +411,72 @@ int base_grid(const mas_pcg *h, const void *func, int nt_block)
     }
     long long gsz = (long long)h->num_sms * occ;
     if (gsz > groups) gsz = groups;
-    if (gsz > MAX_PARTIALS) gsz = MAX_PARTIALS;
     if (gsz < 1) gsz = 1;
     return (int)gsz;
 }
 
-bool use_xfuse(const mas_pcg *h) { return (h->xfuse && h->variant == 2) || h->variant == 3; }   // k1_tma is always xfuse
-bool use_qrec(const mas_pcg *h) { return h->qrecompute && h->xfuse && h->variant == 2; }
-
 void stencil_common(const mas_pcg *h, StencilParams &sp)
 {
     memset(&sp, 0, sizeof(sp));
-    sp.vp = h->vp0; sp.wp = h->wp0; sp.ip = h->ip0;
+    sp.t.vp = h->vp0; sp.t.wp = h->wp0; sp.t.ip = h->ip0;
     sp.args = h->args.p;
+    sp.fault = &h->ctl.p->fault;
 }
 
-KLaunch make_apply(const mas_pcg *h, LoopCtx &c)
+// Fill a plan for (operator part, work set, right-hand sides).  use_cond: the kernels set the graph conditional.
+int make_plan(const mas_pcg *h, const OpDev &op, const Work &work, int nrhs, int use_cond,
+              cudaGraphConditionalHandle cond, Plan &c)
 {
-    KLaunch k;
-    if (h->apply_variant == 1) {                 // marching stencil kernel: S = A_sym (dt-scaled planes)
-        stencil_common(h, c.sp);
-        c.sp.E = h->E.p; c.sp.F = h->F.p; c.sp.AR = h->AR.p; c.sp.AT = h->AT.p;
-        c.sp.u = c.xin; c.sp.out = c.y;
-        stencil_configure_any(h->nr, h->nt, h->np, h->uniform_phi, EPI_APPLY, h->stencil_tile, h->num_sms, &c.sp,
-                              &k.func, &k.grid, &k.block, &k.smem);
-        k.args[0] = &c.op; k.args[1] = &c.sp;
-        k.nargs = 2;
-        return k;
-    }
-    k.func = (const void *)k_apply<NT_BASE>;
-    k.block = dim3(NT_BASE);
-    k.grid = dim3(base_grid(h, k.func, NT_BASE));
-    k.args[0] = &c.op; k.args[1] = &c.xin; k.args[2] = &c.args; k.args[3] = &c.y;
-    k.nargs = 4;
-    return k;
-}
-
-KLaunch make_init(const mas_pcg *h, LoopCtx &c)
-{
-    KLaunch k;
-    k.func = h->uniform_phi ? (const void *)k_init<NT_BASE, true> : (const void *)k_init<NT_BASE, false>;
-    k.block = dim3(NT_BASE);
-    k.grid = dim3(base_grid(h, k.func, NT_BASE));
-    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
-    k.nargs = 4;
-    return k;
-}
-
-KLaunch make_k2(const mas_pcg *h, LoopCtx &c)
-{
-    KLaunch k;
-    if (use_qrec(h)) {                           // marching stencil kernel: q = A p recomputed, r updated in place
-        stencil_common(h, c.sp2);
-        c.sp2.E = h->E.p; c.sp2.F = h->F.p; c.sp2.AR = h->AR.p; c.sp2.AT = h->AT.p; c.sp2.Dinv = h->Dinv.p;
-        c.sp2.w = c.work; c.sp2.cond = c.cond; c.sp2.use_cond = c.use_cond;
-        stencil_configure(h->nr, h->nt, h->np, h->uniform_phi, EPI_K2R, h->k2r_tile, h->num_sms, &c.sp2, &k.func,
-                          &k.grid, &k.block, &k.smem);
-        k.args[0] = &c.op; k.args[1] = &c.sp2;
-        k.nargs = 2;
-        return k;
-    }
-    const bool xf = use_xfuse(h);
-    if (xf)
-        k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true, true> : (const void *)k2_vec<NT_BASE, false, true>;
-    else
-        k.func = h->uniform_phi ? (const void *)k2_vec<NT_BASE, true, false> : (const void *)k2_vec<NT_BASE, false, false>;
-    k.block = dim3(NT_BASE);
-    k.grid = dim3(base_grid(h, k.func, NT_BASE));
-    c.reverse = h->serpentine;
-    k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond; k.args[4] = &c.reverse;
-    k.nargs = 5;
-    return k;
-}
-
-KLaunch make_xtail(const mas_pcg *h, LoopCtx &c)
-{
-    KLaunch k;
-    k.func = (const void *)k_xtail<NT_BASE>;
-    k.block = dim3(NT_BASE);
-    k.grid = dim3(base_grid(h, k.func, NT_BASE));
-    k.args[0] = &c.op; k.args[1] = &c.work;
-    k.nargs = 2;
-    return k;
-}
-
-
-
-KLaunch make_k1(const mas_pcg *h, LoopCtx &c)
-{
-    KLaunch k;
-    if (h->variant == 0) {
-        k.func = h->uniform_phi ? (const void *)k1_v0<NT_BASE, true> : (const void *)k1_v0<NT_BASE, false>;
-        k.block = dim3(NT_BASE);
-        k.grid = dim3(base_grid(h, k.func, NT_BASE));
-        k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.cond; k.args[3] = &c.use_cond;
-        k.nargs = 4;
-        return k;
-    }
-    if (h->variant == 3) {
-        k1_tma_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, h->ci_force, &c.wp, &k.func, &k.grid,
-                         &k.block, &k.smem);
-        c.wp.vp = h->vp0; c.wp.wp = h->wp0; c.wp.ip = h->ip0;
-        k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.wp; k.args[3] = &c.cond; k.args[4] = &c.use_cond;
-        k.nargs = 5;
-        return k;
-    }
-    if (h->variant == 1) {
-        march_configure(h->nr, h->nt, h->np, h->uniform_phi, h->tile, h->num_sms, &c.mp, &k.func, &k.grid, &k.block,
-                        &k.smem);
-        k.args[2] = &c.mp;
+    c.op = op; c.work = work; c.cond = cond; c.use_cond = use_cond; c.reverse = h->serpentine;
+    const bool uni = h->uniform_phi;
+    // A x0 -> q (initial residual)
+    stencil_common(h, c.sp_apply);
+    c.sp_apply.ps = PlaneSetDev{h->E.p, h->F.p, h->AR.p, h->AT.p, nullptr};
+    c.sp_apply.u = nullptr; c.sp_apply.out = work.q; c.sp_apply.ustride = work.vstride;
+    c.sp_apply.args = work.args;
+    stencil_configure(op.nr, op.nt, op.np, uni, EPI_APPLY, h->stencil_tile, h->num_sms, h->ci_force, nrhs, &c.sp_apply,
+                      &c.apply.func, &c.apply.grid, &c.apply.block, &c.apply.smem);
+    c.apply.args[0] = &c.op; c.apply.args[1] = &c.sp_apply;
+    // init
+    c.init.func = uni ? (const void *)k_init<NT_BASE, true> : (const void *)k_init<NT_BASE, false>;
+    c.init.block = dim3(NT_BASE);
+    c.init.grid = dim3(base_grid(h, op, c.init.func, NT_BASE), nrhs);
+    c.init.args[0] = &c.op; c.init.args[1] = &c.work; c.init.args[2] = &c.cond; c.init.args[3] = &c.use_cond;
+    // K1
+    memset(&c.k1p, 0, sizeof(c.k1p));
+    k1_tma_configure(op.nr, op.nt, op.np, uni, h->qrecompute != 0, h->tile, h->num_sms, h->ci_force, nrhs, &c.k1p,
+                     &c.k1.func, &c.k1.grid, &c.k1.block, &c.k1.smem);
+    c.k1p.vp = h->vp0; c.k1p.wp = h->wp0; c.k1p.ip = h->ip0;
+    c.k1p.l2 = h->l2;
+    c.k1.args[0] = &c.op; c.k1.args[1] = &c.work; c.k1.args[2] = &c.k1p; c.k1.args[3] = &c.cond; c.k1.args[4] = &c.use_cond;
+    // K2 (q stored) or K2R (q recomputed)
+    if (h->qrecompute) {
+        stencil_common(h, c.sp_k2);
+        c.sp_k2.ps = PlaneSetDev{h->E.p, h->F.p, h->AR.p, h->AT.p, h->Dinv.p};
+        c.sp_k2.w = work; c.sp_k2.cond = cond; c.sp_k2.use_cond = use_cond;
+        c.sp_k2.args = work.args;
+        stencil_configure(op.nr, op.nt, op.np, uni, EPI_K2R, h->k2r_tile, h->num_sms, h->ci_force, nrhs, &c.sp_k2,
+                          &c.k2.func, &c.k2.grid, &c.k2.block, &c.k2.smem);
+        c.sp_k2.t.reverse = h->serpentine;
+        c.sp_k2.t.l2 = h->l2;
+        c.k2.args[0] = &c.op; c.k2.args[1] = &c.sp_k2;
     } else {
-        wide_configure(h->nr, h->nt, h->np, h->uniform_phi, use_qrec(h) ? 2 : (use_xfuse(h) ? 1 : 0), h->tile, h->num_sms, h->ci_force, &c.wp,
-                       &k.func, &k.grid, &k.block, &k.smem);
-        c.wp.vp = h->vp0; c.wp.wp = h->wp0; c.wp.ip = h->ip0;
-        k.args[2] = &c.wp;
+        c.k2.func = uni ? (const void *)k2_vec<NT_BASE, true> : (const void *)k2_vec<NT_BASE, false>;
+        c.k2.block = dim3(NT_BASE);
+        c.k2.grid = dim3(base_grid(h, op, c.k2.func, NT_BASE), nrhs);
+        c.k2.smem = 0;
+        c.k2.args[0] = &c.op; c.k2.args[1] = &c.work; c.k2.args[2] = &c.cond; c.k2.args[3] = &c.use_cond;
+        c.k2.args[4] = &c.reverse;
     }
-    k.args[0] = &c.op; k.args[1] = &c.work; k.args[3] = &c.cond; k.args[4] = &c.use_cond;
-    k.nargs = 5;
-    return k;
+    // x tail
+    c.xtail.func = (const void *)k_xtail<NT_BASE>;
+    c.xtail.block = dim3(NT_BASE);
+    c.xtail.grid = dim3(base_grid(h, op, c.xtail.func, NT_BASE), nrhs);
+    c.xtail.args[0] = &c.op; c.xtail.args[1] = &c.work;
+    c.max_grid = (int)c.init.grid.x;
+    if ((int)c.k1.grid.x > c.max_grid) c.max_grid = (int)c.k1.grid.x;
+    if ((int)c.k2.grid.x > c.max_grid) c.max_grid = (int)c.k2.grid.x;
+    return c.max_grid <= work.pstride ? MAS_OK : MAS_EINVAL;     // the invariant grid_sum relies on
 }
 
 cudaError_t launch(const KLaunch &k, cudaStream_t s)
@@ -479,77 +497,62 @@ cudaError_t add_node(cudaGraphNode_t *node, cudaGraph_t g, const cudaGraphNode_t
     return cudaGraphAddKernelNode(node, g, dep, dep ? 1 : 0, &p);
 }
 
-void drop_graph(mas_pcg *h)
-{
-    if (h->exec) cudaGraphExecDestroy(h->exec);
-    if (h->graph) cudaGraphDestroy(h->graph);
-    h->exec = nullptr;
-    h->graph = nullptr;
-    h->graph_dirty = true;
-}
+// A solve as three kernel sequences: before the loop, the loop body (one PCG iteration), after the loop.
+struct Seq {
+    std::vector<KLaunch> pre, body, post;
+};
 
-// graph = [A x0 -> q] -> [init] -> WHILE(cond){ K1 -> K2 }   (call stack 2)
-int build_graph(mas_pcg *h)
+// graph = pre... -> WHILE(cond){ body x unroll } -> post...   (call stack 2)
+// `unroll` iterations per WHILE trip: the conditional node is evaluated once per trip, and the kernels return
+// at once when the loop has ended (device flags), so extra copies after convergence cost empty launches.
+int build_graph(const Seq &seq, cudaGraph_t g, cudaGraphConditionalHandle cond, int unroll, cudaGraphExec_t *exec)
 {
-    drop_graph(h);
-    LoopCtx c;
-    c.op = h->op; c.work = h->work; c.use_cond = 1; c.xin = nullptr; c.args = h->args.p; c.y = h->q.p;
-    cudaGraph_t g = nullptr;
-    if (cudaGraphCreate(&g, 0) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
-    h->graph = g;
-    if (cudaGraphConditionalHandleCreate(&c.cond, g, 1, cudaGraphCondAssignDefault) != cudaSuccess) {
-        cudaGetLastError();
-        return MAS_ECUDA;
-    }
-    cudaGraphNode_t n_apply, n_init, n_while, n_k1, n_k2;
-    const KLaunch ka = make_apply(h, c), ki = make_init(h, c);
-    if (add_node(&n_apply, g, nullptr, ka) != cudaSuccess || add_node(&n_init, g, &n_apply, ki) != cudaSuccess) {
-        cudaGetLastError();
-        return MAS_ECUDA;
-    }
-    cudaGraphNodeParams wp = {cudaGraphNodeTypeConditional};
-    wp.conditional.handle = c.cond;
-    wp.conditional.type = cudaGraphCondTypeWhile;
-    wp.conditional.size = 1;
-    if (cudaGraphAddNode(&n_while, g, &n_init, 1, &wp) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
-    cudaGraph_t body = wp.conditional.phGraph_out[0];
-    const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
-    // `unroll` iterations per WHILE trip: the conditional node is evaluated once per trip, and K1 / K2 return
-    // at once when the loop has ended (device flag), so extra pairs after convergence cost two empty launches.
-    // Edges inside the body are programmatic (PDL) when both kernels wait with cudaGridDependencySynchronize
-    // (k1_wide and k2_vec): the successor's blocks launch while the predecessor drains and run the part of
-    // their prologue that does not depend on it.
-    const bool pdl = h->pdl && h->variant >= 2 && !use_qrec(h);
-    cudaGraphNode_t prev = nullptr;
-    for (int u = 0; u < 2 * h->unroll; u++) {
-        cudaGraphNode_t node;
-        if (add_node(&node, body, nullptr, (u & 1) ? k2 : k1) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
-        if (prev) {
-            cudaGraphEdgeData ed;
-            memset(&ed, 0, sizeof(ed));
-            if (pdl) {
-                ed.type = cudaGraphDependencyTypeProgrammatic;
-                ed.from_port = cudaGraphKernelNodePortProgrammatic;
-            }
-            if (cudaGraphAddDependencies_v2(body, &prev, &node, &ed, 1) != cudaSuccess) {
-                cudaGetLastError();
-                return MAS_ECUDA;
-            }
-        }
+    cudaGraphNode_t prev = nullptr, node;
+    for (const KLaunch &k : seq.pre) {
+        if (add_node(&node, g, prev ? &prev : nullptr, k) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
         prev = node;
     }
-    (void)n_k1; (void)n_k2;
-    if (use_xfuse(h)) {
-        cudaGraphNode_t n_tail;
-        const KLaunch kt = make_xtail(h, c);
-        if (add_node(&n_tail, g, &n_while, kt) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+    cudaGraphNodeParams wp = {cudaGraphNodeTypeConditional};
+    wp.conditional.handle = cond;
+    wp.conditional.type = cudaGraphCondTypeWhile;
+    wp.conditional.size = 1;
+    cudaGraphNode_t n_while;
+    if (cudaGraphAddNode(&n_while, g, prev ? &prev : nullptr, prev ? 1 : 0, &wp) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+    cudaGraph_t body = wp.conditional.phGraph_out[0];
+    cudaGraphNode_t bprev = nullptr;
+    for (int u = 0; u < unroll; u++)
+        for (const KLaunch &k : seq.body) {
+            if (add_node(&node, body, bprev ? &bprev : nullptr, k) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+            bprev = node;
+        }
+    prev = n_while;
+    for (const KLaunch &k : seq.post) {
+        if (add_node(&node, g, &prev, k) != cudaSuccess) { cudaGetLastError(); return MAS_ECUDA; }
+        prev = node;
     }
-    if (cudaGraphInstantiate(&h->exec, g, 0) != cudaSuccess) {
+    if (cudaGraphInstantiate(exec, g, 0) != cudaSuccess) {
         cudaGetLastError();
-        h->exec = nullptr;
+        *exec = nullptr;
         return MAS_ECUDA;
     }
-    h->graph_dirty = false;
+    return MAS_OK;
+}
+
+// host-driven loop over the same sequences: chunks of HOST_CHUNK iterations, then a poll of the loop flag
+int run_host_loop(const Seq &seq, const Ctl *d_ctl, Ctl *h_ctl, int maxit, cudaStream_t s, long long *launched_loop)
+{
+    for (const KLaunch &k : seq.pre) CK(launch(k, s));
+    for (int done = 0; done < maxit;) {
+        CK(cudaMemcpyAsync(h_ctl, d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
+        CK(cudaStreamSynchronize(s));
+        if (!h_ctl->loop) break;
+        const int chunk = maxit - done < HOST_CHUNK ? maxit - done : HOST_CHUNK;
+        for (int it = 0; it < chunk; it++)
+            for (const KLaunch &k : seq.body) CK(launch(k, s));
+        *launched_loop += (long long)seq.body.size() * chunk;
+        done += chunk;
+    }
+    for (const KLaunch &k : seq.post) CK(launch(k, s));
     return MAS_OK;
 }
 
@@ -559,26 +562,22 @@ int ensure_hist(mas_pcg *h, int maxit)
     if (need <= h->hist_cap) return MAS_OK;
     size_t cap = h->hist_cap;
     while (cap < need) cap *= 2;
-    if (h->hist.alloc(cap) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    if (h->hist.alloc(MAX_RHS * cap) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
     if (h->h_hist) cudaFreeHost(h->h_hist);
     h->h_hist = nullptr;
-    if (cudaMallocHost((void **)&h->h_hist, cap * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    if (cudaMallocHost((void **)&h->h_hist, MAX_RHS * cap * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
     h->hist_cap = cap;
     fill_op(h);
-    drop_graph(h);              // kernel nodes hold the old hist pointer
+    drop_graphs(h);             // kernel nodes hold the old hist pointer
     return MAS_OK;
 }
 
 bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
 
-constexpr long long PERSIST_AUTO_CELLS = 1LL << 40;   // auto mode: measured faster wherever the state fits on chip
-                                                      // (config 1: 2.0x, config 2 = 786 k cells: 1.46x)
-
 // Plan the one-kernel solve; returns false when it does not apply (too large, no cooperative launch, off).
 bool plan_persistent(const mas_pcg *h, PersistParams *pp, int *grid, size_t *smem, const void **func)
 {
     if (!h->persistent || !h->coop_ok) return false;
-    if (h->persistent == 2 && (long long)h->n > PERSIST_AUTO_CELLS) return false;
     const long long nvec = (long long)h->n / 2;
     long long g = (nvec + PNT - 1) / PNT;
     if (g > h->num_sms) g = h->num_sms;
@@ -596,10 +595,128 @@ bool plan_persistent(const mas_pcg *h, PersistParams *pp, int *grid, size_t *sme
         return false;
     }
     pp->Z = h->r.p; pp->P0 = h->p0.p; pp->P1 = h->p1.p;
-    pp->partials = h->partials.p; pp->hist = h->hist.p; pp->st = h->st.p; pp->args = h->args.p;
+    pp->partials = h->partials.p; pp->pstride = h->pstride;
+    pp->hist = h->hist.p; pp->st = h->st.p; pp->args = h->args.p;
     pp->nvec = (int)nvec; pp->M = (int)M;
     *grid = (int)g;
     return true;
+}
+
+void set_traffic_stats(mas_pcg *h)
+{
+    // qrecompute: K1 r,p,x -> p,x (5N); K2R p,r -> r (3N).  otherwise: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)
+    h->stats[4] = h->qrecompute ? 5 : 6;
+    h->stats[5] = 3;
+    h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
+}
+
+int worst_status(int a, int b)
+{
+    if (a < 0 || b < 0) return a < b ? a : b;
+    return a > b ? a : b;
+}
+
+void seq_for_plan(const Plan &c, Seq &seq)
+{
+    seq.pre = {c.apply, c.init};
+    seq.body = {c.k1, c.k2};
+    seq.post = {c.xtail};
+}
+
+// The common solve: nrhs right-hand sides sharing the operator, each an independent PCG (own alpha, beta, count,
+// status, history), run by ONE set of launches whose grid.y is the right-hand side.
+int solve_core(mas_pcg *h, int nrhs, const double *const *b_dev, double *const *x_dev, double rtol, int maxit,
+               cudaStream_t s, int *iters_out, int *status_out, double *reshist_host)
+{
+    int rc = ensure_hist(h, maxit);
+    if (rc != MAS_OK) return rc;
+    if ((rc = ensure_rhs_capacity(h, nrhs)) != MAS_OK) return rc;
+    memset(h->h_args, 0, sizeof(SolveArgs));
+    for (int j = 0; j < nrhs; j++) { h->h_args->b[j] = b_dev[j]; h->h_args->x[j] = x_dev[j]; }
+    h->h_args->rtol = rtol; h->h_args->maxit = maxit; h->h_args->nrhs = nrhs;
+    CK(cudaMemcpyAsync(h->args.p, h->h_args, sizeof(SolveArgs), cudaMemcpyHostToDevice, s));
+
+    int mode = h->loop_mode;
+    PersistParams ppar;
+    int pgrid = 0;
+    size_t psmem = 0;
+    const void *pfunc = nullptr;
+    long long launched_outside = 0, launched_loop = 0;
+    if (nrhs == 1 && !h->coop_refused && plan_persistent(h, &ppar, &pgrid, &psmem, &pfunc)) {
+        OpDev op = h->op;                      // init + loop + finish in one cooperative kernel
+        void *kargs[2] = {&op, &ppar};
+        if (cudaLaunchCooperativeKernel(pfunc, dim3(pgrid), dim3(PNT), kargs, psmem, s) == cudaSuccess) {
+            mode = 2;
+            launched_loop = 1;
+        } else {
+            cudaGetLastError();                // refused (e.g. co-residency limits): use the streaming loop from now on
+            h->coop_refused = 1;
+        }
+    }
+    if (mode != 2) {
+        std::unique_ptr<Plan> plan(new (std::nothrow) Plan());
+        if (!plan) return MAS_ENOMEM;
+        Seq seq;
+        if (mode == 1 && !h->exec[nrhs - 1]) {
+            cudaGraph_t g = nullptr;
+            cudaGraphConditionalHandle cond;
+            bool ok = cudaGraphCreate(&g, 0) == cudaSuccess;
+            if (ok) h->graph[nrhs - 1] = g;
+            ok = ok && cudaGraphConditionalHandleCreate(&cond, g, 1, cudaGraphCondAssignDefault) == cudaSuccess;
+            if (ok) {
+                if ((rc = make_plan(h, h->op, h->work, nrhs, 1, cond, *plan)) != MAS_OK) return rc;
+                seq_for_plan(*plan, seq);
+                ok = build_graph(seq, g, cond, h->unroll, &h->exec[nrhs - 1]) == MAS_OK;
+            }
+            if (!ok) {                         // driver without conditional nodes: fall back, and say so in stats
+                cudaGetLastError();
+                drop_graphs(h);
+                mode = 0;
+            }
+        }
+        if (mode == 1) {
+            CK(cudaGraphLaunch(h->exec[nrhs - 1], s));
+        } else {
+            cudaGraphConditionalHandle none;
+            memset(&none, 0, sizeof(none));
+            if ((rc = make_plan(h, h->op, h->work, nrhs, 0, none, *plan)) != MAS_OK) return rc;
+            seq.pre.clear(); seq.body.clear(); seq.post.clear();
+            seq_for_plan(*plan, seq);
+            if ((rc = run_host_loop(seq, h->ctl.p, h->h_ctl, maxit, s, &launched_loop)) != MAS_OK) return rc;
+        }
+        launched_outside = 3;
+    }
+    CK(cudaMemcpyAsync(h->h_st, h->st.p, MAX_RHS * sizeof(State), cudaMemcpyDeviceToHost, s));
+    CK(cudaMemcpyAsync(h->h_ctl, h->ctl.p, sizeof(Ctl), cudaMemcpyDeviceToHost, s));
+    for (int j = 0; j < nrhs; j++)
+        CK(cudaMemcpyAsync(h->h_hist + (size_t)j * h->hist_cap, h->hist.p + (size_t)j * h->hist_cap,
+                           ((size_t)maxit + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));          // the one host sync of a graph-mode solve
+    if (h->h_ctl->fault) {                 // a kernel gave up on an mbarrier wait: the result is not trustworthy
+        cudaMemsetAsync(&h->ctl.p->fault, 0, sizeof(int), s);
+        return MAS_ECUDA;
+    }
+    int worst = MAS_OK;
+    long long graph_launches = 0;
+    for (int j = 0; j < nrhs; j++) {
+        const State &st = h->h_st[j];
+        if (st.bb == 0.0) CK(cudaMemsetAsync(x_dev[j], 0, h->n * sizeof(double), s));   // zero right-hand side: x = 0
+        if (iters_out) iters_out[j] = st.k;
+        if (status_out) status_out[j] = st.status;
+        if (reshist_host)
+            memcpy(reshist_host + (size_t)j * ((size_t)maxit + 1), h->h_hist + (size_t)j * h->hist_cap,
+                   ((size_t)st.k + 1) * sizeof(double));
+        worst = worst_status(worst, st.status);
+        if (st.launches > graph_launches) graph_launches = st.launches;
+    }
+    CK(cudaStreamSynchronize(s));
+    h->stats[0] = mode == 1 ? graph_launches : launched_loop;
+    h->stats[1] = launched_outside;
+    h->stats[2] = mode;
+    h->stats[6] = mode == 2 ? pgrid : 0;
+    h->stats[7] = h->coop_refused;
+    set_traffic_stats(h);
+    return worst;
 }
 
 }  // namespace
@@ -607,66 +724,74 @@ bool plan_persistent(const mas_pcg *h, PersistParams *pp, int *grid, size_t *sme
 extern "C" int mas_pcg_set_dt(mas_pcg_t *h, double dt, void *stream)
 {
     if (!h || !(dt >= 0.0) || !isfinite(dt)) return MAS_EINVAL;
+    DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
     return scale_planes(h, dt, (cudaStream_t)stream);
 }
 
 extern "C" int mas_pcg_apply(mas_pcg_t *h, const double *x_dev, double *y_dev, void *stream)
 {
     if (!h || !x_dev || !y_dev || x_dev == y_dev || !aligned16(x_dev) || !aligned16(y_dev)) return MAS_EINVAL;
-    LoopCtx c;
-    c.op = h->op; c.xin = x_dev; c.args = h->args.p; c.y = y_dev;
-    CK(launch(make_apply(h, c), (cudaStream_t)stream));
+    DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
+    StencilParams sp;
+    stencil_common(h, sp);
+    sp.ps = PlaneSetDev{h->E.p, h->F.p, h->AR.p, h->AT.p, nullptr};
+    sp.u = x_dev; sp.out = y_dev;
+    KLaunch k;
+    OpDev op = h->op;
+    stencil_configure(h->nr, h->nt, h->np, h->uniform_phi, EPI_APPLY, h->stencil_tile, h->num_sms, h->ci_force, 1, &sp,
+                      &k.func, &k.grid, &k.block, &k.smem);
+    k.args[0] = &op; k.args[1] = &sp;
+    CK(launch(k, (cudaStream_t)stream));
     return MAS_OK;
 }
 
 extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
 {
     if (!h || !name) return MAS_EINVAL;
+    DeviceGuard dg(h->device);
     if (!strcmp(name, "loop_mode")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->loop_mode = value;
-    } else if (!strcmp(name, "variant")) {
-        if (value < 0 || value > 3) return MAS_EINVAL;
-        h->variant = value;
-        h->tile = 0;
     } else if (!strcmp(name, "tile")) {
-        const int nt_ = h->variant == 1 ? march_num_tiles() : (h->variant == 2 ? wide_num_tiles() : (h->variant == 3 ? k1_tma_num_tiles() : 1));
-        if (value < 0 || value >= nt_) return MAS_EINVAL;
+        if (value < 0 || value >= k1_tma_num_tiles()) return MAS_EINVAL;
         h->tile = value;
-    } else if (!strcmp(name, "apply_variant")) {
-        if (value != 0 && value != 1) return MAS_EINVAL;
-        h->apply_variant = value;
     } else if (!strcmp(name, "stencil_tile")) {
-        if (value < 0 || value >= stencil_num_tiles_any()) return MAS_EINVAL;
+        if (value < 0 || value >= stencil_num_tiles()) return MAS_EINVAL;
         h->stencil_tile = value;
+    } else if (!strcmp(name, "k2r_tile")) {
+        if (value < 0 || value >= stencil_num_tiles()) return MAS_EINVAL;
+        h->k2r_tile = value;
     } else if (!strcmp(name, "serpentine")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->serpentine = value;
-    } else if (!strcmp(name, "pdl")) {
-        if (value != 0 && value != 1) return MAS_EINVAL;
-        h->pdl = value;
     } else if (!strcmp(name, "unroll")) {
         if (value < 1 || value > 16) return MAS_EINVAL;
         h->unroll = value;
     } else if (!strcmp(name, "persistent")) {
-        if (value < 0 || value > 2) return MAS_EINVAL;
+        if (value != 0 && value != 1) return MAS_EINVAL;
         h->persistent = value;
+        h->coop_refused = 0;
     } else if (!strcmp(name, "qrecompute")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->qrecompute = value;
-    } else if (!strcmp(name, "k2r_tile")) {
-        if (value < 0 || value >= stencil_num_tiles()) return MAS_EINVAL;
-        h->k2r_tile = value;
-    } else if (!strcmp(name, "xfuse")) {
-        if (value != 0 && value != 1) return MAS_EINVAL;
-        h->xfuse = value;
     } else if (!strcmp(name, "ci")) {
-        if (value < 0 || value > MARCH_CI_MAX) return MAS_EINVAL;
+        if (value != 0 && (value < CI_FORCE_MIN || value > TILE_CI_MAX)) return MAS_EINVAL;
         h->ci_force = value;
+    } else if (!strcmp(name, "l2_keep_r")) {
+        if (value < 0) return MAS_EINVAL;
+        h->l2.keep_r = value;
+    } else if (!strcmp(name, "l2_keep_p")) {
+        if (value < 0) return MAS_EINVAL;
+        h->l2.keep_p = value;
+    } else if (!strcmp(name, "l2_first_x")) {
+        if (value != 0 && value != 1) return MAS_EINVAL;
+        h->l2.first_x = value;
     } else {
         return MAS_EINVAL;
     }
-    h->graph_dirty = true;
+    drop_graphs(h);
     return MAS_OK;
 }
 
@@ -683,95 +808,32 @@ extern "C" int mas_pcg_solve(mas_pcg_t *h, const double *b_dev, double *x_dev, d
     if (!h || !b_dev || !x_dev || b_dev == x_dev || !(rtol >= 0.0) || maxit < 0 || !aligned16(b_dev) ||
         !aligned16(x_dev))
         return MAS_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    int rc = ensure_hist(h, maxit);
-    if (rc != MAS_OK) return rc;
+    DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
+    return solve_core(h, 1, &b_dev, &x_dev, rtol, maxit, (cudaStream_t)stream, iters_out, nullptr, reshist_host);
+}
 
-    h->h_args->b = b_dev; h->h_args->x = x_dev; h->h_args->rtol = rtol; h->h_args->maxit = maxit; h->h_args->pad = 0;
-    CK(cudaMemcpyAsync(h->args.p, h->h_args, sizeof(SolveArgs), cudaMemcpyHostToDevice, s));
-
-    int mode = h->loop_mode;
-    PersistParams ppar;
-    int pgrid = 0;
-    size_t psmem = 0;
-    const void *pfunc = nullptr;
-    const bool persistent = plan_persistent(h, &ppar, &pgrid, &psmem, &pfunc);
-    long long launched_outside = 2, launched_loop = 0;
-    if (persistent) {                      // init + loop + finish in one cooperative kernel
-        OpDev op = h->op;
-        void *kargs[2] = {&op, &ppar};
-        if (cudaLaunchCooperativeKernel(pfunc, dim3(pgrid), dim3(PNT), kargs, psmem, s) == cudaSuccess) {
-            mode = 2;
-            launched_outside = 0;
-            launched_loop = 1;
-        } else {
-            cudaGetLastError();            // refused (e.g. co-residency limits): use the streaming loop instead
-            h->coop_ok = 0;
-        }
+extern "C" int mas_pcg_solve_multi(mas_pcg_t *h, int nrhs, const double *const *b_dev, double *const *x_dev,
+                                   double rtol, int maxit, void *stream, int *iters_out, int *status_out,
+                                   double *reshist_host)
+{
+    if (!h || nrhs < 1 || nrhs > MAX_RHS || !b_dev || !x_dev || !(rtol >= 0.0) || maxit < 0) return MAS_EINVAL;
+    for (int j = 0; j < nrhs; j++) {
+        if (!b_dev[j] || !x_dev[j] || !aligned16(b_dev[j]) || !aligned16(x_dev[j])) return MAS_EINVAL;
+        for (int l = 0; l < nrhs; l++)
+            if (b_dev[j] == x_dev[l] || (l != j && x_dev[j] == x_dev[l])) return MAS_EINVAL;
     }
-    if (mode == 1 && (h->graph_dirty || !h->exec)) {
-        if (build_graph(h) != MAS_OK && h->pdl) {   // programmatic edges refused: plain edges
-            h->pdl = 0;
-            drop_graph(h);
-        }
-        if ((h->graph_dirty || !h->exec) && build_graph(h) != MAS_OK) {
-            drop_graph(h);                    // driver without conditional nodes: fall back, and say so in stats
-            mode = 0;
-        }
-    }
-    if (mode == 2) {
-        // launched above
-    } else if (mode == 1) {
-        CK(cudaGraphLaunch(h->exec, s));
-    } else {
-        LoopCtx c;
-        c.op = h->op; c.work = h->work; c.use_cond = 0; c.xin = nullptr; c.args = h->args.p; c.y = h->q.p;
-        memset(&c.cond, 0, sizeof(c.cond));
-        CK(launch(make_apply(h, c), s));
-        CK(launch(make_init(h, c), s));
-        const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
-        for (int done = 0; done < maxit;) {
-            CK(cudaMemcpyAsync(h->h_st, h->st.p, sizeof(State), cudaMemcpyDeviceToHost, s));
-            CK(cudaStreamSynchronize(s));
-            if (!h->h_st->active) break;
-            const int chunk = maxit - done < HOST_CHUNK ? maxit - done : HOST_CHUNK;
-            for (int it = 0; it < chunk; it++) {
-                CK(launch(k1, s));
-                CK(launch(k2, s));
-            }
-            launched_loop += 2LL * chunk;
-            done += chunk;
-        }
-        if (use_xfuse(h)) CK(launch(make_xtail(h, c), s));
-    }
-    if (use_xfuse(h) && mode != 2) launched_outside += 1;
-    CK(cudaMemcpyAsync(h->h_st, h->st.p, sizeof(State), cudaMemcpyDeviceToHost, s));
-    CK(cudaMemcpyAsync(h->h_hist, h->hist.p, ((size_t)maxit + 1) * sizeof(double), cudaMemcpyDeviceToHost, s));
-    CK(cudaStreamSynchronize(s));          // the one host sync of a graph-mode solve
-    const State &st = *h->h_st;
-    if (st.bb == 0.0) {                    // zero right-hand side: x = 0
-        CK(cudaMemsetAsync(x_dev, 0, h->n * sizeof(double), s));
-        CK(cudaStreamSynchronize(s));
-    }
-    if (iters_out) *iters_out = st.k;
-    if (reshist_host) memcpy(reshist_host, h->h_hist, ((size_t)st.k + 1) * sizeof(double));
-    h->loop_mode_used = mode;
-    h->stats[0] = mode == 1 ? (long long)st.launches : launched_loop;
-    h->stats[6] = mode == 2 ? pgrid : 0;
-    h->stats[7] = (mode == 1 && h->pdl && h->variant >= 2 && !use_qrec(h)) ? 1 : 0;
-    h->stats[1] = launched_outside;
-    h->stats[2] = mode;
-    // unfused: K1 r,p -> p,q (4N); K2 x,p,r,q -> x,r (6N).  xfuse: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)
-    h->stats[4] = use_qrec(h) ? 5 : (use_xfuse(h) ? 6 : 4);
-    h->stats[5] = use_xfuse(h) ? 3 : 6;
-    h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
-    return st.status;
+    DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
+    return solve_core(h, nrhs, b_dev, x_dev, rtol, maxit, (cudaStream_t)stream, iters_out, status_out, reshist_host);
 }
 
 extern "C" int mas_pcg_solve_host(mas_pcg_t *h, const double *b_host, double *x_host, double rtol, int maxit,
                                   void *stream, int *iters_out, double *reshist_host)
 {
     if (!h || !b_host || !x_host) return MAS_EINVAL;
+    DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
     cudaStream_t s = (cudaStream_t)stream;
     if (!h->bdev.p && h->bdev.alloc(h->n) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
     if (!h->xdev.p && h->xdev.alloc(h->n) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
@@ -779,180 +841,14 @@ extern "C" int mas_pcg_solve_host(mas_pcg_t *h, const double *b_host, double *x_
     CK(cudaMemcpyAsync(h->bdev.p, b_host, bytes, cudaMemcpyHostToDevice, s));
     CK(cudaMemcpyAsync(h->xdev.p, x_host, bytes, cudaMemcpyHostToDevice, s));
     const int rc = mas_pcg_solve(h, h->bdev.p, h->xdev.p, rtol, maxit, stream, iters_out, reshist_host);
-    if (rc < 0) return rc;
+    if (rc < 0 && rc != MAS_EBREAKDOWN) return rc;
     CK(cudaMemcpyAsync(x_host, h->xdev.p, bytes, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
     return rc;
 }
 
-extern "C" int mas_pcg_profile(mas_pcg_t *h, const double *b_dev, double *x_dev, int nit, void *stream, double *ms_out)
-{
-    if (!h || !b_dev || !x_dev || b_dev == x_dev || !ms_out || nit < 1 || nit > 256 || !aligned16(b_dev) ||
-        !aligned16(x_dev))
-        return MAS_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    h->h_args->b = b_dev; h->h_args->x = x_dev; h->h_args->rtol = 0.0; h->h_args->maxit = nit; h->h_args->pad = 0;
-    int rc = ensure_hist(h, nit);
-    if (rc != MAS_OK) return rc;
-    CK(cudaMemcpyAsync(h->args.p, h->h_args, sizeof(SolveArgs), cudaMemcpyHostToDevice, s));
-    LoopCtx c;
-    c.op = h->op; c.work = h->work; c.use_cond = 0; c.xin = nullptr; c.args = h->args.p; c.y = h->q.p;
-    memset(&c.cond, 0, sizeof(c.cond));
-    std::vector<cudaEvent_t> ev(2 * (size_t)nit + 1);
-    for (cudaEvent_t &e : ev) CK(cudaEventCreate(&e));
-    CK(launch(make_apply(h, c), s));
-    CK(launch(make_init(h, c), s));
-    const KLaunch k1 = make_k1(h, c), k2 = make_k2(h, c);
-    CK(cudaEventRecord(ev[0], s));
-    for (int it = 0; it < nit; it++) {
-        CK(launch(k1, s));
-        CK(cudaEventRecord(ev[2 * it + 1], s));
-        CK(launch(k2, s));
-        CK(cudaEventRecord(ev[2 * it + 2], s));
-    }
-    CK(cudaStreamSynchronize(s));
-    double sum1 = 0, sum2 = 0, min1 = 1e30, min2 = 1e30;
-    for (int it = 0; it < nit; it++) {
-        float a = 0, b = 0;
-        CK(cudaEventElapsedTime(&a, ev[2 * it], ev[2 * it + 1]));
-        CK(cudaEventElapsedTime(&b, ev[2 * it + 1], ev[2 * it + 2]));
-        sum1 += a; sum2 += b;
-        if (a < min1) min1 = a;
-        if (b < min2) min2 = b;
-    }
-    for (cudaEvent_t &e : ev) cudaEventDestroy(e);
-    ms_out[0] = sum1 / nit; ms_out[1] = sum2 / nit; ms_out[2] = min1; ms_out[3] = min2;
-    h->stats[4] = use_qrec(h) ? 5 : (use_xfuse(h) ? 6 : 4);
-    h->stats[5] = use_xfuse(h) ? 3 : 6;
-    h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
-    return MAS_OK;
-}
-
-// =============================================================================================
-// NEXT-1: explicit viscosity advance by RKL2 super time stepping (R7)
-// =============================================================================================
-namespace {
-
-double rkl2_b(int j) { return j < 3 ? 1.0 / 3.0 : ((double)j * j + j - 2.0) / (2.0 * j * (j + 1.0)); }
-
-void sts_planes(const mas_pcg *h, StencilParams &sp)
-{
-    stencil_common(h, sp);                       // S = L_sym: the dt-independent planes
-    sp.E = h->SD.p; sp.F = h->CP.p; sp.AR = h->CRoff.p; sp.AT = h->CT.p; sp.Vinv = h->Vinv.p;
-}
-
-int launch_stencil(const mas_pcg *h, StencilParams &sp, int epi, cudaStream_t s)
-{
-    KLaunch k;
-    OpDev op = h->op;
-    stencil_configure_any(h->nr, h->nt, h->np, h->uniform_phi, epi, h->stencil_tile, h->num_sms, &sp, &k.func, &k.grid,
-                          &k.block, &k.smem);
-    k.args[0] = &op; k.args[1] = &sp;
-    CK(launch(k, s));
-    return MAS_OK;
-}
-
-}  // namespace
-
-extern "C" int mas_pcg_lambda_max(const mas_pcg_t *h, double *out)
-{
-    if (!h || !out) return MAS_EINVAL;
-    *out = h->lambda_max;
-    return MAS_OK;
-}
-
-extern "C" int mas_sts_stages(const mas_pcg_t *h, double tau, int *s_out)
-{
-    if (!h || !s_out || !(tau >= 0.0) || !isfinite(tau)) return MAS_EINVAL;
-    // stable iff tau <= (s^2 + s - 2)/4 * 2/lambda_max
-    const double need = 2.0 * tau * h->lambda_max;          // s^2 + s - 2 >= need
-    long long s = (long long)ceil(0.5 * (-1.0 + sqrt(9.0 + 4.0 * need)));
-    if (s < 2) s = 2;
-    while ((double)s * s + s - 2.0 < need) ++s;
-    if (s > (1LL << 30)) return MAS_EINVAL;
-    *s_out = (int)s;
-    return MAS_OK;
-}
-
-extern "C" int mas_pcg_lop(mas_pcg_t *h, const double *u_dev, double *y_dev, void *stream)
-{
-    if (!h || !u_dev || !y_dev || u_dev == y_dev || !aligned16(u_dev) || !aligned16(y_dev)) return MAS_EINVAL;
-    StencilParams sp;
-    sts_planes(h, sp);
-    sp.u = u_dev; sp.out = y_dev; sp.c_u = 0.0; sp.c_L = 1.0;     // out = M u
-    return launch_stencil(h, sp, EPI_STS, (cudaStream_t)stream);
-}
-
-extern "C" int mas_sts_advance(mas_pcg_t *h, double *u_dev, double tau, int s, void *stream)
-{
-    if (!h || !u_dev || !aligned16(u_dev) || s < 2 || !(tau >= 0.0) || !isfinite(tau)) return MAS_EINVAL;
-    cudaStream_t st = (cudaStream_t)stream;
-    double *my0 = h->q.p, *ya = h->p0.p, *yb = h->p1.p;           // the PCG workspaces double as stage buffers
-    const double w1 = 4.0 / ((double)s * s + s - 2.0);
-    StencilParams sp;
-    // stage 1: Y_1 = Y_0 + mu~_1 tau M Y_0 ; keep M Y_0
-    sts_planes(h, sp);
-    sp.u = u_dev; sp.out = ya; sp.out2 = my0; sp.c_u = 1.0; sp.c_L = rkl2_b(1) * w1 * tau;
-    int rc = launch_stencil(h, sp, EPI_STS, st);
-    if (rc != MAS_OK) return rc;
-    const double *yjm1 = ya, *yjm2 = u_dev;
-    for (int j = 2; j <= s; j++) {
-        const double bj = rkl2_b(j), bjm1 = rkl2_b(j - 1), bjm2 = rkl2_b(j - 2);
-        const double mu = (2.0 * j - 1.0) / j * bj / bjm1;
-        const double nu = -(j - 1.0) / j * bj / bjm2;
-        const double mut = mu * w1, gat = -(1.0 - bjm1) * mut;
-        // Y_j overwrites Y_{j-2}'s buffer (each cell is read by the thread that writes it), except that
-        // Y_0 = u_dev must survive until the last stage, which writes the result into it.
-        double *out = (j == s) ? u_dev : (yjm2 == u_dev ? yb : const_cast<double *>(yjm2));
-        sts_planes(h, sp);
-        sp.u = yjm1; sp.a1 = yjm2; sp.a2 = u_dev; sp.a3 = my0; sp.out = out;
-        sp.c_u = mu; sp.c_a1 = nu; sp.c_a2 = 1.0 - mu - nu; sp.c_L = mut * tau; sp.c_a3 = gat * tau;
-        rc = launch_stencil(h, sp, EPI_STS, st);
-        if (rc != MAS_OK) return rc;
-        yjm2 = yjm1;
-        yjm1 = out;
-    }
-    h->graph_dirty = h->graph_dirty;             // PCG workspaces were clobbered; solves re-initialise them
-    return MAS_OK;
-}
-
-// Measurement aid: sustained time of a trivial linear kernel with K1's (which = 6) or K2's (which = 3) DRAM mix
-// over the handle's own N-vectors (their contents are destroyed; the next solve re-initialises them).
-extern "C" int mas_pcg_mix_probe(mas_pcg_t *h, int which, int reps, void *stream, double *ms_out)
-{
-    if (!h || !ms_out || (which != 6 && which != 3) || reps < 1 || reps > 100000) return MAS_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    if (!h->bdev.p && h->bdev.alloc(h->n) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
-    CK(cudaMemsetAsync(h->bdev.p, 0, h->n * sizeof(double), s));
-    CK(cudaMemsetAsync(h->r.p, 0, h->n * sizeof(double), s));
-    CK(cudaMemsetAsync(h->q.p, 0, h->n * sizeof(double), s));
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0));
-    CK(cudaEventCreate(&e1));
-    const size_t n2 = h->n / 2;
-    double best = 1e30;
-    for (int mult = 4; mult <= 32; mult *= 2) {                 // the grid size matters by a few percent: take the best
-        const int blocks = h->num_sms * mult;
-        for (int pass = 0; pass < 2; pass++) {                  // pass 0 = warm-up
-            const int n = pass ? reps : 3;
-            CK(cudaEventRecord(e0, s));
-            for (int r = 0; r < n; r++) {
-                if (which == 6)
-                    k_mix6<<<blocks, 256, 0, s>>>((const double2 *)h->r.p, (const double2 *)h->p0.p, (double2 *)h->bdev.p,
-                                                  (double2 *)h->p1.p, (double2 *)h->q.p, n2);
-                else
-                    k_mix3<<<blocks, 256, 0, s>>>((double2 *)h->r.p, (const double2 *)h->q.p, n2);
-            }
-            CK(cudaEventRecord(e1, s));
-            CK(cudaEventSynchronize(e1));
-            float ms = 0;
-            CK(cudaEventElapsedTime(&ms, e0, e1));
-            if (pass && ms / n < best) best = ms / n;
-        }
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    CK(cudaGetLastError());
-    *ms_out = best;
-    return MAS_OK;
-}
+#include "host_sts.inc"
+#include "host_slabs.inc"
+#ifdef MAS_PCG_DEBUG_PROBES
+#include "host_debug.inc"
+#endif

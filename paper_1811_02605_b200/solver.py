@@ -1,4 +1,4 @@
-"""MasPcg: torch-tensor front end of the C ABI (argument marshalling only)."""
+"""MasPcg / MasPcgSlabs: torch-tensor front ends of the C ABI (argument marshalling only)."""
 from __future__ import annotations
 
 import torch
@@ -13,7 +13,7 @@ def _stream_ptr(stream=None) -> int:
 
 def _dev_ptr(t: torch.Tensor, n: int) -> int:
     if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n):
-        raise ValueError("need a contiguous CUDA float64 tensor with nr*nt*np elements")
+        raise ValueError(f"need a contiguous CUDA float64 tensor with {n} elements")
     return t.data_ptr()
 
 
@@ -52,6 +52,12 @@ class MasPcg:
         return B.mas_pcg_solve(self._h, _dev_ptr(b, self.n), _dev_ptr(x, self.n), rtol, maxit,
                                _stream_ptr(stream), want_hist)
 
+    def solve_multi(self, bs, xs, rtol: float, maxit: int, stream=None, want_hist=True):
+        """nrhs <= 3 right-hand sides sharing the operator, one set of launches; xs updated in place.
+        Returns (worst status, [status_j], [iters_j], [hist_j])."""
+        return B.mas_pcg_solve_multi(self._h, [_dev_ptr(b, self.n) for b in bs], [_dev_ptr(x, self.n) for x in xs],
+                                     rtol, maxit, _stream_ptr(stream), want_hist)
+
     def solve_host(self, b_host: torch.Tensor, x_host: torch.Tensor, rtol: float, maxit: int, stream=None,
                    want_hist=True):
         """Same with HOST (ideally pinned) float64 tensors; H2D/D2H copies happen inside the C call."""
@@ -60,9 +66,6 @@ class MasPcg:
                 raise ValueError("need contiguous host float64 tensors with nr*nt*np elements")
         return B.mas_pcg_solve_host(self._h, b_host.data_ptr(), x_host.data_ptr(), rtol, maxit,
                                     _stream_ptr(stream), want_hist)
-
-    def profile(self, b: torch.Tensor, x: torch.Tensor, nit: int, stream=None):
-        return B.mas_pcg_profile(self._h, _dev_ptr(b, self.n), _dev_ptr(x, self.n), nit, _stream_ptr(stream))
 
     # ---- NEXT-1: explicit operator and RKL2 super time stepping ----
     def lop(self, u: torch.Tensor, y: torch.Tensor | None = None, stream=None) -> torch.Tensor:
@@ -83,8 +86,42 @@ class MasPcg:
         B.mas_sts_advance(self._h, _dev_ptr(u, self.n), tau, s, _stream_ptr(stream))
         return u
 
-    def mix_probe(self, which: int, reps: int = 50, stream=None) -> float:
-        return B.mas_pcg_mix_probe(self._h, which, reps, _stream_ptr(stream))
-
     def stats(self):
         return B.mas_pcg_stats(self._h)
+
+
+class MasPcgSlabs:
+    """The same operator split into r-slabs (NEXT-3), all driven from this process on the current device.
+    b and x are given as whole-mesh tensors and handed to the library slab by slab (views of their planes)."""
+
+    def __init__(self, mesh, dt, nu_kind, nu, bc, i_split):
+        if not torch.cuda.is_available():
+            raise RuntimeError("MasPcgSlabs needs a CUDA device (there is no CPU fallback)")
+        self.shape = (mesh.nr, mesh.nt, mesh.np_)
+        self.split = [int(v) for v in i_split]
+        self._h = B.mas_pcg_slabs_create(self.shape, mesh.metric_arrays(), dt, nu_kind, nu, bc, self.split)
+
+    def close(self):
+        if getattr(self, "_h", None) and B is not None and getattr(B, "mas_pcg_slabs_destroy", None):
+            B.mas_pcg_slabs_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def set_dt(self, dt, stream=None):
+        B.mas_pcg_slabs_set_dt(self._h, dt, _stream_ptr(stream))
+
+    def set_option(self, name, value):
+        B.mas_pcg_slabs_set_option(self._h, name, value)
+
+    def _slab_ptrs(self, t: torch.Tensor):
+        plane = self.shape[1] * self.shape[2]
+        _dev_ptr(t, self.shape[0] * plane)
+        return [t.data_ptr() + 8 * plane * lo for lo in self.split[:-1]]
+
+    def solve(self, b: torch.Tensor, x: torch.Tensor, rtol: float, maxit: int, stream=None, want_hist=True):
+        return B.mas_pcg_slabs_solve(self._h, self._slab_ptrs(b), self._slab_ptrs(x), rtol, maxit,
+                                     _stream_ptr(stream), want_hist)
+
+    def stats(self):
+        return B.mas_pcg_slabs_stats(self._h)

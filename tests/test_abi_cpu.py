@@ -23,10 +23,26 @@ def declared_functions():
 def test_library_exports_every_declared_symbol():
     names = declared_functions()
     assert {"mas_pcg_create", "mas_pcg_solve", "mas_pcg_destroy", "mas_pcg_apply", "mas_pcg_set_dt",
-            "mas_pcg_solve_host", "mas_pcg_strerror", "mas_pcg_stats", "mas_pcg_set_option"} <= set(names)
+            "mas_pcg_solve_host", "mas_pcg_solve_multi", "mas_pcg_strerror", "mas_pcg_stats", "mas_pcg_set_option",
+            "mas_pcg_slabs_create", "mas_pcg_slabs_solve", "mas_pcg_slabs_destroy"} <= set(names)
     L = ctypes.CDLL(B._build.LIB) if os.path.exists(B._build.LIB) else B.lib()
     for n in names:
         assert hasattr(L, n), f"{n} declared in include/mas_pcg.h but not exported"
+
+
+def test_measurement_probes_are_not_in_the_product_library():
+    """include/mas_pcg_debug.h is a separate library (VERDICT r1 #13): the product exports none of it."""
+    dbg_src = open(os.path.join(ROOT, "include", "mas_pcg_debug.h")).read()
+    probes = sorted(set(re.findall(r"\b(mas_pcg_dbg_[a-z_]+)\s*\(", re.sub(r"/\*.*?\*/", "", dbg_src, flags=re.S))))
+    assert probes == ["mas_pcg_dbg_mix_probe", "mas_pcg_dbg_profile"]
+    B.lib()
+    prod, dbg = ctypes.CDLL(B._build.LIB), ctypes.CDLL(B._build.LIB_DBG)
+    for n in probes:
+        assert not hasattr(prod, n), f"{n} leaked into the product library"
+        assert hasattr(dbg, n)
+    for n in declared_functions():
+        assert hasattr(dbg, n)
+    assert not any("dbg" in n or "probe" in n or "profile" in n for n in declared_functions())
 
 
 def test_python_binding_has_the_same_names():
@@ -75,7 +91,11 @@ def test_null_handle_calls_are_einval_and_destroy_null_is_safe():
     assert L.mas_pcg_apply(None, None, None, None) == B.MAS_EINVAL
     assert L.mas_pcg_set_dt(None, 1.0, None) == B.MAS_EINVAL
     assert L.mas_pcg_stats(None, None) == B.MAS_EINVAL
-    assert L.mas_pcg_set_option(None, b"variant", 0) == B.MAS_EINVAL
+    assert L.mas_pcg_set_option(None, b"tile", 0) == B.MAS_EINVAL
+    assert L.mas_pcg_solve_multi(None, 1, None, None, 0.0, 1, None, None, None, None) == B.MAS_EINVAL
+    assert L.mas_pcg_slabs_solve(None, None, None, 0.0, 1, None, None, None) == B.MAS_EINVAL
+    assert L.mas_pcg_slabs_set_dt(None, 1.0, None) == B.MAS_EINVAL
+    L.mas_pcg_slabs_destroy(None)
     L.mas_pcg_destroy(None)
 
 
@@ -84,7 +104,7 @@ def test_product_path_does_not_import_the_oracle():
     pkg = os.path.join(ROOT, "paper_1811_02605_b200")
     for dirpath, _, files in os.walk(pkg):
         for f in files:
-            if f.endswith((".py", ".cu", ".cuh", ".h")):
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".inc")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", txt, flags=re.M), f
                 assert "mas_pcg_ref" not in txt, f

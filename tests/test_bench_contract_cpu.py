@@ -43,6 +43,7 @@ def test_workload_is_seeded_and_rank_offset():
     p1, _, b1, *_ = bench.workload("c1", 1)
     assert np.array_equal(b0, b0b) and not np.array_equal(b0, b1)
     assert (rtol, maxit) == (1e-10, 1000) and "32x32x64" in desc and dt0 > 0
-    assert bench.ncu_traffic("k1_fused_matvec") > 1e9          # committed ncu summary is readable
+    assert bench.ncu_traffic("k_stencil_sts")[0] > 1e9         # committed ncu summary is readable, with provenance
+    assert bench.ncu_traffic("k_stencil_sts")[1]
     peak, src = bench.hbm_peak()
     assert 5000 < peak < 9000 and ("measured" in src or "fallback" in src)

@@ -64,42 +64,61 @@ def test_gpu_operator_symmetric_and_constant_closed_form():
     assert np.allclose(gpu.apply(one).cpu().numpy().reshape(mesh.shape), V, rtol=1e-13, atol=0)
 
 
-# ------------------------------------------------------------------ full solves: every K1 variant / loop mode
-# (variant, tile, xfuse); xfuse = 2 means xfuse + qrecompute (q not stored, K2 recomputes it: 64 B/cell/it)
-VARIANTS = [(0, 0, 0)] + [(1, t, 0) for t in range(7)] + [(2, t, x) for t in range(7) for x in (0, 1)] \
-    + [(2, 0, 2), (2, 1, 2), (2, 3, 2)] + [(3, t, 1) for t in range(7)]      # variant 3: TMA + mbarrier K1
+# ------------------------------------------------------------------ full solves: every K1 tile / traffic form / loop mode
+# (K1 tile, qrecompute, K2R tile): qrecompute = 1 is the 64 B/cell/iteration form (q not stored, K2R recomputes it)
+FORMS = [(t, 0, 0) for t in range(7)] + [(t, 1, t % 6) for t in range(7)]
 
 
 @pytest.mark.parametrize("loop_mode", [1, 0])
-@pytest.mark.parametrize("variant,tile,xfuse", VARIANTS)
-def test_solve_parity_general_mesh_all_variants(variant, tile, xfuse, loop_mode):
-    mesh, dt, nu_kind, nu = H.general_case(21, 19, 134, s=500.0)   # 3 phi tiles (ragged), ragged theta
+@pytest.mark.parametrize("tile,qrec,k2r_tile", FORMS)
+def test_solve_parity_general_mesh_all_forms(tile, qrec, k2r_tile, loop_mode):
+    mesh, dt, nu_kind, nu = H.general_case(21, 19, 134, s=500.0)   # 2 phi tiles (ragged), ragged theta
     oref, gpu = H.both_ops(mesh, dt, nu_kind, nu)
     gpu.set_option("persistent", 0)              # this test is about the streaming kernels
-    gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
-    gpu.set_option("xfuse", min(xfuse, 1))
-    gpu.set_option("qrecompute", int(xfuse == 2))
-    gpu.set_option("k2r_tile", tile % 2)
+    gpu.set_option("qrecompute", qrec)
+    gpu.set_option("k2r_tile", k2r_tile)
     gpu.set_option("loop_mode", loop_mode)
     rng = np.random.default_rng(3)
     b = rng.uniform(-1, 1, mesh.shape)
     x0 = rng.standard_normal(mesh.shape)
-    H.check_parity(gpu, oref, b, x0, 1e-10, 2000, label=f"v{variant} t{tile} m{loop_mode}")
-    assert gpu.stats()["loop_mode"] == loop_mode
+    H.check_parity(gpu, oref, b, x0, 1e-10, 2000, label=f"t{tile} q{qrec} m{loop_mode}")
+    st = gpu.stats()
+    assert st["loop_mode"] == loop_mode and st["bytes_per_cell_iter"] == (64 if qrec else 72)
 
 
-@pytest.mark.parametrize("variant,tile,xfuse", VARIANTS)
-def test_solve_parity_uniform_phi_all_variants(variant, tile, xfuse):
+@pytest.mark.parametrize("tile,qrec,k2r_tile", FORMS)
+def test_solve_parity_uniform_phi_all_forms(tile, qrec, k2r_tile):
     prob = configs.make("c3", shape=(40, 37, 192))
     s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
     oref, gpu = H.both_ops(prob.mesh, 1e3 / s1, prob.nu_kind, prob.nu)
     gpu.set_option("persistent", 0)
-    gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
-    gpu.set_option("xfuse", min(xfuse, 1))
-    gpu.set_option("qrecompute", int(xfuse == 2))
-    H.check_parity(gpu, oref, configs.rhs_blob(prob), None, 1e-9, 3000, label=f"v{variant} t{tile} x{xfuse}")
+    gpu.set_option("qrecompute", qrec)
+    gpu.set_option("k2r_tile", k2r_tile)
+    H.check_parity(gpu, oref, configs.rhs_blob(prob), None, 1e-9, 3000, label=f"uniform t{tile} q{qrec}")
+
+
+@pytest.mark.parametrize("qrec", [0, 1])
+def test_l2_plan_hints_do_not_change_the_bits(qrec):
+    """The L2 eviction-priority hints are performance-only: the same solve with and without them is bit-identical."""
+    import torch
+    prob = configs.make("c3", shape=(40, 37, 192))
+    s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
+    from paper_1811_02605_b200 import MasPcg
+    gpu = MasPcg(prob.mesh, 1e3 / s1, prob.nu_kind, prob.nu)
+    gpu.set_option("persistent", 0)
+    gpu.set_option("qrecompute", qrec)
+    b = _t(configs.rhs_blob(prob))
+    runs = []
+    for keep_r, keep_p, first_x in [(0, 0, 0), (17, 0, 0), (40, 9, 1), (1000, 1000, 1)]:
+        gpu.set_option("l2_keep_r", keep_r)
+        gpu.set_option("l2_keep_p", keep_p)
+        gpu.set_option("l2_first_x", first_x)
+        x = torch.zeros_like(b)
+        st, k, h = gpu.solve(b, x, 1e-9, 3000)
+        runs.append((st, k, h.tobytes(), x.cpu().numpy().tobytes()))
+    assert all(r == runs[0] for r in runs[1:])
 
 
 @pytest.mark.parametrize("persistent", [0, 1])
@@ -358,9 +377,8 @@ def test_history_longer_than_initial_capacity_and_stream():
 
 
 # ------------------------------------------------------------------ determinism as a race detector
-@pytest.mark.parametrize("variant,tile,xfuse", [(0, 0, 0), (1, 1, 0), (2, 0, 0), (2, 0, 1), (2, 1, 1), (2, 3, 1), (2, 0, 2), (3, 0, 1), (3, 1, 1),
-                                                (3, 3, 1)])
-def test_rerun_bit_identity_every_kernel_family(variant, tile, xfuse):
+@pytest.mark.parametrize("tile,qrec,k2r_tile", [(0, 0, 0), (1, 0, 0), (3, 0, 0), (0, 1, 1), (1, 1, 0), (3, 1, 2), (5, 1, 4)])
+def test_rerun_bit_identity_every_kernel_family(tile, qrec, k2r_tile):
     """north_star (3): deterministic reductions => a rerun gives the same bits.  compute-sanitizer is closed on
     this GPU pool, so this doubles as the race check of the shared-memory rings: a missing barrier shows up as
     run-to-run differences on a mesh with thousands of blocks in flight."""
@@ -370,10 +388,9 @@ def test_rerun_bit_identity_every_kernel_family(variant, tile, xfuse):
     from paper_1811_02605_b200 import MasPcg
     gpu = MasPcg(prob.mesh, 1e3 / s1, prob.nu_kind, prob.nu)
     gpu.set_option("persistent", 0)
-    gpu.set_option("variant", variant)
     gpu.set_option("tile", tile)
-    gpu.set_option("xfuse", min(xfuse, 1))
-    gpu.set_option("qrecompute", int(xfuse == 2))
+    gpu.set_option("qrecompute", qrec)
+    gpu.set_option("k2r_tile", k2r_tile)
     b = _t(configs.rhs_blob(prob))
     runs = []
     for _ in range(4):
@@ -416,6 +433,7 @@ def test_large_mesh_64bit_offsets_closed_forms():
     x = torch.zeros_like(b)
     st, k, h = gpu.solve(b, x, 0.0, 5)
     assert (st, k) == (1, 5) and np.isfinite(h).all() and (np.diff(h) != 0).all()
+    assert gpu.stats()["bytes_per_cell_iter"] == 64        # the default form: K2R (two sums) on 11 840+ K1 blocks
     gpu.apply(x, y)                       # y = A x
     y.neg_().add_(V * b)                  # true residual b_s - A x
     bs_norm = float((V * b).norm())
@@ -445,13 +463,13 @@ def test_persistent_kernel_parity_general_mesh_warm_start_and_bits(shape, bc):
     assert runs[0] == runs[1] == runs[2]
 
 
-def test_persistent_auto_threshold_and_too_large_falls_back():
+def test_persistent_default_and_too_large_falls_back():
     from paper_1811_02605_b200 import MasPcg
     small = configs.make("c1")
     gpu = MasPcg(small.mesh, small.dt_for(2.0), small.nu_kind, small.nu)
     b = _t(configs.rhs_uniform(small))
     gpu.solve(b, _t(np.zeros(small.mesh.shape)), 1e-10, 100)
-    assert gpu.stats()["loop_mode"] == 2                     # auto: small mesh -> one kernel
+    assert gpu.stats()["loop_mode"] == 2                     # default: small mesh -> one kernel
     big = configs.make("c3", shape=(64, 96, 256))            # 1.6 M cells: state does not fit on chip
     s1 = H.oracle_s1(big.mesh, big.nu_kind, big.nu)
     gpu = MasPcg(big.mesh, 100.0 / s1, big.nu_kind, big.nu)

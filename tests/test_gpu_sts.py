@@ -8,7 +8,7 @@ from tests import helpers as H
 
 pytestmark = pytest.mark.gpu
 
-LOP_RTOL = 1e-13      # one stencil application: rounding-order differences only
+LOP_RTOL = 1e-14      # one stencil application: rounding-order differences only (observed <= 4e-16 in round 2)
 STS_RTOL = 1e-11      # s stages of such differences (s <= 64 here), relative to max |u|
 
 
@@ -17,7 +17,7 @@ def _t(a):
     return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
 
 
-@pytest.mark.parametrize("tile", list(range(12)))      # 6, 7: TMA bulk-copy + mbarrier variant
+@pytest.mark.parametrize("tile", list(range(6)))
 @pytest.mark.parametrize("shape,bc", [((9, 11, 70), (0, 0)), ((21, 19, 134), (1, 0)), ((1, 1, 2), (0, 0)),
                                       ((5, 17, 260), (1, 1)), ((40, 9, 128), (0, 1))])
 def test_lop_and_apply_match_oracle_general_mesh(shape, bc, tile):
@@ -28,26 +28,22 @@ def test_lop_and_apply_match_oracle_general_mesh(shape, bc, tile):
     for fn_ref, fn_gpu in ((oref.lop, gpu.lop), (oref.apply, gpu.apply)):
         y_ref = fn_ref(u)
         y = fn_gpu(_t(u)).cpu().numpy().reshape(mesh.shape)
-        assert np.abs(y - y_ref).max() <= LOP_RTOL * np.abs(y_ref).max()
+        assert H.apply_gap(y, y_ref, f"lop/apply {shape} tile {tile}") <= LOP_RTOL
     assert gpu.lambda_max() == pytest.approx(oref.lambda_max_bound(), rel=1e-12)
 
 
-def test_lop_uniform_phi_and_baseline_apply_kernel_agree():
+def test_lop_and_apply_uniform_phi():
     prob = configs.make("c3", shape=(40, 37, 192))
     oref, gpu = H.both_ops(prob.mesh, 1e-3, prob.nu_kind, prob.nu)
     u = configs.rhs_blob(prob)
     y_ref = oref.lop(u)
     y = gpu.lop(_t(u)).cpu().numpy()
-    assert np.abs(y - y_ref).max() <= LOP_RTOL * np.abs(y_ref).max()
-    a1 = gpu.apply(_t(u)).cpu().numpy()
-    gpu.set_option("apply_variant", 0)
-    a0 = gpu.apply(_t(u)).cpu().numpy()
+    assert H.apply_gap(y, y_ref, "lop uniform") <= LOP_RTOL
     a_ref = oref.apply(u)
-    for a in (a0, a1):
-        assert np.abs(a - a_ref).max() <= H.APPLY_RTOL * np.abs(a_ref).max()
+    assert H.apply_gap(gpu.apply(_t(u)).cpu().numpy(), a_ref, "apply uniform") <= H.APPLY_RTOL
 
 
-@pytest.mark.parametrize("tile", [0, 1, 3, 4, 6, 7, 8, 11])
+@pytest.mark.parametrize("tile", list(range(6)))
 @pytest.mark.parametrize("s", [2, 3, 5, 16, 64])
 @pytest.mark.parametrize("uniform", [False, True])
 def test_sts_advance_matches_oracle(s, uniform, tile):
