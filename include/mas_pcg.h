@@ -132,8 +132,8 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
  *                 K2R / for apply and RKL2 stages, "ci" r-chunk length of the marching kernels (0 = automatic, else 2..32);
  *   "serpentine"  1 (default): K2 sweeps the mesh backward (L2 reuse across K1 -> K2 -> K1);
  *   "unroll"      PCG iterations per WHILE trip of the graph loop (1..16, default 4);
- *   "l2_keep_r", "l2_keep_p"  number of leading r-planes of r / p whose accesses carry the L2 evict_last priority
- *                 (0 = no hints), "l2_first_x" 1: x is streamed with evict_first.
+ *   "l2_first_x"  1: x (read once and written once per iteration, never reused inside it) is streamed with the L2
+ *                 evict_first priority so that it does not displace r and p on meshes whose vectors fit in L2; 0 (default).
  * Unknown name or value: MAS_EINVAL. */
 int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value);
 

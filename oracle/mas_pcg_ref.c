@@ -385,3 +385,218 @@ done:
     free(y0); free(my0); free(yjm2); free(yjm1); free(yj); free(my);
     return status;
 }
+
+/* ==============================================================================================
+ * NEXT-4: the paper's second preconditioner -- "The second (PC2) uses a
+ * non-overlapping domain decomposition with zero-fill incomplete LU factorization" (Sec. 2.2;
+ * 100-200 iterations against ~550 with PC1; its triangular solves are what the authors call
+ * "not vectorizable" and leave on the CPU).
+ *
+ * The paper prints neither the decomposition nor the factorisation.  Reading (R8):
+ *   * the domains are boxes of bi x bj x bk cells aligned at the mesh origin (the last box of a direction may be
+ *     smaller); A_blk = A_sym with every coupling between cells of different boxes dropped, i.e. the
+ *     block-diagonal part of A_sym in the box partition (block Jacobi; "communication-free");
+ *     a box that spans all of phi keeps the periodic wrap coupling, any other box does not have it;
+ *   * ILU(0) is the textbook zero-fill factorisation (Saad [22], the reference the paper cites for its solvers)
+ *     of A_blk in the natural ordering (phi fastest, then theta, then r): unit lower L and upper U whose
+ *     non-zeros are confined to the pattern of A_blk and with (L U)_ij = (A_blk)_ij on that pattern;
+ *   * M = L U;  z = M^-1 r by a forward and a backward substitution;  the PCG loop is C3's with z = M^-1 r.
+ * Written out generically on a compressed-sparse-row copy of A_blk (row-wise IKJ elimination restricted to
+ * the pattern), so that nothing about the stencil's structure is assumed by the factorisation.
+ * Pinned by tests/test_oracle_pc2_pins.py: (L U = A_blk on the pattern) on dense copies, exactness for
+ * tridiagonal operators (1-D meshes: ILU(0) = LU, one PCG iteration), dt = 0, symmetry and positivity of
+ * M^-1, box locality, dense-LU agreement of the PCG solution, fewer iterations than PC1.
+ * What is tied to the paper's own run (its domains = its MPI ranks' sub-meshes, its 100-200 counts) is
+ * "parity unpinned": not available.
+ * ============================================================================================== */
+
+typedef struct ref_pc2 {
+    size_t n;
+    int nnz_max;
+    size_t *rowptr;     /* [n+1] */
+    int *col;           /* [nnz] ascending within a row */
+    double *val;        /* [nnz] A_blk, overwritten by the factors: strictly lower = L (unit diagonal implied), rest = U */
+    size_t *diag;       /* [n] position of the diagonal entry of each row */
+} ref_pc2;
+
+void mas_ref_pc2_destroy(ref_pc2 *pc)
+{
+    if (!pc) return;
+    free(pc->rowptr); free(pc->col); free(pc->val); free(pc->diag);
+    free(pc);
+}
+
+static int cmp_entry(const void *a, const void *b)
+{
+    const long long ca = *(const long long *)a, cb = *(const long long *)b;
+    return ca < cb ? -1 : (ca > cb ? 1 : 0);
+}
+
+/* A_blk in CSR (values at the operator's current dt), then ILU(0) in place.  bi, bj, bk <= 0 mean "the whole extent". */
+ref_pc2 *mas_ref_pc2_create(const ref_op *op, int bi, int bj, int bk)
+{
+    if (!op) return NULL;
+    const int nr = op->nr, nt = op->nt, np = op->np;
+    if (bi <= 0 || bi > nr) bi = nr;
+    if (bj <= 0 || bj > nt) bj = nt;
+    if (bk <= 0 || bk > np) bk = np;
+    const size_t n = (size_t)nr * nt * np;
+    ref_pc2 *pc = (ref_pc2 *)calloc(1, sizeof(ref_pc2));
+    if (!pc) return NULL;
+    pc->n = n;
+    pc->rowptr = (size_t *)malloc((n + 1) * sizeof(size_t));
+    pc->col = (int *)malloc(7 * n * sizeof(int));
+    pc->val = (double *)malloc(7 * n * sizeof(double));
+    pc->diag = (size_t *)malloc(n * sizeof(size_t));
+    if (!pc->rowptr || !pc->col || !pc->val || !pc->diag) { mas_ref_pc2_destroy(pc); return NULL; }
+
+    /* ---- rows of A_blk: diagonal of A_sym, and -dt G_f for every face whose two cells lie in the same box ---- */
+    size_t nnz = 0;
+    double g[6];
+    for (int i = 0; i < nr; i++)
+        for (int j = 0; j < nt; j++)
+            for (int k = 0; k < np; k++) {
+                const size_t c = ((size_t)i * nt + j) * np + k;
+                faces(op, i, j, k, g);
+                long long cols[7];
+                double vals[7];
+                int m = 0;
+                cols[m] = (long long)c;
+                vals[m++] = volume(op, i, j, k) + op->dt * (g[0] + g[1] + g[2] + g[3] + g[4] + g[5]);
+                const int kp = (k + 1) % np, km = (k + np - 1) % np;
+                const int nb_i[6] = {i - 1, i + 1, i, i, i, i};
+                const int nb_j[6] = {j, j, j - 1, j + 1, j, j};
+                const int nb_k[6] = {k, k, k, k, km, kp};
+                for (int f = 0; f < 6; f++) {
+                    const int ii = nb_i[f], jj = nb_j[f], kk = nb_k[f];
+                    if (ii < 0 || ii >= nr || jj < 0 || jj >= nt) continue;          /* boundary face: no neighbour cell */
+                    if (ii / bi != i / bi || jj / bj != j / bj || kk / bk != k / bk) continue;   /* another box */
+                    const long long cc = (long long)(((size_t)ii * nt + jj) * np + kk);
+                    if (cc == (long long)c) continue;                                 /* np = 1: the cell is its own phi neighbour; flux is zero */
+                    int hit = -1;
+                    for (int e = 1; e < m; e++) if (cols[e] == cc) hit = e;          /* np = 2: both phi faces lead to the same cell */
+                    if (hit >= 0) vals[hit] += -op->dt * g[f];
+                    else { cols[m] = cc; vals[m++] = -op->dt * g[f]; }
+                }
+                /* sort the row by column */
+                long long key[7]; double v2[7];
+                for (int e = 0; e < m; e++) key[e] = cols[e];
+                qsort(key, (size_t)m, sizeof(long long), cmp_entry);
+                for (int e = 0; e < m; e++)
+                    for (int f2 = 0; f2 < m; f2++) if (cols[f2] == key[e]) v2[e] = vals[f2];
+                pc->rowptr[c] = nnz;
+                for (int e = 0; e < m; e++) {
+                    if (key[e] == (long long)c) pc->diag[c] = nnz;
+                    pc->col[nnz] = (int)key[e];
+                    pc->val[nnz++] = v2[e];
+                }
+            }
+    pc->rowptr[n] = nnz;
+
+    /* ---- ILU(0), row-wise IKJ variant restricted to the pattern (Saad, "Iterative Methods for Sparse Linear
+     * Systems", the zero-fill ILU algorithm):
+     *   for i = 1..n-1:  for k in pattern(i), k < i (ascending):  a_ik /= a_kk
+     *                        for j in pattern(i), j > k:  if (k, j) in pattern:  a_ij -= a_ik a_kj          ---- */
+    for (size_t i = 0; i < n; i++)
+        for (size_t e = pc->rowptr[i]; e < pc->diag[i]; e++) {
+            const size_t k = (size_t)pc->col[e];
+            pc->val[e] /= pc->val[pc->diag[k]];
+            const double lik = pc->val[e];
+            for (size_t f = e + 1; f < pc->rowptr[i + 1]; f++) {
+                const int j = pc->col[f];
+                for (size_t t = pc->diag[k] + 1; t < pc->rowptr[k + 1]; t++)
+                    if (pc->col[t] == j) pc->val[f] -= lik * pc->val[t];
+            }
+        }
+    return pc;
+}
+
+/* z = M^-1 r = U^-1 (L^-1 r): forward substitution with the unit lower factor, then backward with U */
+void mas_ref_pc2_apply(const ref_pc2 *pc, const double *r, double *z)
+{
+    const size_t n = pc->n;
+    for (size_t i = 0; i < n; i++) {
+        double s = r[i];
+        for (size_t e = pc->rowptr[i]; e < pc->diag[i]; e++) s -= pc->val[e] * z[pc->col[e]];
+        z[i] = s;
+    }
+    for (size_t i = n; i-- > 0;) {
+        double s = z[i];
+        for (size_t e = pc->diag[i] + 1; e < pc->rowptr[i + 1]; e++) s -= pc->val[e] * z[pc->col[e]];
+        z[i] = s / pc->val[pc->diag[i]];
+    }
+}
+
+/* the factors as dense matrices, for the pins (tiny meshes): Ld = unit lower L, Ud = U, both n x n row-major */
+void mas_ref_pc2_dense_factors(const ref_pc2 *pc, double *Ld, double *Ud)
+{
+    const size_t n = pc->n;
+    memset(Ld, 0, n * n * sizeof(double));
+    memset(Ud, 0, n * n * sizeof(double));
+    for (size_t i = 0; i < n; i++) {
+        Ld[i * n + i] = 1.0;
+        for (size_t e = pc->rowptr[i]; e < pc->rowptr[i + 1]; e++) {
+            if (e < pc->diag[i]) Ld[i * n + (size_t)pc->col[e]] = pc->val[e];
+            else Ud[i * n + (size_t)pc->col[e]] = pc->val[e];
+        }
+    }
+}
+
+/* PCG of SURVEY.md 8(c) C3 with z = M^-1 r, M = the block-Jacobi ILU(0) `pc` (built from `op` at its current dt).
+ * Same arguments, statuses and stopping rule as mas_ref_pcg. */
+int mas_ref_pcg_pc2(const ref_op *op, const ref_pc2 *pc, const double *b_phys, double *x, double rtol, int maxit,
+                    int *iters, double *hist)
+{
+    if (!op || !pc || !b_phys || !x || !iters || rtol < 0.0 || maxit < 0) return REF_EINVAL;
+    const size_t n = (size_t)op->nr * op->nt * op->np;
+    if (pc->n != n) return REF_EINVAL;
+    double *r = (double *)malloc(n * sizeof(double)), *z = (double *)malloc(n * sizeof(double));
+    double *p = (double *)malloc(n * sizeof(double)), *q = (double *)malloc(n * sizeof(double));
+    int status = REF_ENOMEM, k = 0;
+    if (!r || !z || !p || !q) goto done;
+
+    mas_ref_volume(op, z);
+    for (size_t c = 0; c < n; c++) r[c] = z[c] * b_phys[c];     /* b_s = V.b */
+    const double bb = dot(n, r, r);
+    if (!isfinite(bb)) {
+        if (hist) hist[0] = bb;
+        *iters = 0; status = REF_EBREAKDOWN; goto done;
+    }
+    if (bb == 0.0) {
+        memset(x, 0, n * sizeof(double));
+        if (hist) hist[0] = 0.0;
+        *iters = 0; status = REF_OK; goto done;
+    }
+    mas_ref_apply(op, x, q);
+    for (size_t c = 0; c < n; c++) r[c] -= q[c];
+    mas_ref_pc2_apply(pc, r, z);
+    memcpy(p, z, n * sizeof(double));
+    double rho = dot(n, r, z), rr = dot(n, r, r);
+    double h = sqrt(rr / bb);
+    if (hist) hist[0] = h;
+    status = REF_OK;
+    if (!isfinite(rho) || !isfinite(rr)) { *iters = 0; status = REF_EBREAKDOWN; goto done; }
+    while (k < maxit && h > rtol && rho != 0.0) {
+        mas_ref_apply(op, p, q);
+        const double sigma = dot(n, p, q);
+        if (!(sigma > 0.0) || !isfinite(sigma)) { status = REF_EBREAKDOWN; break; }
+        const double alpha = rho / sigma;
+        for (size_t c = 0; c < n; c++) x[c] += alpha * p[c];
+        for (size_t c = 0; c < n; c++) r[c] -= alpha * q[c];
+        mas_ref_pc2_apply(pc, r, z);
+        const double rho1 = dot(n, r, z);
+        rr = dot(n, r, r);
+        k += 1;
+        h = sqrt(rr / bb);
+        if (hist) hist[k] = h;
+        if (!isfinite(rho1) || !isfinite(rr)) { status = REF_EBREAKDOWN; break; }
+        const double beta = rho1 / rho;
+        rho = rho1;
+        for (size_t c = 0; c < n; c++) p[c] = z[c] + beta * p[c];
+    }
+    if (status == REF_OK) status = (h <= rtol || rho == 0.0) ? REF_OK : REF_MAXIT;
+    *iters = k;
+done:
+    free(r); free(z); free(p); free(q);
+    return status;
+}

@@ -58,6 +58,14 @@ def lib():
         L.mas_ref_lambda_max_bound.argtypes = [ctypes.c_void_p]
         L.mas_ref_sts.restype = ctypes.c_int
         L.mas_ref_sts.argtypes = [ctypes.c_void_p, _dp, ctypes.c_double, ctypes.c_int]
+        L.mas_ref_pc2_create.restype = ctypes.c_void_p
+        L.mas_ref_pc2_create.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int]
+        L.mas_ref_pc2_destroy.argtypes = [ctypes.c_void_p]
+        L.mas_ref_pc2_apply.argtypes = [ctypes.c_void_p, _dp, _dp]
+        L.mas_ref_pc2_dense_factors.argtypes = [ctypes.c_void_p, _dp, _dp]
+        L.mas_ref_pcg_pc2.restype = ctypes.c_int
+        L.mas_ref_pcg_pc2.argtypes = [ctypes.c_void_p, ctypes.c_void_p, _dp, _dp, ctypes.c_double, ctypes.c_int,
+                                      ctypes.POINTER(ctypes.c_int), _dp]
         _lib = L
     return _lib
 
@@ -154,6 +162,21 @@ class RefOperator:
             raise ValueError(f"mas_ref_sts status {st}")
         return y
 
+    # ---- NEXT-4: PC2, block-Jacobi ILU(0) ----
+    def pc2(self, boxes=(0, 0, 0)) -> "RefPc2":
+        """The block-Jacobi ILU(0) preconditioner of this operator AT ITS CURRENT dt; boxes = (bi, bj, bk) cells
+        per box in r, theta, phi (0 = the whole extent)."""
+        return RefPc2(self, boxes)
+
+    def pcg_pc2(self, pc: "RefPc2", b_phys: np.ndarray, x0: np.ndarray | None, rtol: float, maxit: int):
+        """PCG with z = M^-1 r, M = pc.  Returns (status, iters, x, hist[0..iters])."""
+        b = np.ascontiguousarray(b_phys, dtype=np.float64).reshape(self.shape)
+        x = np.zeros(self.shape) if x0 is None else np.array(x0, dtype=np.float64, order="C").reshape(self.shape)
+        hist = np.full(maxit + 1, np.nan)
+        it = ctypes.c_int(0)
+        st = lib().mas_ref_pcg_pc2(self._h, pc._h, _p(b), _p(x), float(rtol), int(maxit), ctypes.byref(it), _p(hist))
+        return st, it.value, x, hist[: it.value + 1].copy()
+
     def dense(self) -> np.ndarray:
         """Dense A_sym, column by column from unit vectors (tiny meshes only)."""
         n = int(np.prod(self.shape))
@@ -165,3 +188,35 @@ class RefOperator:
             A[:, c] = self.apply(e.reshape(self.shape)).ravel()
             e[c] = 0.0
         return A
+
+
+class RefPc2:
+    """PC2: zero-fill ILU of the block-diagonal part of A_sym in a box partition."""
+
+    def __init__(self, op: RefOperator, boxes=(0, 0, 0)):
+        self.shape = op.shape
+        self._h = lib().mas_ref_pc2_create(op._h, int(boxes[0]), int(boxes[1]), int(boxes[2]))
+        if not self._h:
+            raise MemoryError("mas_ref_pc2_create failed")
+
+    def close(self):
+        if self._h:
+            lib().mas_ref_pc2_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def apply(self, r: np.ndarray) -> np.ndarray:
+        """z = M^-1 r."""
+        r = np.ascontiguousarray(r, dtype=np.float64).reshape(self.shape)
+        z = np.empty(self.shape)
+        lib().mas_ref_pc2_apply(self._h, _p(r), _p(z))
+        return z
+
+    def dense_factors(self):
+        """(L, U) as dense n x n arrays (tiny meshes only)."""
+        n = int(np.prod(self.shape))
+        assert n <= 4096
+        Ld, Ud = np.empty((n, n)), np.empty((n, n))
+        lib().mas_ref_pc2_dense_factors(self._h, _p(Ld), _p(Ud))
+        return Ld, Ud

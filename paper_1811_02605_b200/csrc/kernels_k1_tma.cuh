@@ -9,9 +9,10 @@
 //
 // Tiling: tile.cuh.  Data movement per step (= one r plane):
 //   * every warp owns one tile row; lane 0 bulk-copies (cp.async.bulk, SASS UBLKCP) that row's r, p_old, x segments
-//     and the two 16-byte phi-halo pairs of r and p_old for the plane DEPTH steps ahead into the warp's own FIFO
-//     stage, signalling the warp's own mbarrier ldfull[stage][warp] (count 1 + transaction bytes).  A warp waits only
-//     for ITS row -- there is no block-wide coupling on the load path;
+//     for the plane DEPTH steps ahead into the warp's own FIFO stage -- r and p_old with their two phi-halo pairs,
+//     ONE copy per vector when the halo cells are adjacent in memory (tile.cuh row_copy) -- signalling the warp's
+//     own mbarrier ldfull[stage][warp] (count 1 + transaction bytes).  A warp waits only for ITS row -- there is no
+//     block-wide coupling on the load path; source addresses are running offsets bumped by one plane per step;
 //   * p_new planes go to a shared ring of FOUR planes; every thread arrives on ringfull[plane % 4] after storing its
 //     part, and a warp waits for plane t-1 to be complete before reading its theta-neighbours' rows.  With four
 //     buffers that wait also proves the slot written at step t (plane t-4) is no longer being read, so K1 has no
@@ -32,10 +33,9 @@ template <int TJ, int DEPTH, bool UNIFORM>
 struct K1TmaSmem {
     static constexpr int NW = TJ + 2;
     static constexpr int NT = NW * 32;
-    alignas(16) double2 fr[DEPTH][NW][64];                // r rows (tile + theta-halo rows), 128 cells each
-    alignas(16) double2 fp[DEPTH][NW][64];                // p_old rows
+    alignas(16) double2 fr[DEPTH][NW][ROW_V2];            // r rows (tile + theta-halo rows): [halo pair | 128 cells | halo pair]
+    alignas(16) double2 fp[DEPTH][NW][ROW_V2];            // p_old rows, same layout
     alignas(16) double2 fx[DEPTH][TJ][64];                // x rows (interior rows only)
-    alignas(16) double2 fh[DEPTH][NW][4];                 // phi-halo pairs: r left, r right, p left, p right
     alignas(16) double2 ring[4][NW][64];                  // p_new planes
     TileCoefs<NW, UNIFORM> c;
     double red[32];
@@ -56,21 +56,25 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     const TileGeom g = tile_geom<TJ>(op, mp);
     const int lane = g.lane, warp = g.warp, tid = g.tid;
 
+    // 32-bit shared addresses of this warp's barriers and staging rows (stage 0), computed once
+    const unsigned s_ldfull = smem_u32(&sm.ldfull[0][warp]), s_ring = smem_u32(&sm.ringfull[0]);
+    const unsigned s_fr = smem_u32(&sm.fr[0][warp][0]), s_fp = smem_u32(&sm.fp[0][warp][0]);
+    const unsigned s_fx = smem_u32(&sm.fx[0][g.interior ? warp - 1 : 0][0]);
+    constexpr unsigned BAR_STAGE = NW * 8u, ROWS_STAGE = NW * ROW_BYTES, X_STAGE = TJ * 1024u;
+
     // ---- zero-fill and barrier init first, so that the first bulk copies can be issued as early as possible ----
     const double2 zero2 = make_double2(0.0, 0.0);
 #pragma unroll
     for (int s = 0; s < DEPTH; s++) {
-        sm.fr[s][warp][lane] = zero2; sm.fr[s][warp][lane + 32] = zero2;
-        sm.fp[s][warp][lane] = zero2; sm.fp[s][warp][lane + 32] = zero2;
+        for (int e = lane; e < ROW_V2; e += 32) { sm.fr[s][warp][e] = zero2; sm.fp[s][warp][e] = zero2; }
         if (g.interior) { sm.fx[s][warp - 1][lane] = zero2; sm.fx[s][warp - 1][lane + 32] = zero2; }
-        if (lane < 4) sm.fh[s][warp][lane] = zero2;
     }
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < DEPTH; s++)
-            for (int r = 0; r < NW; r++) mbar_init(&sm.ldfull[s][r], 1);
+            for (int r = 0; r < NW; r++) mbar_init(smem_u32(&sm.ldfull[s][r]), 1);
 #pragma unroll
-        for (int s = 0; s < 4; s++) mbar_init(&sm.ringfull[s], NT);
+        for (int s = 0; s < 4; s++) mbar_init(s_ring + 8u * s, NT);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
@@ -96,42 +100,42 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     };
 
     const long long plane = (long long)op.nt * op.np;
-    const long long rowbase0 = (long long)g.first * plane + (g.row_ok ? (long long)g.j * op.np : 0);
+    const long long rowoff = g.row_ok ? (long long)g.j * op.np : 0;
+    const long long rowbase0 = (long long)g.first * plane + rowoff;
     long long prow = rowbase0 + plane;           // row base of plane i0: p_new / x stores
     long long qrow = rowbase0 + plane;           // row base of plane i0: q stores
     const unsigned rowbytes = (unsigned)g.tkeff * 8u;
-    const bool hints = (mp.l2.keep_r | mp.l2.keep_p | mp.l2.first_x) != 0;
-    const uint64_t pol_last = hints ? l2_policy_evict_last() : 0, pol_first = hints ? l2_policy_evict_first() : 0;
+    const bool fx = mp.l2.first_x != 0;
+    const uint64_t pol_first = fx ? l2_policy_evict_first() : 0;
 
-    // lane 0: this warp's row of plane index pl -> FIFO stage pl % DEPTH
-    auto produce = [&](int pl) {
-        const int stage = pl % DEPTH, ii = g.first + pl;
-        uint64_t *bar = &sm.ldfull[stage][warp];
-        const double *rrow = g.row_ok ? plane_row(rV, op, ii, g.j) : nullptr;
-        const double *prw = g.row_ok ? plane_row(pV, op, ii, g.j) : nullptr;
-        const bool in = rrow != nullptr;
-        const bool xin = in && g.interior && ii >= g.i0 && ii < g.i1;
-        const unsigned bytes = in ? (2u * rowbytes + (g.interior ? 64u : 0u) + (xin ? rowbytes : 0u)) : 0u;
-        if (bytes == 0) { mbar_arrive(bar); return; }
-        mbar_arrive_expect_tx(bar, bytes);
-        if (hints && ii < mp.l2.keep_r) bulk_g2s_hint(&sm.fr[stage][warp][0], rrow + g.k0, rowbytes, bar, pol_last);
-        else bulk_g2s(&sm.fr[stage][warp][0], rrow + g.k0, rowbytes, bar);
-        if (hints && ii < mp.l2.keep_p) bulk_g2s_hint(&sm.fp[stage][warp][0], prw + g.k0, rowbytes, bar, pol_last);
-        else bulk_g2s(&sm.fp[stage][warp][0], prw + g.k0, rowbytes, bar);
-        if (g.interior) {
-            bulk_g2s(&sm.fh[stage][warp][0], rrow + (g.kl - 1), 16u, bar);
-            bulk_g2s(&sm.fh[stage][warp][1], rrow + g.kr, 16u, bar);
-            bulk_g2s(&sm.fh[stage][warp][2], prw + (g.kl - 1), 16u, bar);
-            bulk_g2s(&sm.fh[stage][warp][3], prw + g.kr, 16u, bar);
+    // lane 0: this warp's row of plane index pl -> FIFO stage `stage`.  `src` is the running offset (cell k0 of this
+    // warp's row in plane first + pl of the own vectors), bumped by one plane per call: no multiplications here.
+    long long src = rowbase0 + g.k0;
+    const unsigned tx_rows = 2u * (rowbytes + 32u);
+    auto produce = [&](int pl, int stage) {
+        const unsigned bar = s_ldfull + BAR_STAGE * stage;
+        const int ii = g.first + pl;
+        const double *rrow, *prw;
+        if (ii >= 0 && ii < op.nr) { rrow = rV.own + src; prw = pV.own + src; }
+        else {                                                  // the adjacent plane of a neighbour slab, or nothing
+            const double *rh = ii < 0 ? rV.lo : rV.hi, *phh = ii < 0 ? pV.lo : pV.hi;
+            rrow = rh ? rh + rowoff + g.k0 : nullptr;
+            prw = phh ? phh + rowoff + g.k0 : nullptr;
         }
+        const bool xin = g.interior && pl >= 1 && pl <= g.nsteps - 2;
+        const long long xoff = src;
+        src += plane;
+        if (!g.row_ok || !rrow) { mbar_arrive(bar); return; }
+        mbar_arrive_expect_tx(bar, xin ? tx_rows + rowbytes : tx_rows);
+        row_copy(s_fr + ROWS_STAGE * stage, rrow, g, rowbytes, bar);
+        row_copy(s_fp + ROWS_STAGE * stage, prw, g, rowbytes, bar);
         if (xin) {
-            const double *xrow = xvec + (long long)ii * plane + (long long)g.j * op.np + g.k0;
-            if (hints && mp.l2.first_x) bulk_g2s_hint(&sm.fx[stage][warp - 1][0], xrow, rowbytes, bar, pol_first);
-            else bulk_g2s(&sm.fx[stage][warp - 1][0], xrow, rowbytes, bar);
+            if (fx) bulk_g2s_hint(s_fx + X_STAGE * stage, xvec + xoff, rowbytes, bar, pol_first);
+            else bulk_g2s(s_fx + X_STAGE * stage, xvec + xoff, rowbytes, bar);
         }
     };
     if (lane == 0)
-        for (int pl = 0; pl < DEPTH && pl < g.nsteps; pl++) produce(pl);
+        for (int pl = 0; pl < DEPTH && pl < g.nsteps; pl++) produce(pl, pl);
 
     // ---- coefficient columns and phi factors, staged while the first planes are already in flight ----
     const PlaneSetDev ps = {op.E, op.F, op.AR, op.AT, op.Dinv};
@@ -141,18 +145,21 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
     double acc = 0.0;
+    int stage = 0;                              // t % DEPTH
 
     for (int t = 0; t < g.nsteps; t++) {
-        const int stage = t % DEPTH, rs = t & 3, rsp = (t + 3) & 3;
+        const int rs = t & 3, rsp = (t + 3) & 3;
         const int ii = g.first + t;
         const bool plane_ok = (unsigned)(op.i_lo + ii) < (unsigned)op.nr_glob;
+        const bool own = t >= 1 && t <= g.nsteps - 2;       // a plane of this block: p_new and x are stored
         const double En = sm.c.cE[t][warp], Fn = sm.c.cF[t][warp], dinv = sm.c.cD[t][warp];
-        mbar_wait(&sm.ldfull[stage][warp], (unsigned)(t / DEPTH) & 1u, fault);      // this warp's row of plane ii
+        mbar_wait(s_ldfull + BAR_STAGE * stage, (unsigned)(t / DEPTH) & 1u, fault);   // this warp's row of plane ii
         double2 an = zero2, bn = zero2;
         double hl_n = 0.0, hr_n = 0.0;
         if (plane_ok) {
-            const double2 ra = sm.fr[stage][warp][lane], rb = sm.fr[stage][warp][lane + 32];
-            const double2 pa = sm.fp[stage][warp][lane], pb = sm.fp[stage][warp][lane + 32];
+            const double2 *fr = sm.fr[stage][warp], *fp = sm.fp[stage][warp];
+            const double2 ra = fr[1 + lane], rb = fr[33 + lane];
+            const double2 pa = fp[1 + lane], pb = fp[33 + lane];
             if (UNIFORM || g.vA) {
                 an.x = fma(beta, pa.x, zval(ra.x, En, Fn, dinv, ea));
                 an.y = fma(beta, pa.y, zval(ra.y, En, Fn, dinv, ea + 1));
@@ -161,33 +168,32 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
                 bn.x = fma(beta, pb.x, zval(rb.x, En, Fn, dinv, eb));
                 bn.y = fma(beta, pb.y, zval(rb.y, En, Fn, dinv, eb + 1));
             }
-            if (g.left_edge) hl_n = fma(beta, sm.fh[stage][warp][2].y, zval(sm.fh[stage][warp][0].y, En, Fn, dinv, 0));
-            if (g.right_edge) hr_n = fma(beta, sm.fh[stage][warp][3].x, zval(sm.fh[stage][warp][1].x, En, Fn, dinv, g.tkeff + 1));
-            if (t >= 1 && t <= g.nsteps - 2) {  // interior plane: store p_new and the deferred x-update
-                const bool keep_p = hints && ii < mp.l2.keep_p, fx = hints && mp.l2.first_x;
+            if (g.left_edge) hl_n = fma(beta, fp[0].y, zval(fr[0].y, En, Fn, dinv, 0));
+            if (g.right_edge) hr_n = fma(beta, fp[g.hr].x, zval(fr[g.hr].x, En, Fn, dinv, g.tkeff + 1));
+            if (own) {                          // store p_new and the deferred x-update
                 if (g.qA) {
-                    if (keep_p) st2_hint(pout, prow + g.ka, an, pol_last); else st2g(pout, prow + g.ka, an);
+                    st2g(pout, prow + g.ka, an);
                     double2 xa = sm.fx[stage][warp - 1][lane];
                     xa.x = fma(alpha_prev, pa.x, xa.x); xa.y = fma(alpha_prev, pa.y, xa.y);
                     if (fx) st2_hint(xvec, prow + g.ka, xa, pol_first); else st2g(xvec, prow + g.ka, xa);
                 }
                 if (g.qB) {
-                    if (keep_p) st2_hint(pout, prow + g.kb, bn, pol_last); else st2g(pout, prow + g.kb, bn);
+                    st2g(pout, prow + g.kb, bn);
                     double2 xb = sm.fx[stage][warp - 1][lane + 32];
                     xb.x = fma(alpha_prev, pb.x, xb.x); xb.y = fma(alpha_prev, pb.y, xb.y);
                     if (fx) st2_hint(xvec, prow + g.kb, xb, pol_first); else st2g(xvec, prow + g.kb, xb);
                 }
             }
         }
-        if (t >= 1 && t <= g.nsteps - 2) prow += plane;
+        if (own) prow += plane;
         __syncwarp();                                        // the warp is done with its FIFO stage
-        if (lane == 0 && t + DEPTH < g.nsteps) produce(t + DEPTH);
+        if (lane == 0 && t + DEPTH < g.nsteps) produce(t + DEPTH, stage);
         // ---- publish p_new of plane ii; wait for plane ii-1 of the whole tile ----
         sm.ring[rs][warp][lane] = an;
         sm.ring[rs][warp][lane + 32] = bn;
-        mbar_arrive(&sm.ringfull[rs]);                       // every thread: its own stores are released
+        mbar_arrive(s_ring + 8u * rs);                       // every thread: its own stores are released
         const PhiNb nb = phi_neighbours(ac, bc, lane);
-        if (t >= 1) mbar_wait(&sm.ringfull[rsp], (unsigned)((t - 1) >> 2) & 1u, fault);
+        if (t >= 1) mbar_wait(s_ring + 8u * rsp, (unsigned)((t - 1) >> 2) & 1u, fault);
         // ---- q for plane i = ii-1 ----
         if (t >= 2 && g.interior && g.row_ok) {
             const RowCoefs rc = row_coefs(sm.c, t, warp);
@@ -211,6 +217,7 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
         if (t >= 2) qrow += plane;
         am = ac; ac = an; bm = bc; bc = bn;
         hl_c = hl_n; hr_c = hr_n;
+        stage = stage + 1 == DEPTH ? 0 : stage + 1;
     }
     double a1[1] = {acc};
     if (grid_sum<NT, 1>(a1, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 1], sm.red) && threadIdx.x == 0)
@@ -222,7 +229,7 @@ struct K1TmaTile {
     int tj, depth, minb;
 };
 static const K1TmaTile kK1TmaTiles[] = {{14, 2, 1}, {8, 2, 2}, {6, 2, 2}, {8, 3, 1}, {10, 2, 1}, {16, 2, 1}, {12, 2, 1},
-                                          {8, 4, 1}, {14, 3, 1}, {6, 3, 2}, {10, 3, 1}, {12, 3, 1}};
+                                          {8, 4, 1}, {6, 3, 2}, {10, 3, 1}, {12, 3, 1}};
 inline int k1_tma_num_tiles() { return (int)(sizeof(kK1TmaTiles) / sizeof(kK1TmaTiles[0])); }
 
 template <int TJ, int DEPTH, int MINB>
@@ -250,9 +257,8 @@ inline void k1_tma_configure(int nr, int nt, int np, int uniform, bool noq, int 
         case 5: k1_tma_pick<16, 2, 1>(uniform, noq, func, block, smem); break;
         case 6: k1_tma_pick<12, 2, 1>(uniform, noq, func, block, smem); break;
         case 7: k1_tma_pick<8, 4, 1>(uniform, noq, func, block, smem); break;
-        case 8: k1_tma_pick<14, 3, 1>(uniform, noq, func, block, smem); break;
-        case 9: k1_tma_pick<6, 3, 2>(uniform, noq, func, block, smem); break;
-        case 10: k1_tma_pick<10, 3, 1>(uniform, noq, func, block, smem); break;
+        case 8: k1_tma_pick<6, 3, 2>(uniform, noq, func, block, smem); break;
+        case 9: k1_tma_pick<10, 3, 1>(uniform, noq, func, block, smem); break;
         default: k1_tma_pick<12, 3, 1>(uniform, noq, func, block, smem); break;
     }
     mp->nkt = (np + TILE_TK - 1) / TILE_TK;
@@ -262,7 +268,7 @@ inline void k1_tma_configure(int nr, int nt, int np, int uniform, bool noq, int 
         cudaGetLastError();
         occ = 1;
     }
-    mp->ci = tile_pick_ci(nr, (long long)mp->nkt * mp->njt, (long long)num_sms * occ, ny, ci_force);
+    mp->ci = tile_pick_ci(nr, (long long)mp->nkt * mp->njt, (long long)num_sms * occ, ci_force);
     mp->nit = (nr + mp->ci - 1) / mp->ci;
     *grid = dim3((unsigned)(mp->nkt * mp->njt * mp->nit), (unsigned)ny);
 }

@@ -45,8 +45,7 @@ struct StencilTmaSmem {
     static constexpr int NW = TJ + 2;
     static constexpr int NT = NW * 32;
     static constexpr int R = DEPTH + 2;
-    alignas(16) double2 ring[R][NW][64];                 // [slot][row][128 cells]
-    alignas(16) double2 halo[R][NW][2];                  // [slot][row][left pair (kl-1, kl) | right pair (kr, kr+1)]
+    alignas(16) double2 ring[R][NW][ROW_V2];             // [slot][row][left halo pair | 128 cells | right halo pair]
     alignas(16) double2 xf[NX ? DEPTH : 1][NX ? NX : 1][NX ? TJ : 1][NX ? 64 : 1];   // [stage][stream][interior row][128 cells]
     TileCoefs<NW, UNIFORM> c;
     double red[32];
@@ -92,16 +91,19 @@ k_stencil_tma(OpDev op, StencilParams mp)
     const double *x1p = EPI == EPI_K2R ? rvec : mp.a1;           // K2R: the one extra stream is r
     int *fault = mp.fault;
 
+    // 32-bit shared addresses of the barriers and of this warp's rows (slot / stage 0), computed once
+    const unsigned s_full = smem_u32(&sm.full[0]), s_empty = smem_u32(&sm.empty[0]);
+    const unsigned s_ring = smem_u32(&sm.ring[0][warp][0]);
+    const unsigned s_xf = smem_u32(&sm.xf[0][0][NX && g.interior ? warp - 1 : 0][0]);
+    constexpr unsigned SLOT_BYTES = NW * ROW_BYTES, XSTREAM = (NX ? TJ : 1) * 1024u, XSTAGE = (NX ? NX : 1) * XSTREAM;
+
     // ---- zero the ring, init the barriers, start the first planes, then stage the coefficient columns ----
 #pragma unroll
-    for (int s = 0; s < R; s++) {
-        sm.ring[s][warp][lane] = make_double2(0.0, 0.0);
-        sm.ring[s][warp][lane + 32] = make_double2(0.0, 0.0);
-        if (lane < 2) sm.halo[s][warp][lane] = make_double2(0.0, 0.0);
-    }
+    for (int s = 0; s < R; s++)
+        for (int e = lane; e < ROW_V2; e += 32) sm.ring[s][warp][e] = make_double2(0.0, 0.0);
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < R; s++) { mbar_init(&sm.full[s], NW); mbar_init(&sm.empty[s], NW); }
+        for (int s = 0; s < R; s++) { mbar_init(s_full + 8u * s, NW); mbar_init(s_empty + 8u * s, NW); }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");   // inits visible to the async proxy
     }
     // the zero-fill above was written through the generic proxy; the bulk copies write through the async proxy
@@ -111,47 +113,42 @@ k_stencil_tma(OpDev op, StencilParams mp)
     const PhiFac<UNIFORM, TileCoefs<NW, UNIFORM>> ph = {sm.c, mp.t.vp, mp.t.wp, mp.t.ip};
     const int ea = 2 * lane + 1, eb = 2 * lane + 65;
     const long long plane = (long long)op.nt * op.np;
-    const long long rowbase0 = (long long)g.first * plane + (g.row_ok ? (long long)g.j * op.np : 0);
+    const long long rowoff = g.row_ok ? (long long)g.j * op.np : 0;
+    const long long rowbase0 = (long long)g.first * plane + rowoff;
     long long orow = rowbase0 + plane;                      // row base of plane i0: outputs
     const bool has1 = (EPI == EPI_STS && mp.a1 != nullptr) || EPI == EPI_K2R,
                has2 = EPI == EPI_STS && mp.a2 != nullptr, has3 = EPI == EPI_STS && mp.a3 != nullptr;
     const unsigned rowbytes = (unsigned)g.tkeff * 8u;
-    const bool hints = EPI == EPI_K2R && (mp.t.l2.keep_r | mp.t.l2.keep_p) != 0;
-    const uint64_t pol_last = hints ? l2_policy_evict_last() : 0;
+    const unsigned tx_u = rowbytes + 32u;
+    const unsigned tx_x = rowbytes * ((has1 ? 1u : 0u) + (has2 ? 1u : 0u) + (has3 ? 1u : 0u));
 
-    // lane 0 of each warp: load THIS warp's row of plane index pl (ring plane first+pl) and, for interior rows,
-    // the extras of the plane whose outputs are formed when that ring plane is consumed (first+pl-1).
-    auto produce = [&](int pl) {
-        const int slot = pl % R, ii = g.first + pl;
-        uint64_t *bar = &sm.full[slot];
-        unsigned bytes = 0;
-        const double *urow = g.row_ok ? plane_row(uV, op, ii, g.j) : nullptr;
-        if (urow) bytes += rowbytes + (g.interior ? 32u : 0u);
-        const bool xin = NX > 0 && g.interior && g.row_ok && (ii - 1 >= g.i0) && (ii - 1 < g.i1);
-        if (xin) bytes += rowbytes * ((has1 ? 1u : 0u) + (has2 ? 1u : 0u) + (has3 ? 1u : 0u));
+    // lane 0 of each warp: load THIS warp's row of plane index pl (ring plane first+pl) into `slot` and, for interior
+    // rows, the extras of the plane whose outputs are formed when that ring plane is consumed (first+pl-1) into
+    // `xs`.  `src` = running offset of cell k0 of this warp's row in plane first + pl (bumped by a plane per call).
+    long long src = rowbase0 + g.k0;
+    auto produce = [&](int pl, int slot, int xs) {
+        const unsigned bar = s_full + 8u * slot;
+        const int ii = g.first + pl;
+        const double *urow;
+        if (ii >= 0 && ii < op.nr) urow = uV.own + src;
+        else { const double *h = ii < 0 ? uV.lo : uV.hi; urow = h ? h + rowoff + g.k0 : nullptr; }
+        const long long xoff = src - plane;
+        src += plane;
+        if (!g.row_ok) urow = nullptr;
+        const bool xin = NX > 0 && g.interior && g.row_ok && pl >= 2 && pl <= g.nsteps - 1 && tx_x != 0;
+        const unsigned bytes = (urow ? tx_u : 0u) + (xin ? tx_x : 0u);
         if (bytes == 0) { mbar_arrive(bar); return; }
         mbar_arrive_expect_tx(bar, bytes);
-        if (urow) {
-            if (hints && ii < mp.t.l2.keep_p) bulk_g2s_hint(&sm.ring[slot][warp][0], urow + g.k0, rowbytes, bar, pol_last);
-            else bulk_g2s(&sm.ring[slot][warp][0], urow + g.k0, rowbytes, bar);
-            if (g.interior) {
-                bulk_g2s(&sm.halo[slot][warp][0], urow + (g.kl - 1), 16u, bar);
-                bulk_g2s(&sm.halo[slot][warp][1], urow + g.kr, 16u, bar);
-            }
-        }
+        if (urow) row_copy(s_ring + SLOT_BYTES * slot, urow, g, rowbytes, bar);
         if (xin) {
-            const int xs = pl % DEPTH;
-            const long long xb = (long long)(ii - 1) * plane + (long long)g.j * op.np + g.k0;
-            if (has1) {
-                if (hints && ii - 1 < mp.t.l2.keep_r) bulk_g2s_hint(&sm.xf[xs][0][warp - 1][0], x1p + xb, rowbytes, bar, pol_last);
-                else bulk_g2s(&sm.xf[xs][0][warp - 1][0], x1p + xb, rowbytes, bar);
-            }
-            if (has2) bulk_g2s(&sm.xf[xs][NX > 1 ? 1 : 0][warp - 1][0], mp.a2 + xb, rowbytes, bar);
-            if (has3) bulk_g2s(&sm.xf[xs][NX > 2 ? 2 : 0][warp - 1][0], mp.a3 + xb, rowbytes, bar);
+            const unsigned dst = s_xf + XSTAGE * xs;
+            if (has1) bulk_g2s(dst, x1p + xoff, rowbytes, bar);
+            if (has2) bulk_g2s(dst + (NX > 1 ? XSTREAM : 0u), mp.a2 + xoff, rowbytes, bar);
+            if (has3) bulk_g2s(dst + (NX > 2 ? 2u * XSTREAM : 0u), mp.a3 + xoff, rowbytes, bar);
         }
     };
     if (lane == 0)
-        for (int pl = 0; pl < DEPTH && pl < g.nsteps; pl++) produce(pl);
+        for (int pl = 0; pl < DEPTH && pl < g.nsteps; pl++) produce(pl, pl, pl);
 
     stage_coefs<TJ, UNIFORM>(sm.c, g, op, mp.ps);
     __syncthreads();                                        // coefficient columns visible
@@ -160,29 +157,30 @@ k_stencil_tma(OpDev op, StencilParams mp)
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
     double acc[2] = {0.0, 0.0};                             // K2R: rho', rr
+    int slot = 0, slot_prev = R - 1, xs = 0;                // t % R, (t - 1) % R, t % DEPTH
+    int pslot = DEPTH, puse = 0;                            // (t + DEPTH) % R and (t + DEPTH) / R: slot of the plane produced at step t, and which use of that slot it is
+    unsigned full_par = 0;                                  // (t / R) & 1
 
     for (int t = 0; t < g.nsteps; t++) {
-        const int slot = t % R, slot_prev = (t + R - 1) % R;
         const int ii = g.first + t;
         const bool plane_ok = (unsigned)(op.i_lo + ii) < (unsigned)op.nr_glob;
-        mbar_wait(&sm.full[slot], (unsigned)(t / R) & 1u, fault);   // plane ii: every row has landed
+        mbar_wait(s_full + 8u * slot, full_par, fault);     // plane ii: every row has landed
         double2 an = zero2, bn = zero2;
         double hl_n = 0.0, hr_n = 0.0;
         if (plane_ok) {
-            an = sm.ring[slot][warp][lane];
-            bn = sm.ring[slot][warp][lane + 32];
-            if (g.left_edge) hl_n = sm.halo[slot][warp][0].y;
-            if (g.right_edge) hr_n = sm.halo[slot][warp][1].x;
+            const double2 *row = sm.ring[slot][warp];
+            an = row[1 + lane];
+            bn = row[33 + lane];
+            if (g.left_edge) hl_n = row[0].y;
+            if (g.right_edge) hr_n = row[g.hr].x;
         }
         const PhiNb nb = phi_neighbours(ac, bc, lane);
         if (t >= 2 && g.interior && g.row_ok) {
             const RowCoefs rc = row_coefs(sm.c, t, warp);
             const double dsc = EPI != EPI_APPLY ? sm.c.cD[t - 1][warp] : 0.0;      // 1/V2 (STS) or Dinv (K2R)
-            const int xs = t % DEPTH;
             auto finish = [&](double2 s, double2 uc, int half, int e, int kcell) {
                 double2 o;
                 const int xi = lane + 32 * half;
-                const bool keep = hints && (ii - 1) < mp.t.l2.keep_r;
                 if (EPI == EPI_APPLY) {
                     o = s;
                 } else if (EPI == EPI_K2R) {                     // s = q = A p;  stream 0 = r
@@ -205,36 +203,38 @@ k_stencil_tma(OpDev op, StencilParams mp)
                     if (has2) { const double2 x2 = sm.xf[xs][NX > 1 ? 1 : 0][warp - 1][xi]; o.x = fma(mp.c_a2, x2.x, o.x); o.y = fma(mp.c_a2, x2.y, o.y); }
                     if (has3) { const double2 x3 = sm.xf[xs][NX > 2 ? 2 : 0][warp - 1][xi]; o.x = fma(mp.c_a3, x3.x, o.x); o.y = fma(mp.c_a3, x3.y, o.y); }
                 }
-                if (keep) st2_hint(out, orow + kcell, o, pol_last); else st2g(out, orow + kcell, o);
+                st2g(out, orow + kcell, o);
             };
             if (g.qA) {
                 const double ukm = g.left_edge ? hl_c : nb.mA;
                 const double ukp = g.right_A ? hr_c : (lane == 31 ? nb.pB : nb.pA);
-                const double2 s = stencil_half(ph, ea, rc, am, ac, an, sm.ring[slot_prev][warp - 1][lane],
-                                               sm.ring[slot_prev][warp + 1][lane], ukm, ukp);
+                const double2 s = stencil_half(ph, ea, rc, am, ac, an, sm.ring[slot_prev][warp - 1][1 + lane],
+                                               sm.ring[slot_prev][warp + 1][1 + lane], ukm, ukp);
                 finish(s, ac, 0, ea, g.ka);
             }
             if (g.qB) {
                 const double ukm = lane == 0 ? nb.mA : nb.mB;
                 const double ukp = g.right_B ? hr_c : nb.pB;
-                const double2 s = stencil_half(ph, eb, rc, bm, bc, bn, sm.ring[slot_prev][warp - 1][lane + 32],
-                                               sm.ring[slot_prev][warp + 1][lane + 32], ukm, ukp);
+                const double2 s = stencil_half(ph, eb, rc, bm, bc, bn, sm.ring[slot_prev][warp - 1][33 + lane],
+                                               sm.ring[slot_prev][warp + 1][33 + lane], ukm, ukp);
                 finish(s, bc, 1, eb, g.kb);
             }
         }
         if (t >= 2) orow += plane;
         __syncwarp();                                       // the warp's reads of slot_prev and of its extras are done
         if (lane == 0) {
-            if (t >= 1) mbar_arrive(&sm.empty[slot_prev]);  // plane t-1 released by this warp
-            const int pl = t + DEPTH;                       // refill: plane pl goes to the slot plane pl-R used
-            if (pl < g.nsteps) {
-                const int use = pl / R;                     // n-th use of that slot
-                if (use >= 1) mbar_wait(&sm.empty[pl % R], (unsigned)(use - 1) & 1u, fault);
-                produce(pl);
+            if (t >= 1) mbar_arrive(s_empty + 8u * slot_prev);   // plane t-1 released by this warp
+            if (t + DEPTH < g.nsteps) {                     // refill: plane t+DEPTH goes to the slot plane t+DEPTH-R used
+                if (puse >= 1) mbar_wait(s_empty + 8u * pslot, (unsigned)(puse - 1) & 1u, fault);
+                produce(t + DEPTH, pslot, xs);
             }
         }
         am = ac; ac = an; bm = bc; bc = bn;
         hl_c = hl_n; hr_c = hr_n;
+        slot_prev = slot;
+        if (++slot == R) { slot = 0; full_par ^= 1u; }
+        if (++pslot == R) { pslot = 0; ++puse; }
+        if (++xs == DEPTH) xs = 0;
     }
     if (EPI == EPI_K2R) {
         if (grid_sum<NT, 2>(acc, part_base(mp.w, rhs), mp.w.pstride, &mp.w.tickets[rhs * 4 + 2], sm.red) && threadIdx.x == 0)
@@ -293,7 +293,7 @@ inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int 
         cudaGetLastError();
         occ = 1;
     }
-    mp->t.ci = tile_pick_ci(nr, (long long)mp->t.nkt * mp->t.njt, (long long)num_sms * occ, ny, ci_force);
+    mp->t.ci = tile_pick_ci(nr, (long long)mp->t.nkt * mp->t.njt, (long long)num_sms * occ, ci_force);
     mp->t.nit = (nr + mp->t.ci - 1) / mp->t.ci;
     *grid = dim3((unsigned)(mp->t.nkt * mp->t.njt * mp->t.nit), (unsigned)ny);
 }

@@ -105,7 +105,7 @@ struct mas_pcg {
     int coop_ok = 0, coop_refused = 0;
     int unroll = 4;                  // PCG iterations per WHILE trip of the graph loop (measured: +1 % c4, +3 % c3)
     int qrecompute = 1;              // 1: q is not stored, K2R recomputes it: 64 B/cell/iteration; 0: 72 B
-    L2Plan l2{0, 0, 0};
+    L2Plan l2{0};
     cudaGraph_t graph[MAX_RHS] = {};
     cudaGraphExec_t exec[MAX_RHS] = {};
     long long stats[8] = {};
@@ -779,12 +779,6 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
     } else if (!strcmp(name, "ci")) {
         if (value != 0 && (value < CI_FORCE_MIN || value > TILE_CI_MAX)) return MAS_EINVAL;
         h->ci_force = value;
-    } else if (!strcmp(name, "l2_keep_r")) {
-        if (value < 0) return MAS_EINVAL;
-        h->l2.keep_r = value;
-    } else if (!strcmp(name, "l2_keep_p")) {
-        if (value < 0) return MAS_EINVAL;
-        h->l2.keep_p = value;
     } else if (!strcmp(name, "l2_first_x")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->l2.first_x = value;

@@ -22,30 +22,33 @@ constexpr int TILE_NPL = TILE_CI_MAX + 2;
 // PTX: mbarrier, bulk copy, L2 policies
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+// Barriers and bulk-copy destinations are addressed by their 32-bit shared-memory address, computed once per kernel:
+// the generic -> shared conversion per call was 6 % of the stencil kernel's instructions (ncu, round 2).
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
 {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+__device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, unsigned bytes)
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes)
 {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
 }
 // try_wait suspends the warp in hardware for a bounded time (it is not a busy poll), then reports the phase
-__device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, unsigned parity)
+__device__ __forceinline__ bool mbar_try_wait(unsigned bar, unsigned parity)
 {
     unsigned ok;
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
-                 : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
 // Wait for a phase.  A wait that is still unsatisfied after MBAR_TIMEOUT_NS of wall time (%globaltimer, so that
 // time-slicing, a debugger or a profiler replay cannot trip it the way an iteration count can) is a protocol error:
 // it is reported through *fault (the host turns it into MAS_ECUDA) and the wait is abandoned -- no __trap(), which
-// would poison the CUDA context for every handle in the process.
+// would poison the CUDA context for every handle in the process.  The clock is read once per 1024 failed polls only:
+// reading it on every poll cost 4 % of K1's and 8 % of K2R's instructions (ncu, round 2).
 constexpr unsigned long long MBAR_TIMEOUT_NS = 20ull * 1000 * 1000 * 1000;
 __device__ __forceinline__ unsigned long long globaltimer_ns()
 {
@@ -53,37 +56,43 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     asm volatile("mov.u64 %0, %%globaltimer;\n" : "=l"(t));
     return t;
 }
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity, int *fault)
+__device__ __noinline__ void mbar_wait_slow(unsigned bar, unsigned parity, int *fault)
+{
+    unsigned long long t0 = 0;
+    for (unsigned polls = 1;; polls++) {
+        if (mbar_try_wait(bar, parity)) return;
+        if ((polls & 1023u) == 0) {
+            const unsigned long long t = globaltimer_ns();
+            if (t0 == 0) t0 = t;
+            else if (t - t0 > MBAR_TIMEOUT_NS) { *fault = 1; return; }
+        }
+    }
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity, int *fault)
 {
     if (mbar_try_wait(bar, parity)) return;
-    const unsigned long long t0 = globaltimer_ns();
-    while (!mbar_try_wait(bar, parity))
-        if (globaltimer_ns() - t0 > MBAR_TIMEOUT_NS) {
-            *fault = 1;
-            return;
-        }
+    if (mbar_try_wait(bar, parity)) return;
+    mbar_wait_slow(bar, parity, fault);
 }
-__device__ __forceinline__ uint64_t l2_policy_evict_last()
-{
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;\n" : "=l"(p));
-    return p;
-}
+// x is read once and written once per iteration and never reused inside it: its accesses may carry the L2
+// evict_first priority so that they do not displace r and p.  evict_last hints are NOT used: on
+// this pool's B200s every access carrying an evict_last policy (created by createpolicy or given as the constant
+// CUTLASS uses) ended the kernel with "unspecified launch failure" (gpurun, round 2); evict_first works.
 __device__ __forceinline__ uint64_t l2_policy_evict_first()
 {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;\n" : "=l"(p));
     return p;
 }
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, uint64_t *bar)
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s_hint(void *dst, const void *src, unsigned bytes, uint64_t *bar, uint64_t pol)
+__device__ __forceinline__ void bulk_g2s_hint(unsigned dst, const void *src, unsigned bytes, unsigned bar, uint64_t pol)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;\n"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(pol) : "memory");
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void st2_hint(double *p, long long cell, double2 v, uint64_t pol)
 {
@@ -98,13 +107,9 @@ __device__ __forceinline__ void st2g(double *p, long long cell, double2 v)
     *reinterpret_cast<double2 *>(p + cell) = v;
 }
 
-// L2 residency plan of a launch: accesses to the first `keep` planes of the vector named in the
-// kernel are issued with evict_last priority, so that this part of the vector stays in the 126 MB L2 from one kernel to
-// the next; every other access of the kernels that take a plan is plain.  keep = 0: no hints at all.
+// L2 plan of a launch: first_x = 1: x is streamed with evict_first (see above); 0: no hints at all.
 struct L2Plan {
-    int keep_r;                              // planes [0, keep_r) of r
-    int keep_p;                              // planes [0, keep_p) of p (both ping-pong buffers)
-    int first_x;                             // 1: x is streamed with evict_first
+    int first_x;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -123,6 +128,8 @@ struct TileGeom {
     int j, k0, tkeff, kl, kr;                // this warp's theta row; first phi cell; valid cells; periodic halo cells
     int ka, kb;                              // first cell of this lane's A and B vectors
     bool row_ok, vA, vB, interior, qA, qB, left_edge, right_A, right_B, right_edge;
+    bool wrapless;                           // the two phi-halo pairs are adjacent in memory to the row segment
+    int hr;                                  // index of the right halo pair in a staged row (1 + tkeff/2)
 };
 
 template <int TJ>
@@ -149,6 +156,8 @@ __device__ __forceinline__ TileGeom tile_geom(const OpDev &op, const TileParams 
     g.kl = g.k0 == 0 ? op.np - 1 : g.k0 - 1;                    // odd (k0 and np are even)
     g.kr = g.k0 + g.tkeff >= op.np ? 0 : g.k0 + g.tkeff;        // even
     g.ka = g.k0 + 2 * g.lane; g.kb = g.ka + 64;
+    g.wrapless = g.k0 > 0 && g.k0 + g.tkeff < op.np;
+    g.hr = 1 + g.tkeff / 2;
     return g;
 }
 
@@ -165,6 +174,24 @@ __device__ __forceinline__ const double *plane_row(const VecHalo &v, const OpDev
     if (ii == -1) return v.lo ? v.lo + rowoff : nullptr;
     if (ii == op.nr) return v.hi ? v.hi + rowoff : nullptr;
     return nullptr;
+}
+
+// A tile row as it is staged in shared memory: ROW_V2 double2 = [left phi-halo pair | 128 cells | right pair]; the
+// pairs are (kl-1, kl) and (kr, kr+1), so the halo cells are .y of element 0 and .x of element g.hr.  A lane's A / B
+// vectors are elements 1 + lane and 33 + lane.  When the halo pairs are adjacent in memory to the segment (no periodic
+// wrap inside this tile) the whole row is ONE bulk copy, otherwise three -- issued by one lane, `row_k0` = address of
+// cell k0 of the row.  (Round 2: five separate copies per vector and row were 21 % of K1's instructions.)
+constexpr int ROW_V2 = 66;
+constexpr unsigned ROW_BYTES = ROW_V2 * 16;
+__device__ __forceinline__ void row_copy(unsigned dst, const double *row_k0, const TileGeom &g, unsigned rowbytes, unsigned bar)
+{
+    if (g.wrapless) {
+        bulk_g2s(dst, row_k0 - 2, rowbytes + 32u, bar);
+    } else {
+        bulk_g2s(dst + 16u, row_k0, rowbytes, bar);
+        bulk_g2s(dst, row_k0 + (g.kl - 1 - g.k0), 16u, bar);
+        bulk_g2s(dst + 16u + rowbytes, row_k0 + (g.kr - g.k0), 16u, bar);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -259,13 +286,15 @@ __device__ __forceinline__ PhiNb phi_neighbours(double2 ac, double2 bc, int lane
 }
 
 // r-chunk length of a marching kernel: minimise rounds x (planes per block + halo planes + start-up), ties ->
-// longer chunks.  `nslots` = blocks resident at once; `ny` = gridDim.y (right-hand sides) sharing the SMs.
-inline int tile_pick_ci(int nr, long long cols, long long nslots, int ny, int ci_force)
+// longer chunks.  `nslots` = blocks resident at once.  The choice must NOT depend on the number of right-hand sides
+// of a batched solve: the chunk length fixes the grid and with it the order of the partial sums, and a batched
+// solve is promised to be bit-identical to single solves.
+inline int tile_pick_ci(int nr, long long cols, long long nslots, int ci_force)
 {
     int best = TILE_CI_MAX;
     double best_cost = 1e300;
     for (int ci = TILE_CI_MAX; ci >= 4; ci -= 2) {
-        const long long tiles = cols * ((nr + ci - 1) / ci) * ny;
+        const long long tiles = cols * ((nr + ci - 1) / ci);
         const double rounds = (double)((tiles + nslots - 1) / nslots);
         const double cost = rounds * (ci + 2 + 3);
         if (cost < best_cost * 0.999) { best_cost = cost; best = ci; }

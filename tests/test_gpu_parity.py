@@ -111,9 +111,7 @@ def test_l2_plan_hints_do_not_change_the_bits(qrec):
     gpu.set_option("qrecompute", qrec)
     b = _t(configs.rhs_blob(prob))
     runs = []
-    for keep_r, keep_p, first_x in [(0, 0, 0), (17, 0, 0), (40, 9, 1), (1000, 1000, 1)]:
-        gpu.set_option("l2_keep_r", keep_r)
-        gpu.set_option("l2_keep_p", keep_p)
+    for first_x in (0, 1):
         gpu.set_option("l2_first_x", first_x)
         x = torch.zeros_like(b)
         st, k, h = gpu.solve(b, x, 1e-9, 3000)
