@@ -127,8 +127,9 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
  *   "loop_mode"   0 host-driven chunks of 16 iterations, 1 CUDA-graph WHILE loop (default);
  *   "persistent"  1 (default): meshes whose per-cell state fits in the SMs' shared memory are solved by ONE
  *                 cooperative kernel, whatever loop_mode says; 0: always the streaming loop;
- *   "qrecompute"  1 (default): 64 B/cell/iteration -- K1 does not store q, K2 recomputes it; 0: 72 B, q stored;
- *   "tile"        K1 tile configuration (0..6), "k2r_tile" / "stencil_tile" (0..5) the stencil kernel's tile for
+ *   "qrecompute"  0 (default): 72 B/cell/iteration, q stored by K1 and streamed by K2; 1: 64 B -- K1 does not store q,
+ *                 K2 recomputes it with the stencil kernel (fewer bytes, more instructions: measured slower);
+ *   "tile"        K1 tile configuration (0..10), "k2r_tile" / "stencil_tile" (0..10) the stencil kernel's tile for
  *                 K2R / for apply and RKL2 stages, "ci" r-chunk length of the marching kernels (0 = automatic, else 2..32);
  *   "serpentine"  1 (default): K2 sweeps the mesh backward (L2 reuse across K1 -> K2 -> K1);
  *   "unroll"      PCG iterations per WHILE trip of the graph loop (1..16, default 4);

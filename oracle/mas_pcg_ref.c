@@ -209,19 +209,33 @@ static double dot(size_t n, const double *a, const double *b)
     return (double)s;
 }
 
+/* PC2 (block-Jacobi ILU(0), defined at the end of this file): z = M^-1 r */
+typedef struct ref_pc2 ref_pc2;
+void mas_ref_pc2_apply(const ref_pc2 *pc, const double *r, double *z);
+static size_t pc2_size(const ref_pc2 *pc);
+
+/* z = M^-1 r:  PC1, M = diag(A_sym) (pc == NULL), or PC2, M = the block-Jacobi ILU(0) factors */
+static void precondition(const ref_pc2 *pc, size_t n, const double *d, const double *r, double *z)
+{
+    if (pc) mas_ref_pc2_apply(pc, r, z);
+    else for (size_t c = 0; c < n; c++) z[c] = r[c] / d[c];
+}
+
 /*
- * Textbook PCG with M = diag(A_sym) ("PCG ... PC1 ... point-Jacobi", Saad [22]),
- * in the order and notation of DESIGN.md R3 / SURVEY.md 8(c) C3.
+ * Textbook PCG ("PCG ...", Saad [22]) in the order and notation of DESIGN.md R3 / SURVEY.md 8(c) C3,
+ * with the paper's two preconditioners: PC1, M = diag(A_sym) ("the inverse diagonal of the matrix
+ * (point-Jacobi)"), when pc == NULL; PC2, M = block-Jacobi ILU(0), otherwise.
  *   b_phys : physical right-hand side (b_s = V.b is formed here)
  *   x      : in = x0, out = last iterate
  *   hist   : NULL or >= maxit+1 doubles; hist[k] = ||r_k||_2 / ||b_s||_2
  * returns REF_OK / REF_MAXIT / negative error; *iters = k.
  */
-int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, int maxit,
-                int *iters, double *hist)
+static int pcg_core(const ref_op *op, const ref_pc2 *pc, const double *b_phys, double *x, double rtol, int maxit,
+                    int *iters, double *hist)
 {
     if (!op || !b_phys || !x || !iters || rtol < 0.0 || maxit < 0) return REF_EINVAL;
     const size_t n = (size_t)op->nr * op->nt * op->np;
+    if (pc && pc2_size(pc) != n) return REF_EINVAL;
     double *d = (double *)malloc(n * sizeof(double)), *r = (double *)malloc(n * sizeof(double));
     double *z = (double *)malloc(n * sizeof(double)), *p = (double *)malloc(n * sizeof(double));
     double *q = (double *)malloc(n * sizeof(double));
@@ -243,7 +257,7 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
     }
     mas_ref_apply(op, x, q);
     for (size_t c = 0; c < n; c++) r[c] -= q[c];                /* r = b_s - A x0 */
-    for (size_t c = 0; c < n; c++) z[c] = r[c] / d[c];
+    precondition(pc, n, d, r, z);
     memcpy(p, z, n * sizeof(double));
     double rho = dot(n, r, z), rr = dot(n, r, r);
     double h = sqrt(rr / bb);
@@ -257,7 +271,7 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
         const double alpha = rho / sigma;
         for (size_t c = 0; c < n; c++) x[c] += alpha * p[c];
         for (size_t c = 0; c < n; c++) r[c] -= alpha * q[c];
-        for (size_t c = 0; c < n; c++) z[c] = r[c] / d[c];
+        precondition(pc, n, d, r, z);
         const double rho1 = dot(n, r, z);
         rr = dot(n, r, r);
         k += 1;
@@ -273,6 +287,13 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
 done:
     free(d); free(r); free(z); free(p); free(q);
     return status;
+}
+
+/* PCG with PC1 (point-Jacobi) */
+int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, int maxit,
+                int *iters, double *hist)
+{
+    return pcg_core(op, NULL, b_phys, x, rtol, maxit, iters, hist);
 }
 
 /*
@@ -410,14 +431,16 @@ done:
  * "parity unpinned": not available.
  * ============================================================================================== */
 
-typedef struct ref_pc2 {
+struct ref_pc2 {
     size_t n;
     int nnz_max;
     size_t *rowptr;     /* [n+1] */
     int *col;           /* [nnz] ascending within a row */
     double *val;        /* [nnz] A_blk, overwritten by the factors: strictly lower = L (unit diagonal implied), rest = U */
     size_t *diag;       /* [n] position of the diagonal entry of each row */
-} ref_pc2;
+};
+
+static size_t pc2_size(const ref_pc2 *pc) { return pc->n; }
 
 void mas_ref_pc2_destroy(ref_pc2 *pc)
 {
@@ -472,9 +495,8 @@ ref_pc2 *mas_ref_pc2_create(const ref_op *op, int bi, int bj, int bk)
                     if (ii < 0 || ii >= nr || jj < 0 || jj >= nt) continue;          /* boundary face: no neighbour cell */
                     if (ii / bi != i / bi || jj / bj != j / bj || kk / bk != k / bk) continue;   /* another box */
                     const long long cc = (long long)(((size_t)ii * nt + jj) * np + kk);
-                    if (cc == (long long)c) continue;                                 /* np = 1: the cell is its own phi neighbour; flux is zero */
-                    int hit = -1;
-                    for (int e = 1; e < m; e++) if (cols[e] == cc) hit = e;          /* np = 2: both phi faces lead to the same cell */
+                    int hit = -1;                                                     /* np = 2: both phi faces lead to the same cell; */
+                    for (int e = 0; e < m; e++) if (cols[e] == cc) hit = e;          /* np = 1: the cell is its own phi neighbour     */
                     if (hit >= 0) vals[hit] += -op->dt * g[f];
                     else { cols[m] = cc; vals[m++] = -op->dt * g[f]; }
                 }
@@ -547,56 +569,6 @@ void mas_ref_pc2_dense_factors(const ref_pc2 *pc, double *Ld, double *Ud)
 int mas_ref_pcg_pc2(const ref_op *op, const ref_pc2 *pc, const double *b_phys, double *x, double rtol, int maxit,
                     int *iters, double *hist)
 {
-    if (!op || !pc || !b_phys || !x || !iters || rtol < 0.0 || maxit < 0) return REF_EINVAL;
-    const size_t n = (size_t)op->nr * op->nt * op->np;
-    if (pc->n != n) return REF_EINVAL;
-    double *r = (double *)malloc(n * sizeof(double)), *z = (double *)malloc(n * sizeof(double));
-    double *p = (double *)malloc(n * sizeof(double)), *q = (double *)malloc(n * sizeof(double));
-    int status = REF_ENOMEM, k = 0;
-    if (!r || !z || !p || !q) goto done;
-
-    mas_ref_volume(op, z);
-    for (size_t c = 0; c < n; c++) r[c] = z[c] * b_phys[c];     /* b_s = V.b */
-    const double bb = dot(n, r, r);
-    if (!isfinite(bb)) {
-        if (hist) hist[0] = bb;
-        *iters = 0; status = REF_EBREAKDOWN; goto done;
-    }
-    if (bb == 0.0) {
-        memset(x, 0, n * sizeof(double));
-        if (hist) hist[0] = 0.0;
-        *iters = 0; status = REF_OK; goto done;
-    }
-    mas_ref_apply(op, x, q);
-    for (size_t c = 0; c < n; c++) r[c] -= q[c];
-    mas_ref_pc2_apply(pc, r, z);
-    memcpy(p, z, n * sizeof(double));
-    double rho = dot(n, r, z), rr = dot(n, r, r);
-    double h = sqrt(rr / bb);
-    if (hist) hist[0] = h;
-    status = REF_OK;
-    if (!isfinite(rho) || !isfinite(rr)) { *iters = 0; status = REF_EBREAKDOWN; goto done; }
-    while (k < maxit && h > rtol && rho != 0.0) {
-        mas_ref_apply(op, p, q);
-        const double sigma = dot(n, p, q);
-        if (!(sigma > 0.0) || !isfinite(sigma)) { status = REF_EBREAKDOWN; break; }
-        const double alpha = rho / sigma;
-        for (size_t c = 0; c < n; c++) x[c] += alpha * p[c];
-        for (size_t c = 0; c < n; c++) r[c] -= alpha * q[c];
-        mas_ref_pc2_apply(pc, r, z);
-        const double rho1 = dot(n, r, z);
-        rr = dot(n, r, r);
-        k += 1;
-        h = sqrt(rr / bb);
-        if (hist) hist[k] = h;
-        if (!isfinite(rho1) || !isfinite(rr)) { status = REF_EBREAKDOWN; break; }
-        const double beta = rho1 / rho;
-        rho = rho1;
-        for (size_t c = 0; c < n; c++) p[c] = z[c] + beta * p[c];
-    }
-    if (status == REF_OK) status = (h <= rtol || rho == 0.0) ? REF_OK : REF_MAXIT;
-    *iters = k;
-done:
-    free(r); free(z); free(p); free(q);
-    return status;
+    if (!pc) return REF_EINVAL;
+    return pcg_core(op, pc, b_phys, x, rtol, maxit, iters, hist);
 }

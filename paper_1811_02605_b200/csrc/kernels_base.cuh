@@ -226,7 +226,8 @@ __global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditio
 // when the next K1 starts at i = 0).  The row -> block -> partial mapping stays fixed, so determinism holds.
 // ---------------------------------------------------------------------------------------------
 template <int NT, bool UNIFORM>
-__global__ void __launch_bounds__(NT) k2_vec(OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond,
+__global__ void __launch_bounds__(NT, 5) k2_vec(   // 5 blocks of 256 threads per SM (<= 48 registers): K2 hides latency by memory parallelism only
+OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond,
                                              int reverse)
 {
     __shared__ double sh[32];

@@ -104,7 +104,7 @@ struct mas_pcg {
     int persistent = 1;              // 1: one cooperative kernel for the whole solve whenever the state fits on chip
     int coop_ok = 0, coop_refused = 0;
     int unroll = 4;                  // PCG iterations per WHILE trip of the graph loop (measured: +1 % c4, +3 % c3)
-    int qrecompute = 1;              // 1: q is not stored, K2R recomputes it: 64 B/cell/iteration; 0: 72 B
+    int qrecompute = 0;              // 1: q is not stored, K2R recomputes it: 64 B/cell/iteration; 0: 72 B (default: faster)
     L2Plan l2{0};
     cudaGraph_t graph[MAX_RHS] = {};
     cudaGraphExec_t exec[MAX_RHS] = {};

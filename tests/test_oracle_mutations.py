@@ -1,7 +1,7 @@
 """Mutation check of the oracle's pins (What's weak #3): each single-token mutation of
 oracle/mas_pcg_ref.c -- a dropped factor, a wrong index, a sign, a transposed operand -- is built in a temp
 directory and the mathematical pin tests are run against it; at least one pin must fail.  The pins are the
-ones in tests/test_oracle_pins.py and tests/test_oracle_sts_pins.py; stored oracle outputs (golden files,
+ones in tests/test_oracle_pins.py, tests/test_oracle_sts_pins.py and tests/test_oracle_pc2_pins.py; stored oracle outputs (golden files,
 the dt calibration file) do NOT count as pins and are excluded (-k / --deselect below).
 
 One mutation is expected to SURVIVE the mathematical pins and is listed as such: the face-nu mean (reading Q3).
@@ -30,8 +30,8 @@ MUTATIONS = [
      "double g = nuf * r_f[i] * r_c[i < nr ? i : nr - 1] * sin_c[j] * dth_c[j] / dr_f[i];", True),
     ("boundary_nu_cell", "if (i == 0)        nuf = nu_at(nu_kind, nu, nt, 0, j);",
      "if (i == 0)        nuf = nu_at(nu_kind, nu, nt, nr - 1, j);", True),
-    ("z_without_dinv", "for (size_t c = 0; c < n; c++) z[c] = r[c] / d[c];\n        const double rho1",
-     "for (size_t c = 0; c < n; c++) z[c] = r[c];\n        const double rho1", True),
+    ("z_without_dinv", "else for (size_t c = 0; c < n; c++) z[c] = r[c] / d[c];",
+     "else for (size_t c = 0; c < n; c++) z[c] = r[c];", True),
     ("theta_face_sin_c", "g = nuf * dr_c[i] * sin_f[j] / dth_f[j];", "g = nuf * dr_c[i] * sin_c[j] / dth_f[j];", True),
     ("dirichlet_neighbour_not_zero", "const double u_im = i > 0      ? u[c - (size_t)nt * np] : 0.0;\n"
      "                const double u_ip = i < nr - 1 ? u[c + (size_t)nt * np] : 0.0;\n"
@@ -48,6 +48,18 @@ MUTATIONS = [
      "op->v2[(size_t)i * nt + j] = r_c[i] * dr_c[i] * sin_c[j] * dth_c[j];", True),
     ("alpha_sign", "for (size_t c = 0; c < n; c++) r[c] -= alpha * q[c];", "for (size_t c = 0; c < n; c++) r[c] += alpha * q[c];",
      True),
+    # PC2 (block-Jacobi ILU(0)); caught by tests/test_oracle_pc2_pins.py
+    ("ilu_pivot_division_dropped", "pc->val[e] /= pc->val[pc->diag[k]];", ";", True),
+    ("ilu_update_sign", "pc->val[f] -= lik * pc->val[t];", "pc->val[f] += lik * pc->val[t];", True),
+    ("ilu_update_wrong_row", "for (size_t t = pc->diag[k] + 1; t < pc->rowptr[k + 1]; t++)",
+     "for (size_t t = pc->rowptr[k]; t < pc->diag[k]; t++)", True),
+    ("pc2_forward_sign", "for (size_t e = pc->rowptr[i]; e < pc->diag[i]; e++) s -= pc->val[e] * z[pc->col[e]];",
+     "for (size_t e = pc->rowptr[i]; e < pc->diag[i]; e++) s += pc->val[e] * z[pc->col[e]];", True),
+    ("pc2_backward_without_pivot", "z[i] = s / pc->val[pc->diag[i]];", "z[i] = s;", True),
+    ("pc2_box_cut_in_phi_ignored", "if (ii / bi != i / bi || jj / bj != j / bj || kk / bk != k / bk) continue;",
+     "if (ii / bi != i / bi || jj / bj != j / bj) continue;", True),
+    ("pc2_wrap_coupling_dropped", "const int nb_k[6] = {k, k, k, k, km, kp};",
+     "const int nb_k[6] = {k, k, k, k, k > 0 ? km : -1, kp};", True),
     # Q3: a declared reading, not fixed by mathematics -- expected to survive every mathematical pin
     ("face_nu_harmonic_mean_Q3",
      "else               nuf = 0.5 * (nu_at(nu_kind, nu, nt, i - 1, j) + nu_at(nu_kind, nu, nt, i, j));",
@@ -58,9 +70,11 @@ MUTATIONS = [
 NOT_PINS = ["--deselect", "tests/test_oracle_pins.py::test_calibration_file_matches_oracle"]
 
 
-def _run_pins(repo, sts_first=False):
-    files = ["tests/test_oracle_pins.py", "tests/test_oracle_sts_pins.py"]
-    cmd = [sys.executable, "-m", "pytest", *(files[::-1] if sts_first else files), "-x", "-q",
+def _run_pins(repo, first=None):
+    files = ["tests/test_oracle_pins.py", "tests/test_oracle_sts_pins.py", "tests/test_oracle_pc2_pins.py"]
+    if first:
+        files = [first] + [f for f in files if f != first]
+    cmd = [sys.executable, "-m", "pytest", *files, "-x", "-q",
            "-p", "no:cacheprovider", *NOT_PINS]
     env = dict(os.environ, PYTHONDONTWRITEBYTECODE="1")
     return subprocess.run(cmd, cwd=repo, env=env, capture_output=True, text=True, timeout=900)
@@ -73,7 +87,7 @@ def sandbox(tmp_path_factory):
     for d in ("oracle", "mas_inputs"):
         shutil.copytree(os.path.join(ROOT, d), repo / d, ignore=shutil.ignore_patterns("*.so", "__pycache__", "*.tmp"))
     os.makedirs(repo / "tests")
-    for f in ("__init__.py", "helpers.py", "test_oracle_pins.py", "test_oracle_sts_pins.py"):
+    for f in ("__init__.py", "helpers.py", "test_oracle_pins.py", "test_oracle_sts_pins.py", "test_oracle_pc2_pins.py"):
         shutil.copy(os.path.join(ROOT, "tests", f), repo / "tests" / f)
     open(repo / "tests" / "conftest.py", "w").write(
         "import os, sys\nsys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))\n")
@@ -99,7 +113,9 @@ def test_mutation(sandbox, name, old, new, caught):
     so = sandbox / "oracle" / "libmas_pcg_ref.so"
     if so.exists():
         so.unlink()
-    res = _run_pins(sandbox, sts_first=name.startswith("rkl2"))
+    first = ("tests/test_oracle_sts_pins.py" if name.startswith("rkl2") else
+             "tests/test_oracle_pc2_pins.py" if name.startswith(("ilu", "pc2")) else None)
+    res = _run_pins(sandbox, first=first)
     if caught:
         assert res.returncode != 0, f"mutation {name} survived every mathematical pin"
     else:
