@@ -117,11 +117,24 @@ int mas_pcg_apply(mas_pcg_t *h, const double *x_dev, double *y_dev, void *stream
 /* Fills HOST array out[8] with counters of the last solve:
  *   [0] kernels launched inside the iteration loop, [1] kernels launched outside it,
  *   [2] loop mode used (1 = CUDA-graph WHILE node, 0 = host-driven chunks, 2 = one persistent cooperative kernel),
- *   [3] algorithmic bytes per cell per iteration of the kernels in use,
+ *   [3] algorithmic bytes per cell per iteration of the kernels in use (72 default, 64 with "qrecompute", 88 with PC2),
  *   [4] doubles per cell K1 moves, [5] doubles per cell K2 moves,
  *   [6] grid size of the persistent kernel (0 if not used; slab groups: the number of slabs),
  *   [7] 1 if a cooperative launch was refused and the handle fell back to the streaming loop. */
 int mas_pcg_stats(const mas_pcg_t *h, long long *out);
+
+/* The paper's two "communication-free preconditioning options" (Sec. 2.2):
+ *   MAS_PC1  point-Jacobi, "the inverse diagonal of the matrix" (the default);
+ *   MAS_PC2  "a non-overlapping domain decomposition with zero-fill incomplete LU factorization" (SURVEY 8(f)
+ *            NEXT-4): block Jacobi over boxes of bi x bj x bk cells, ILU(0) of A_sym restricted to each box, natural
+ *            ordering (R8).  PAPER.md:80: 100-200 iterations against ~550 with PC1; the
+ *            authors kept it on the CPU because its triangular solves do not vectorise.
+ * On the GPU the boxes are the phi lines: bi = bj = 1 and bk = 0 (or >= np) = the whole periodic line, wrap coupling
+ * included; any other box shape returns MAS_EINVAL (the oracle covers general boxes and shows the line boxes within
+ * 2 iterations of the undivided factorisation on the synthetic meshes).  4 <= np <= 1024.  The factors follow dt:
+ * mas_pcg_set_dt refactors.  Not available for slab groups; mas_pcg_solve_multi works.  Synchronous. */
+enum { MAS_PC1 = 1, MAS_PC2 = 2 };
+int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj, int bk);
 
 /* Tuning knob, takes effect at the next solve.  name in
  *   "loop_mode"   0 host-driven chunks of 16 iterations, 1 CUDA-graph WHILE loop (default);

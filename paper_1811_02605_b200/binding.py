@@ -58,6 +58,7 @@ def _prototypes(L):
         "mas_sts_advance": (ci, [vp, vp, cd, ci, vp]),
         "mas_pcg_stats": (ci, [vp, ctypes.POINTER(ctypes.c_longlong)]),
         "mas_pcg_set_option": (ci, [vp, ctypes.c_char_p, ci]),
+        "mas_pcg_set_preconditioner": (ci, [vp, ci, ci, ci, ci]),
         "mas_pcg_destroy": (None, [vp]),
         "mas_pcg_strerror": (ctypes.c_char_p, [ci]),
         "mas_pcg_slabs_create": (ci, create_args + [ci, _ip, _vpp]),
@@ -145,6 +146,15 @@ def mas_pcg_set_option(handle, name: str, value: int, L=None):
     st = (L or lib()).mas_pcg_set_option(handle, name.encode(), int(value))
     if st != MAS_OK:
         raise MasError(st, f"mas_pcg_set_option({name}={value})")
+
+
+MAS_PC1, MAS_PC2 = 1, 2
+
+
+def mas_pcg_set_preconditioner(handle, kind: int, boxes=(1, 1, 0), L=None):
+    st = (L or lib()).mas_pcg_set_preconditioner(handle, int(kind), int(boxes[0]), int(boxes[1]), int(boxes[2]))
+    if st != MAS_OK:
+        raise MasError(st, f"mas_pcg_set_preconditioner({kind}, {tuple(boxes)})")
 
 
 def mas_pcg_apply(handle, x_ptr, y_ptr, stream=0):

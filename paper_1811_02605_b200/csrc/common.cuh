@@ -63,6 +63,7 @@ struct Ctl {
 
 struct Work {                    // handle-owned vectors; right-hand side j at + j * vstride
     double *r, *p0, *p1, *q;     // p ping-pongs: iteration k reads p[k&1], writes p[(k+1)&1]
+    double *z;                   // PC2 only: z = M^-1 r, written by the line kernel, read by K1 (null with PC1)
     long long vstride;
     double *partials;            // [MAX_RHS][PART_REGIONS][pstride]
     int pstride;                 // >= gridDim.x of every reducing kernel of the plan

@@ -3,7 +3,8 @@
 // kernel for sm_100a with the TMA engine as the loader and mbarriers instead of block barriers:
 //
 //     x    += alpha_{k-1} p_old       (the x-update of the PREVIOUS iteration, deferred into this pass: "xfuse")
-//     p_new = r/d + beta p_old        (the p-update of the previous iteration, fused as a prologue)
+//     p_new = r/d + beta p_old        (the p-update of the previous iteration, fused as a prologue; with PC2 the
+//                                      preconditioned residual z is read from memory in place of r/d)
 //     q     = A_sym p_new             (7-point, matrix-free, coefficients from 2-D planes)   [not stored when NOQ]
 //     sigma = p_new . q               (deterministic two-stage reduction; last block: alpha = rho / sigma)
 //
@@ -86,7 +87,8 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     const int par = st->k & 1;
     const long long voff = rhs * w.vstride;
     const VecHalo pV = {(par ? w.p1 : w.p0) + voff, par ? w.lo_p1 : w.lo_p0, par ? w.hi_p1 : w.hi_p0};
-    const VecHalo rV = {w.r + voff, w.lo_r, w.hi_r};
+    const bool zin = mp.zin != 0;               // PC2: "r" below is z = M^-1 r, already preconditioned
+    const VecHalo rV = zin ? VecHalo{w.z + voff, nullptr, nullptr} : VecHalo{w.r + voff, w.lo_r, w.hi_r};
     double *__restrict__ pout = (par ? w.p0 : w.p1) + voff;
     double *__restrict__ qout = w.q + voff;
     const double alpha_prev = st->alpha;        // x += alpha_{k-1} p_{k-1}: the deferred x-update (xfuse)
@@ -96,7 +98,7 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     const PhiFac<UNIFORM, TileCoefs<NW, UNIFORM>> ph = {sm.c, mp.vp, mp.wp, mp.ip};
     const int ea = 2 * lane + 1, eb = 2 * lane + 65;
     auto zval = [&](double r, double E, double F, double dinv, int e) {
-        return UNIFORM ? r * dinv : r / fma(ph.VP(e), E, F * ph.WP(e));
+        return zin ? r : (UNIFORM ? r * dinv : r / fma(ph.VP(e), E, F * ph.WP(e)));
     };
 
     const long long plane = (long long)op.nt * op.np;

@@ -19,6 +19,7 @@
 #include "kernels_stencil_tma.cuh"
 #include "kernels_k1_tma.cuh"
 #include "kernels_persistent.cuh"
+#include "kernels_pc2.cuh"
 
 using namespace mas;
 
@@ -83,6 +84,10 @@ struct mas_pcg {
     // workspaces for `nrhs_cap` right-hand sides (vectors back to back, stride n)
     int nrhs_cap = 0;
     DevBuf<double> r, p0, p1, q, partials, hist, bdev, xdev;
+    // PC2 (block-Jacobi ILU(0) on phi-line boxes; kernels_pc2.cuh): z vectors, 1/pivot in chunk order, ip in chunk order
+    int precond = MAS_PC1;
+    int pc2_M = 0;
+    DevBuf<double> z, dinvT, ipT;
     int pstride = 0;
     DevBuf<State> st;
     DevBuf<SolveArgs> args;
@@ -168,6 +173,7 @@ void fill_op(mas_pcg *h)
     Work &w = h->work;
     memset(&w, 0, sizeof(w));
     w.r = h->r.p; w.p0 = h->p0.p; w.p1 = h->p1.p; w.q = h->q.p;
+    w.z = h->z.p;
     w.vstride = (long long)h->n;
     w.partials = h->partials.p; w.pstride = h->pstride;
     w.hist = h->hist.p; w.hstride = (int)h->hist_cap;
@@ -184,6 +190,11 @@ int scale_planes(mas_pcg *h, double dt, cudaStream_t s)
     k_scale_planes<<<(total + 255) / 256, 256, 0, s>>>(ps, dt);
     CK(cudaGetLastError());
     h->dt = dt;
+    if (h->precond == MAS_PC2) {                 // the ILU(0) pivots depend on dt: factor again (stream order)
+        const int lines = h->nr * h->nt;
+        k_pc2_factor<<<(lines + 127) / 128, 128, 0, s>>>(h->op, h->dinvT.p, h->pc2_M);
+        CK(cudaGetLastError());
+    }
     return MAS_OK;
 }
 
@@ -203,7 +214,8 @@ int ensure_rhs_capacity(mas_pcg *h, int nrhs)
     if (nrhs <= h->nrhs_cap) return MAS_OK;
     drop_graphs(h);
     const size_t tot = h->n * (size_t)nrhs;
-    if (h->r.alloc(tot) || h->p0.alloc(tot) || h->p1.alloc(tot) || h->q.alloc(tot)) {
+    if (h->r.alloc(tot) || h->p0.alloc(tot) || h->p1.alloc(tot) || h->q.alloc(tot) ||
+        (h->precond == MAS_PC2 && h->z.alloc(tot))) {
         cudaGetLastError();
         h->nrhs_cap = 0;
         return MAS_ENOMEM;
@@ -237,7 +249,7 @@ extern "C" void mas_pcg_destroy(mas_pcg_t *h)
     drop_graphs(h);
     DevBuf<double> *bufs[] = {&h->V2, &h->SD, &h->CP, &h->CRoff, &h->CT, &h->E, &h->F, &h->AR, &h->AT, &h->Dinv,
                               &h->vp, &h->wp, &h->ip, &h->Vinv, &h->r, &h->p0, &h->p1, &h->q, &h->partials, &h->hist,
-                              &h->bdev, &h->xdev};
+                              &h->bdev, &h->xdev, &h->z, &h->dinvT, &h->ipT};
     for (DevBuf<double> *b : bufs) b->release();
     h->st.release();
     h->args.release();
@@ -396,6 +408,8 @@ struct Plan {                        // storage that kernel argument pointers re
     TileParams k1p;
     StencilParams sp_apply, sp_k2;
     KLaunch apply, init, k1, k2, xtail;
+    Pc2Dev pc2;
+    int zero = 0;
     int max_grid = 0;
 };
 
@@ -442,15 +456,38 @@ int make_plan(const mas_pcg *h, const OpDev &op, const Work &work, int nrhs, int
     c.init.block = dim3(NT_BASE);
     c.init.grid = dim3(base_grid(h, op, c.init.func, NT_BASE), nrhs);
     c.init.args[0] = &c.op; c.init.args[1] = &c.work; c.init.args[2] = &c.cond; c.init.args[3] = &c.use_cond;
+    const bool pc2 = h->precond == MAS_PC2;
+    auto pc2_launch = [&](KLaunch &k, bool init, int *reverse) {       // the line kernel: init or K2P
+        k.func = pc2_line_pick(h->pc2_M, uni, init);
+        k.block = dim3(PC2_NT);
+        k.smem = pc2_smem(h->pc2_M);
+        cudaFuncSetAttribute(k.func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.smem);
+        int occ = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k.func, PC2_NT, k.smem) != cudaSuccess || occ < 1) {
+            cudaGetLastError();
+            occ = 1;
+        }
+        long long g = (long long)h->num_sms * occ, need = ((long long)op.nrows + PC2_NWARP - 1) / PC2_NWARP;
+        k.grid = dim3((unsigned)(g < need ? g : need), nrhs);
+        k.args[0] = &c.op; k.args[1] = &c.work; k.args[2] = &c.pc2; k.args[3] = &c.cond; k.args[4] = &c.use_cond;
+        k.args[5] = reverse;
+    };
+    if (pc2) {
+        c.pc2 = Pc2Dev{h->dinvT.p, h->ipT.p, h->ip0, h->pc2_M};
+        pc2_launch(c.init, true, &c.zero);
+    }
     // K1
     memset(&c.k1p, 0, sizeof(c.k1p));
-    k1_tma_configure(op.nr, op.nt, op.np, uni, h->qrecompute != 0, h->tile, h->num_sms, h->ci_force, nrhs, &c.k1p,
+    k1_tma_configure(op.nr, op.nt, op.np, uni, h->qrecompute != 0 && !pc2, h->tile, h->num_sms, h->ci_force, nrhs, &c.k1p,
                      &c.k1.func, &c.k1.grid, &c.k1.block, &c.k1.smem);
     c.k1p.vp = h->vp0; c.k1p.wp = h->wp0; c.k1p.ip = h->ip0;
     c.k1p.l2 = h->l2;
+    c.k1p.zin = pc2 ? 1 : 0;
     c.k1.args[0] = &c.op; c.k1.args[1] = &c.work; c.k1.args[2] = &c.k1p; c.k1.args[3] = &c.cond; c.k1.args[4] = &c.use_cond;
-    // K2 (q stored) or K2R (q recomputed)
-    if (h->qrecompute) {
+    // K2 (q stored), K2R (q recomputed), or K2P (PC2: r-update + line solves)
+    if (pc2) {
+        pc2_launch(c.k2, false, &c.reverse);
+    } else if (h->qrecompute) {
         stencil_common(h, c.sp_k2);
         c.sp_k2.ps = PlaneSetDev{h->E.p, h->F.p, h->AR.p, h->AT.p, h->Dinv.p};
         c.sp_k2.w = work; c.sp_k2.cond = cond; c.sp_k2.use_cond = use_cond;
@@ -577,7 +614,7 @@ bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
 // Plan the one-kernel solve; returns false when it does not apply (too large, no cooperative launch, off).
 bool plan_persistent(const mas_pcg *h, PersistParams *pp, int *grid, size_t *smem, const void **func)
 {
-    if (!h->persistent || !h->coop_ok) return false;
+    if (!h->persistent || !h->coop_ok || h->precond != MAS_PC1) return false;
     const long long nvec = (long long)h->n / 2;
     long long g = (nvec + PNT - 1) / PNT;
     if (g > h->num_sms) g = h->num_sms;
@@ -605,8 +642,10 @@ bool plan_persistent(const mas_pcg *h, PersistParams *pp, int *grid, size_t *sme
 void set_traffic_stats(mas_pcg *h)
 {
     // qrecompute: K1 r,p,x -> p,x (5N); K2R p,r -> r (3N).  otherwise: K1 r,p,x -> p,q,x (6N); K2 r,q -> r (3N)
-    h->stats[4] = h->qrecompute ? 5 : 6;
-    h->stats[5] = 3;
+    // PC2: K1 z,p,x -> p,q,x (6N); K2P r,q,1/piv -> r,z (5N)
+    const bool pc2 = h->precond == MAS_PC2;
+    h->stats[4] = (h->qrecompute && !pc2) ? 5 : 6;
+    h->stats[5] = pc2 ? 5 : 3;
     h->stats[3] = 8 * (h->stats[4] + h->stats[5]);
 }
 
@@ -744,6 +783,43 @@ extern "C" int mas_pcg_apply(mas_pcg_t *h, const double *x_dev, double *y_dev, v
                       &k.func, &k.grid, &k.block, &k.smem);
     k.args[0] = &op; k.args[1] = &sp;
     CK(launch(k, (cudaStream_t)stream));
+    return MAS_OK;
+}
+
+extern "C" int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj, int bk)
+{
+    if (!h || (kind != MAS_PC1 && kind != MAS_PC2)) return MAS_EINVAL;
+    DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
+    if (kind == MAS_PC1) {
+        if (h->precond != MAS_PC1) drop_graphs(h);
+        h->precond = MAS_PC1;
+        fill_op(h);
+        return MAS_OK;
+    }
+    // the GPU path builds the line domains only: 1 x 1 x (all of phi); other boxes are the oracle's (R8)
+    if (bi != 1 || bj != 1 || (bk != 0 && bk < h->np)) return MAS_EINVAL;
+    const int M = pc2_chunk(h->np);
+    if (M == 0) return MAS_EINVAL;                           // np < 4 or np > 1024
+    const size_t lines = (size_t)h->nr * h->nt;
+    if (!h->dinvT.p || h->pc2_M != M) {
+        if (h->dinvT.alloc(lines * 32 * M) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+        std::vector<double> ipT((size_t)32 * M, 0.0), ip(h->np);
+        CK(cudaMemcpy(ip.data(), h->ip.p, (size_t)h->np * sizeof(double), cudaMemcpyDeviceToHost));
+        for (int k = 0; k < h->np; k++) ipT[(size_t)pc2_slot(k, M)] = ip[(size_t)k];
+        const int rc = upload(h->ipT, ipT);
+        if (rc != MAS_OK) return rc;
+    }
+    if (!h->z.p || h->z.n < h->n * (size_t)h->nrhs_cap) {
+        if (h->z.alloc(h->n * (size_t)(h->nrhs_cap > 0 ? h->nrhs_cap : 1)) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    }
+    h->pc2_M = M;
+    h->precond = MAS_PC2;
+    fill_op(h);
+    drop_graphs(h);
+    k_pc2_factor<<<(unsigned)((lines + 127) / 128), 128>>>(h->op, h->dinvT.p, M);
+    CK(cudaGetLastError());
+    CK(cudaDeviceSynchronize());
     return MAS_OK;
 }
 

@@ -119,6 +119,7 @@ struct TileParams {
     int nkt, njt, nit, ci;                   // tiles in phi, theta, r; interior planes per block
     double vp, wp, ip;                       // uniform-phi factors (dph_c, 2/dph_f, 1/dph_f)
     int reverse;                             // 1: blocks take the tiles in reverse order (serpentine sweeps)
+    int zin;                                 // K1 with PC2: the preconditioned residual z is read from Work::z instead of formed as r/d
     L2Plan l2;
 };
 

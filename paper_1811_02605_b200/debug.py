@@ -32,9 +32,11 @@ def lib_dbg():
 class MasPcgProbe:
     """One operator created through the debug library; profile() and mix_probe() only."""
 
-    def __init__(self, mesh, dt, nu_kind, nu, bc=(0, 0), options=()):
+    def __init__(self, mesh, dt, nu_kind, nu, bc=(0, 0), options=(), precond=1):
         self.n = mesh.nr * mesh.nt * mesh.np_
         self._h = B.mas_pcg_create((mesh.nr, mesh.nt, mesh.np_), mesh.metric_arrays(), dt, nu_kind, nu, bc, L=lib_dbg())
+        if precond != 1:
+            B.mas_pcg_set_preconditioner(self._h, precond, L=lib_dbg())
         for name, value in options:
             B.mas_pcg_set_option(self._h, name, value, L=lib_dbg())
 

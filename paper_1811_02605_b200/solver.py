@@ -40,6 +40,10 @@ class MasPcg:
     def set_option(self, name, value):
         B.mas_pcg_set_option(self._h, name, value)
 
+    def set_preconditioner(self, kind: int, boxes=(1, 1, 0)):
+        """kind 1 = PC1 (point Jacobi), 2 = PC2 (block-Jacobi ILU(0); on the GPU the boxes are the phi lines)"""
+        B.mas_pcg_set_preconditioner(self._h, kind, boxes)
+
     def apply(self, x: torch.Tensor, y: torch.Tensor | None = None, stream=None) -> torch.Tensor:
         """y = A_sym x"""
         if y is None:
