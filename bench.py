@@ -41,7 +41,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "sts", "visc"])
+    ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "sts", "visc", "precond"])
+    ap.add_argument("--precond", type=int, default=1, choices=[1, 2],
+                    help="1 = PC1 point Jacobi (default), 2 = PC2 block-Jacobi ILU(0) over phi lines (NEXT-4)")
     ap.add_argument("--opt", action="append", default=[], help="name=value passed to mas_pcg_set_option (tuning)")
     ap.add_argument("--nrhs", type=int, default=1, help="right-hand sides per batched solve (1..3; NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -225,6 +227,8 @@ def run_chain(args):
     for kv in args.opt:
         name, val = kv.split("=")
         gpu.set_option(name, int(val))
+    if args.precond == 2:
+        gpu.set_preconditioner(2)
     stream = torch.cuda.current_stream()
     n = prob.mesh.ncells
     x = torch.zeros(prob.mesh.shape, dtype=torch.float64, device="cuda")
@@ -278,7 +282,8 @@ def run_chain(args):
             "config": {"workload": f"c5: 192x256x384 fp64, s=100 at dt0, dt +-20 %/step, warm start, rtol 1e-9, "
                                    f"{'all' if nsteps == 100 else 'first ' + str(nsteps) + ' of'} 100 chained solves",
                        "l2": "inputs larger than L2 (5 live vectors x 151 MB vs 126 MB)",
-                       "mean_iters_per_solve": float(np.mean(iters)), "iters": iters, "bytes_per_cell_iter": bpc},
+                       "mean_iters_per_solve": float(np.mean(iters)), "iters": iters, "bytes_per_cell_iter": bpc,
+                       "preconditioner": {1: "PC1 point Jacobi", 2: "PC2 block-Jacobi ILU(0), phi-line domains"}[args.precond]},
             "iterations_per_s": its / (total_ms * 1e-3),
             "clocks": clocks,
             "e2e": {"value": nsteps / e2e_s, "unit": "solves/s", "h2d_bytes_per_step": 2 * 8 * n,
@@ -297,7 +302,12 @@ def run_chain(args):
         for step in range(3):
             op.set_dt(dt0 * ch.dt_factor[step])
             t0 = time.perf_counter()
-            st_o, k_o, xo, _ = op.pcg(b, xo, prob.rtol, prob.maxit)
+            if args.precond == 2:
+                pc = op.pc2((1, 1, 0))                      # factorisation at the new dt, inside the timed region
+                st_o, k_o, xo, _ = op.pcg_pc2(pc, b, xo, prob.rtol, prob.maxit)
+                pc.close()
+            else:
+                st_o, k_o, xo, _ = op.pcg(b, xo, prob.rtol, prob.maxit)
             t_or += time.perf_counter() - t0
             k_or.append(k_o)
             b = xo + ch.noise()
@@ -415,6 +425,57 @@ def run_visc(args):
     print(json.dumps(line), flush=True)
 
 
+def run_precond(args):
+    """The paper's preconditioner comparison (PC2 needs 100-200 iterations against ~550
+    with PC1 but its triangular solves were left on the CPU; with cuSparse on the GPU "similar performance as using
+    PC1"), on the synthetic hard viscosity solves: configs 3 and 4 (stiffness 1e4) solved to rtol 1e-9 with PC1 and
+    with PC2 (block-Jacobi ILU(0) over phi-line domains), time to solution and iterations."""
+    import torch
+    from mas_inputs import configs
+    from paper_1811_02605_b200 import MasPcg
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    out = {}
+    for name in ("c3", "c4"):
+        prob = configs.make(name)
+        dt = prob.dt_for(1e4)
+        b = torch.from_numpy(workload_rhs(name, prob)).cuda()
+        x = torch.zeros_like(b)
+        gpu = MasPcg(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)
+        res = {}
+        for pc in (1, 2):
+            gpu.set_preconditioner(pc)
+            for _ in range(max(args.warmup, 1)):
+                x.zero_()
+                gpu.solve(b, x, 1e-9, 5000, want_hist=False)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ms = 0.0
+            for _ in range(args.steps):
+                x.zero_()
+                torch.cuda.synchronize()
+                e0.record(stream)
+                st, k, _ = gpu.solve(b, x, 1e-9, 5000, want_hist=False)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms += e0.elapsed_time(e1)
+            s = gpu.stats()
+            res[f"pc{pc}"] = {"ms": ms / args.steps, "iterations": k, "status": st,
+                              "ms_per_iteration": ms / args.steps / max(k, 1),
+                              "bytes_per_cell_iter": s["bytes_per_cell_iter"],
+                              "model_gbs": s["bytes_per_cell_iter"] * prob.mesh.ncells * k / (ms / args.steps * 1e-3) / 1e9}
+        res["pc2_speedup"] = res["pc1"]["ms"] / res["pc2"]["ms"]
+        res["iteration_ratio"] = res["pc1"]["iterations"] / res["pc2"]["iterations"]
+        out[name] = res
+        gpu.close()
+    line = {"metric": "viscosity_solve_ms_pc2_256x256x512", "value": out["c4"]["pc2"]["ms"], "unit": "ms", "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 1), "ms_per_step": out["c4"]["pc2"]["ms"],
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "precond: configs 3 (128x192x256) and 4 (256x256x512) at stiffness 1e4, solved to "
+                                   "rtol 1e-9 from x0 = 0 with PC1 (point Jacobi) and PC2 (block-Jacobi ILU(0), phi-line domains)"},
+            "c3": out["c3"], "c4": out["c4"]}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse()
     if args.impl == "ours" and args.workload == "visc":
@@ -422,6 +483,9 @@ def main():
         return
     if args.impl == "ours" and args.workload == "c5":
         run_chain(args)
+        return
+    if args.impl == "ours" and args.workload == "precond":
+        run_precond(args)
         return
     if args.impl == "ours" and args.workload == "sts":
         run_sts(args)
@@ -456,6 +520,8 @@ def main():
     gpu = MasPcg(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)
     for name, val in opts:
         gpu.set_option(name, val)
+    if args.precond == 2:
+        gpu.set_preconditioner(2)
     # right-hand side j of a batched solve = the workload's b from seed + j (independent problems, one operator)
     b_hosts = [torch.from_numpy(b_np).pin_memory()]
     for j in range(1, nrhs):
@@ -516,7 +582,8 @@ def main():
 
     # ---------------- per-kernel durations: CUDA events around each launch (debug library, same source + probes) ----
     from paper_1811_02605_b200.debug import MasPcgProbe
-    probe = MasPcgProbe(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc, options=[o for o in opts if o[0] != "persistent"])
+    probe = MasPcgProbe(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc, options=[o for o in opts if o[0] != "persistent"],
+                        precond=args.precond)
     x.zero_()
     prof = probe.profile(b, x, 40, int(stream.cuda_stream))
     pstats = probe.stats()
@@ -538,8 +605,9 @@ def main():
         k1_bytes, k2_bytes = pstats["k1_doubles_per_cell"] * 8 * n, pstats["k2_doubles_per_cell"] * 8 * n
         k1_gbs = k1_bytes / (prof["k1_ms"] * 1e-3) / 1e9
         k2_gbs = k2_bytes / (prof["k2_ms"] * 1e-3) / 1e9
-        k1_name = "k1_tma_noq" if pstats["k1_doubles_per_cell"] == 5 else "k1_tma"
-        k2_name = "k2r_stencil_tma" if pstats["k1_doubles_per_cell"] == 5 else "k2_vec"
+        k1_name = "k1_tma_noq" if pstats["k1_doubles_per_cell"] == 5 else ("k1_tma_zin" if args.precond == 2 else "k1_tma")
+        k2_name = ("k2r_stencil_tma" if pstats["k1_doubles_per_cell"] == 5 else
+                   ("k_pc2_line" if args.precond == 2 else "k2_vec"))
         dom = k1_name if prof["k1_ms"] >= prof["k2_ms"] else k2_name
         dom_gbs = k1_gbs if dom == k1_name else k2_gbs
         traffic, traffic_src = ncu_traffic(dom)
@@ -554,6 +622,7 @@ def main():
                        "l2": "inputs larger than L2 (%d live vectors x %.0f MB vs 126 MB)" % (4 * nrhs, 8 * n / 1e6),
                        "loop_mode": {0: "host chunks", 1: "cuda-graph while", 2: "persistent cooperative kernel"}[loop_mode],
                        "bytes_per_cell_iter": bpc, "status": st, "iters_per_step": k, "nrhs": nrhs,
+                       "preconditioner": {1: "PC1 point Jacobi", 2: "PC2 block-Jacobi ILU(0), phi-line domains"}[args.precond],
                        "options": dict(opts)},
             "clocks": clocks,
             "e2e": {"value": e2e_iters_all / (e2e_ms * 1e-3), "unit": UNIT,

@@ -116,25 +116,43 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
         const int row = reverse ? op.nrows - 1 - ln : ln;
         const size_t base = (size_t)row * np;
         const double F = __ldg(op.F + row);
+        // ---- all loads of the line first (q, r or b in the natural order, 1/piv in the chunk order): the stores
+        // below may alias them as far as the compiler knows, so loads left between stores would be serialised ----
+        double2 qn[H], rn[H];
+        double dv[M], e[M], yd[M];
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            const int v = lane + 32 * h;
+            qn[h] = rn[h] = make_double2(0.0, 0.0);
+            if (v < nv) {
+                qn[h] = ld2(qvec, base + 2 * v);
+                rn[h] = ld2(INIT ? bvec : rvec, base + 2 * v);
+            }
+        }
+        const double2 *dT = reinterpret_cast<const double2 *>(pc.dinvT + (size_t)(op.i_lo * op.nt + row) * 32 * M);
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            const double2 t = __ldg(dT + h * 32 + lane);
+            dv[2 * h] = t.x; dv[2 * h + 1] = t.y;
+        }
         // ---- natural order: r' = r - alpha q (init: V.b - A x0), stored; staged for the chunk order ----
         double V2 = 0.0;
         if (INIT) V2 = __ldg(op.V2 + row);
-        for (int v = lane; v < 16 * M; v += 32) {
+#pragma unroll
+        for (int h = 0; h < H; h++) {
+            const int v = lane + 32 * h;
             double2 rv = make_double2(0.0, 0.0);
             if (v < nv) {
                 const size_t cell = base + 2 * v;
-                const double2 qv = ld2(qvec, cell);
                 if (INIT) {
-                    const double2 bv = ld2(bvec, cell);
-                    const double bs0 = V2 * __ldg(op.vp + 2 * v) * bv.x, bs1 = V2 * __ldg(op.vp + 2 * v + 1) * bv.y;
-                    rv.x = bs0 - qv.x;
-                    rv.y = bs1 - qv.y;
+                    const double bs0 = V2 * __ldg(op.vp + 2 * v) * rn[h].x, bs1 = V2 * __ldg(op.vp + 2 * v + 1) * rn[h].y;
+                    rv.x = bs0 - qn[h].x;
+                    rv.y = bs1 - qn[h].y;
                     acc[2] += bs0 * bs0 + bs1 * bs1;
                     st2(p0, cell, make_double2(0.0, 0.0));
                 } else {
-                    rv = ld2(rvec, cell);
-                    rv.x = fma(-alpha, qv.x, rv.x);
-                    rv.y = fma(-alpha, qv.y, rv.y);
+                    rv.x = fma(-alpha, qn[h].x, rn[h].x);
+                    rv.y = fma(-alpha, qn[h].y, rn[h].y);
                 }
                 st2(rvec, cell, rv);
                 acc[1] += rv.x * rv.x + rv.y * rv.y;
@@ -142,14 +160,7 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
             const int l = (2 * v) / M, u2 = v - l * H;      // chunk and pair index inside it
             buf[l * (S / 2) + u2] = rv;
         }
-        // ---- 1 / piv of this lane's chunk (coalesced: chunk order in memory), e_k = c_k / piv_k ----
-        double dv[M], e[M], yd[M];
-        const double2 *dT = reinterpret_cast<const double2 *>(pc.dinvT + (size_t)(op.i_lo * op.nt + row) * 32 * M);
-#pragma unroll
-        for (int h = 0; h < H; h++) {
-            const double2 t = __ldg(dT + h * 32 + lane);
-            dv[2 * h] = t.x; dv[2 * h + 1] = t.y;
-        }
+        // ---- e_k = c_k / piv_k ----
 #pragma unroll
         for (int u = 0; u < M; u++) {
             const double c = -F * (UNIFORM ? pc.ip0 : ipc[u]);
