@@ -429,15 +429,21 @@ def test_large_mesh_64bit_offsets_closed_forms():
     b = torch.rand(mesh.shape, dtype=torch.float64, device="cuda", generator=g) * 2 - 1
     gpu.set_dt(50.0 / lam)
     x = torch.zeros_like(b)
-    st, k, h = gpu.solve(b, x, 0.0, 5)
-    assert (st, k) == (1, 5) and np.isfinite(h).all() and (np.diff(h) != 0).all()
-    assert gpu.stats()["bytes_per_cell_iter"] == 64        # the default form: K2R (two sums) on 11 840+ K1 blocks
-    gpu.apply(x, y)                       # y = A x
-    y.neg_().add_(V * b)                  # true residual b_s - A x
     bs_norm = float((V * b).norm())
-    assert float(y.norm()) / bs_norm == pytest.approx(h[-1], rel=1e-9)
-    # last plane was really updated (a wrapped 32-bit byte offset would leave it untouched)
-    assert float(x[-1].abs().max()) > 0 and float(x[0].abs().max()) > 0
+    hs = []
+    for qrec, bpc in ((0, 72), (1, 64)):  # both forms: K2 (q stored) and K2R (two sums per block) on 11 840+ K1 blocks
+        gpu.set_option("qrecompute", qrec)
+        x.zero_()
+        st, k, h = gpu.solve(b, x, 0.0, 5)
+        assert (st, k) == (1, 5) and np.isfinite(h).all() and (np.diff(h) != 0).all()
+        assert gpu.stats()["bytes_per_cell_iter"] == bpc
+        gpu.apply(x, y)                   # y = A x
+        y.neg_().add_(V * b)              # true residual b_s - A x
+        assert float(y.norm()) / bs_norm == pytest.approx(h[-1], rel=1e-9)
+        # last plane was really updated (a wrapped 32-bit byte offset would leave it untouched)
+        assert float(x[-1].abs().max()) > 0 and float(x[0].abs().max()) > 0
+        hs.append(h)
+    assert np.allclose(hs[0], hs[1], rtol=1e-11, atol=0.0)
 
 
 # ------------------------------------------------------------------ the one-kernel (persistent cooperative) path
