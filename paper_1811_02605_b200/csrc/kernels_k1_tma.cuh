@@ -129,8 +129,8 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
         src += plane;
         if (!g.row_ok || !rrow) { mbar_arrive(bar); return; }
         mbar_arrive_expect_tx(bar, xin ? tx_rows + rowbytes : tx_rows);
-        row_copy(s_fr + ROWS_STAGE * stage, rrow, g, rowbytes, bar);
-        row_copy(s_fp + ROWS_STAGE * stage, prw, g, rowbytes, bar);
+        row_copy(s_fr + ROWS_STAGE * stage, rrow, g, op.np, rowbytes, bar);
+        row_copy(s_fp + ROWS_STAGE * stage, prw, g, op.np, rowbytes, bar);
         if (xin) {
             if (fx) bulk_g2s_hint(s_fx + X_STAGE * stage, xvec + xoff, rowbytes, bar, pol_first);
             else bulk_g2s(s_fx + X_STAGE * stage, xvec + xoff, rowbytes, bar);
@@ -141,7 +141,7 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
 
     // ---- coefficient columns and phi factors, staged while the first planes are already in flight ----
     const PlaneSetDev ps = {op.E, op.F, op.AR, op.AT, op.Dinv};
-    stage_coefs<TJ, UNIFORM>(sm.c, g, op, ps);
+    stage_coefs<TJ, UNIFORM>(sm.c, g, op, ps, mp.vp, mp.wp, mp.ip);
     __syncthreads();                            // coefficient columns visible
 
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;

@@ -139,7 +139,7 @@ k_stencil_tma(OpDev op, StencilParams mp)
         const unsigned bytes = (urow ? tx_u : 0u) + (xin ? tx_x : 0u);
         if (bytes == 0) { mbar_arrive(bar); return; }
         mbar_arrive_expect_tx(bar, bytes);
-        if (urow) row_copy(s_ring + SLOT_BYTES * slot, urow, g, rowbytes, bar);
+        if (urow) row_copy(s_ring + SLOT_BYTES * slot, urow, g, op.np, rowbytes, bar);
         if (xin) {
             const unsigned dst = s_xf + XSTAGE * xs;
             if (has1) bulk_g2s(dst, x1p + xoff, rowbytes, bar);
@@ -150,7 +150,7 @@ k_stencil_tma(OpDev op, StencilParams mp)
     if (lane == 0)
         for (int pl = 0; pl < DEPTH && pl < g.nsteps; pl++) produce(pl, pl, pl);
 
-    stage_coefs<TJ, UNIFORM>(sm.c, g, op, mp.ps);
+    stage_coefs<TJ, UNIFORM>(sm.c, g, op, mp.ps, mp.t.vp, mp.t.wp, mp.t.ip);
     __syncthreads();                                        // coefficient columns visible
 
     const double2 zero2 = make_double2(0.0, 0.0);

@@ -56,11 +56,19 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     asm volatile("mov.u64 %0, %%globaltimer;\n" : "=l"(t));
     return t;
 }
+// the same with a suspend-time hint (ns): the warp may sleep that long in hardware unless the phase completes first
+__device__ __forceinline__ bool mbar_try_wait_hint(unsigned bar, unsigned parity, unsigned ns)
+{
+    unsigned ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+                 : "=r"(ok) : "r"(bar), "r"(parity), "r"(ns) : "memory");
+    return ok != 0;
+}
 __device__ __noinline__ void mbar_wait_slow(unsigned bar, unsigned parity, int *fault)
 {
     unsigned long long t0 = 0;
     for (unsigned polls = 1;; polls++) {
-        if (mbar_try_wait(bar, parity)) return;
+        if (mbar_try_wait_hint(bar, parity, 20000u)) return;   // polling warps took 12 % of the stencil kernel's issue slots
         if ((polls & 1023u) == 0) {
             const unsigned long long t = globaltimer_ns();
             if (t0 == 0) t0 = t;
@@ -184,11 +192,17 @@ __device__ __forceinline__ const double *plane_row(const VecHalo &v, const OpDev
 // cell k0 of the row.  (Round 2: five separate copies per vector and row were 21 % of K1's instructions.)
 constexpr int ROW_V2 = 66;
 constexpr unsigned ROW_BYTES = ROW_V2 * 16;
-__device__ __forceinline__ void row_copy(unsigned dst, const double *row_k0, const TileGeom &g, unsigned rowbytes, unsigned bar)
+__device__ __forceinline__ void row_copy(unsigned dst, const double *row_k0, const TileGeom &g, int op_np, unsigned rowbytes, unsigned bar)
 {
     if (g.wrapless) {
         bulk_g2s(dst, row_k0 - 2, rowbytes + 32u, bar);
-    } else {
+    } else if (g.k0 > 0) {                               // last tile of the row: only the right pair wraps
+        bulk_g2s(dst, row_k0 - 2, rowbytes + 16u, bar);
+        bulk_g2s(dst + 16u + rowbytes, row_k0 + (g.kr - g.k0), 16u, bar);
+    } else if (g.tkeff < op_np) {                        // first tile: only the left pair wraps
+        bulk_g2s(dst + 16u, row_k0, rowbytes + 16u, bar);
+        bulk_g2s(dst, row_k0 + (g.kl - 1 - g.k0), 16u, bar);
+    } else {                                             // the tile is the whole row
         bulk_g2s(dst + 16u, row_k0, rowbytes, bar);
         bulk_g2s(dst, row_k0 + (g.kl - 1 - g.k0), 16u, bar);
         bulk_g2s(dst + 16u + rowbytes, row_k0 + (g.kr - g.k0), 16u, bar);
@@ -210,8 +224,12 @@ struct PlaneSetDev {                         // which planes the stencil uses (d
 };
 
 // One global latency, then LDS broadcasts.  Coefficient planes are global: plane index op.i_lo + local.
+// Uniform phi: vp, wp, ip are constants, so the per-row products the stencil needs are formed HERE, once per block:
+//   cE <- vp E + F wp (the diagonal d),  cF <- F ip,  cAR <- vp AR,  cAT <- vp AT
+// and the stencil of a cell is 1 mul + 4 fma + 1 add + 1 fma instead of 11 operations.
 template <int TJ, bool UNIFORM, class C>
-__device__ __forceinline__ void stage_coefs(C &sm, const TileGeom &g, const OpDev &op, const PlaneSetDev &ps)
+__device__ __forceinline__ void stage_coefs(C &sm, const TileGeom &g, const OpDev &op, const PlaneSetDev &ps, double vp,
+                                            double wp, double ip)
 {
     constexpr int NW = TJ + 2, NT = NW * 32;
     for (int e = g.tid; e < g.nsteps * NW; e += NT) {
@@ -219,11 +237,14 @@ __device__ __forceinline__ void stage_coefs(C &sm, const TileGeom &g, const OpDe
         const int ii = op.i_lo + g.first + pl, jj = g.jt * TJ + wr - 1;
         const bool in = ii >= 0 && ii < op.nr_glob && jj >= 0 && jj < op.nt;
         const int row = ii * op.nt + jj;
-        sm.cE[pl][wr] = in ? __ldg(ps.E + row) : 0.0;
-        sm.cF[pl][wr] = in ? __ldg(ps.F + row) : 0.0;
+        const double E = in ? __ldg(ps.E + row) : 0.0, F = in ? __ldg(ps.F + row) : 0.0;
+        const double AR = (ii >= 0 && ii <= op.nr_glob && jj >= 0 && jj < op.nt) ? __ldg(ps.AR + row) : 0.0;
+        const double AT = (ii >= 0 && ii < op.nr_glob && jj >= 0 && jj <= op.nt) ? __ldg(ps.AT + ii * (op.nt + 1) + jj) : 0.0;
+        sm.cE[pl][wr] = UNIFORM ? fma(vp, E, F * wp) : E;
+        sm.cF[pl][wr] = UNIFORM ? F * ip : F;
         sm.cD[pl][wr] = (in && ps.D) ? __ldg(ps.D + row) : 0.0;
-        sm.cAR[pl][wr] = (ii >= 0 && ii <= op.nr_glob && jj >= 0 && jj < op.nt) ? __ldg(ps.AR + row) : 0.0;
-        sm.cAT[pl][wr] = (ii >= 0 && ii < op.nr_glob && jj >= 0 && jj <= op.nt) ? __ldg(ps.AT + ii * (op.nt + 1) + jj) : 0.0;
+        sm.cAR[pl][wr] = UNIFORM ? vp * AR : AR;
+        sm.cAT[pl][wr] = UNIFORM ? vp * AT : AT;
     }
     if (!UNIFORM)
         for (int e = g.tid; e < TILE_TK + 2; e += NT) {
@@ -237,6 +258,7 @@ __device__ __forceinline__ void stage_coefs(C &sm, const TileGeom &g, const OpDe
 // phi factors of cell e (index into the staged arrays = cell - k0 + 1); uniform meshes use the kernel constants
 template <bool UNIFORM, class C>
 struct PhiFac {
+    static constexpr bool uniform = UNIFORM;
     const C &sm;
     double vp, wp, ip;
     __device__ __forceinline__ double VP(int e) const { return UNIFORM ? vp : sm.phv[e]; }
@@ -263,10 +285,15 @@ template <class PF>
 __device__ __forceinline__ double2 stencil_half(const PF &ph, int e, const RowCoefs &c, double2 um, double2 uc, double2 un,
                                                 double2 ujm, double2 ujp, double ukm, double ukp)
 {
-    const double d0 = fma(ph.VP(e), c.Ec, c.Fc * ph.WP(e)), d1 = fma(ph.VP(e + 1), c.Ec, c.Fc * ph.WP(e + 1));
     const double sx = c.ARm * um.x + c.ARp * un.x + c.ATm * ujm.x + c.ATp * ujp.x;
     const double sy = c.ARm * um.y + c.ARp * un.y + c.ATm * ujm.y + c.ATp * ujp.y;
     double2 s;
+    if (PF::uniform) {                       // the staged coefficients already hold d, vp AR, vp AT, F ip (stage_coefs)
+        s.x = fma(-c.Fc, uc.y + ukm, c.Ec * uc.x - sx);
+        s.y = fma(-c.Fc, ukp + uc.x, c.Ec * uc.y - sy);
+        return s;
+    }
+    const double d0 = fma(ph.VP(e), c.Ec, c.Fc * ph.WP(e)), d1 = fma(ph.VP(e + 1), c.Ec, c.Fc * ph.WP(e + 1));
     s.x = d0 * uc.x - ph.VP(e) * sx - c.Fc * (ph.IP(e) * uc.y + ph.IP(e - 1) * ukm);
     s.y = d1 * uc.y - ph.VP(e + 1) * sy - c.Fc * (ph.IP(e + 1) * ukp + ph.IP(e) * uc.x);
     return s;
