@@ -147,10 +147,16 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
     double acc = 0.0;
-    int stage = 0;                              // t % DEPTH
 
-    for (int t = 0; t < g.nsteps; t++) {
-        const int rs = t & 3, rsp = (t + 3) & 3;
+    // The plane loop is unrolled by the ring length (4), so that the ring slot, its barrier and (when DEPTH divides
+    // 4) the FIFO stage and its phase are compile-time: no slot arithmetic and no register rotation inside a step.
+    for (int q4 = 0; 4 * q4 < g.nsteps; q4++) {
+#pragma unroll
+      for (int u = 0; u < 4; u++) {
+        const int t = 4 * q4 + u;
+        if (t >= g.nsteps) break;
+        const int rs = u, rsp = (u + 3) & 3;
+        const int stage = (4 % DEPTH == 0) ? u % DEPTH : t % DEPTH;
         const int ii = g.first + t;
         const bool plane_ok = (unsigned)(op.i_lo + ii) < (unsigned)op.nr_glob;
         const bool own = t >= 1 && t <= g.nsteps - 2;       // a plane of this block: p_new and x are stored
@@ -219,7 +225,7 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
         if (t >= 2) qrow += plane;
         am = ac; ac = an; bm = bc; bc = bn;
         hl_c = hl_n; hr_c = hr_n;
-        stage = stage + 1 == DEPTH ? 0 : stage + 1;
+      }
     }
     double a1[1] = {acc};
     if (grid_sum<NT, 1>(a1, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 1], sm.red) && threadIdx.x == 0)

@@ -157,11 +157,19 @@ k_stencil_tma(OpDev op, StencilParams mp)
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
     double acc[2] = {0.0, 0.0};                             // K2R: rho', rr
-    int slot = 0, slot_prev = R - 1, xs = 0;                // t % R, (t - 1) % R, t % DEPTH
-    int pslot = DEPTH, puse = 0;                            // (t + DEPTH) % R and (t + DEPTH) / R: slot of the plane produced at step t, and which use of that slot it is
-    unsigned full_par = 0;                                  // (t / R) & 1
-
-    for (int t = 0; t < g.nsteps; t++) {
+    // The plane loop is unrolled by the ring length R, so that ring slots, their barriers and (when DEPTH divides R)
+    // the extras' stage are compile-time: no slot arithmetic and no register rotation inside a step.
+    for (int t0 = 0; t0 < g.nsteps; t0 += R) {
+      const int use0 = t0 / R;                              // how often the ring has been filled before this trip
+      const unsigned full_par = (unsigned)use0 & 1u;
+#pragma unroll
+      for (int u = 0; u < R; u++) {
+        const int t = t0 + u;
+        if (t >= g.nsteps) break;
+        const int slot = u, slot_prev = (u + R - 1) % R;    // t % R, (t - 1) % R
+        const int pslot = (u + DEPTH) % R;                  // slot of the plane produced at step t
+        const int puse = use0 + (u + DEPTH >= R ? 1 : 0);   // which use of that slot it is: (t + DEPTH) / R
+        const int xs = (R % DEPTH == 0) ? u % DEPTH : t % DEPTH;   // t % DEPTH: stage of the extras consumed at step t
         const int ii = g.first + t;
         const bool plane_ok = (unsigned)(op.i_lo + ii) < (unsigned)op.nr_glob;
         mbar_wait(s_full + 8u * slot, full_par, fault);     // plane ii: every row has landed
@@ -231,10 +239,7 @@ k_stencil_tma(OpDev op, StencilParams mp)
         }
         am = ac; ac = an; bm = bc; bc = bn;
         hl_c = hl_n; hr_c = hr_n;
-        slot_prev = slot;
-        if (++slot == R) { slot = 0; full_par ^= 1u; }
-        if (++pslot == R) { pslot = 0; ++puse; }
-        if (++xs == DEPTH) xs = 0;
+      }
     }
     if (EPI == EPI_K2R) {
         if (grid_sum<NT, 2>(acc, part_base(mp.w, rhs), mp.w.pstride, &mp.w.tickets[rhs * 4 + 2], sm.red) && threadIdx.x == 0)
