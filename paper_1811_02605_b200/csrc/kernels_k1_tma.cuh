@@ -148,13 +148,10 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     double hl_c = 0.0, hr_c = 0.0;
     double acc = 0.0;
 
-    // The plane loop is unrolled by the ring length (4), so that the ring slot, its barrier and (when DEPTH divides
-    // 4) the FIFO stage and its phase are compile-time: no slot arithmetic and no register rotation inside a step.
-    for (int q4 = 0; 4 * q4 < g.nsteps; q4++) {
-#pragma unroll
-      for (int u = 0; u < 4; u++) {
-        const int t = 4 * q4 + u;
-        if (t >= g.nsteps) break;
+    // One step = one plane.  `uc` is the ring slot t % 4: a compile-time constant in the unrolled trips (run_trip), a
+    // run-time value in the tail; with it (when DEPTH divides 4) the FIFO stage is compile-time too.
+    auto step = [&](const int t, const int, auto uc) {
+        const int u = uc;
         const int rs = u, rsp = (u + 3) & 3;
         const int stage = (4 % DEPTH == 0) ? u % DEPTH : t % DEPTH;
         const int ii = g.first + t;
@@ -225,8 +222,10 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
         if (t >= 2) qrow += plane;
         am = ac; ac = an; bm = bc; bc = bn;
         hl_c = hl_n; hr_c = hr_n;
-      }
-    }
+    };
+    int t0 = 0;
+    for (; t0 + 4 <= g.nsteps; t0 += 4) run_trip(step, t0, 0, std::make_integer_sequence<int, 4>{});
+    for (int t = t0; t < g.nsteps; t++) step(t, 0, t - t0);
     double a1[1] = {acc};
     if (grid_sum<NT, 1>(a1, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 1], sm.red) && threadIdx.x == 0)
         reduction_done<ROLE_K1, 1>(w, rhs, a1, cond, use_cond);

@@ -157,15 +157,11 @@ k_stencil_tma(OpDev op, StencilParams mp)
     double2 am = zero2, ac = zero2, bm = zero2, bc = zero2;
     double hl_c = 0.0, hr_c = 0.0;
     double acc[2] = {0.0, 0.0};                             // K2R: rho', rr
-    // The plane loop is unrolled by the ring length R, so that ring slots, their barriers and (when DEPTH divides R)
-    // the extras' stage are compile-time: no slot arithmetic and no register rotation inside a step.
-    for (int t0 = 0; t0 < g.nsteps; t0 += R) {
-      const int use0 = t0 / R;                              // how often the ring has been filled before this trip
-      const unsigned full_par = (unsigned)use0 & 1u;
-#pragma unroll
-      for (int u = 0; u < R; u++) {
-        const int t = t0 + u;
-        if (t >= g.nsteps) break;
+    // One step = one plane.  `uc` is the ring slot t % R: a compile-time constant in the unrolled trips (run_trip),
+    // a run-time value in the tail.
+    auto step = [&](const int t, const int use0, auto uc) {
+        const int u = uc;
+        const unsigned full_par = (unsigned)use0 & 1u;      // use0 = t / R: how often the ring was filled before
         const int slot = u, slot_prev = (u + R - 1) % R;    // t % R, (t - 1) % R
         const int pslot = (u + DEPTH) % R;                  // slot of the plane produced at step t
         const int puse = use0 + (u + DEPTH >= R ? 1 : 0);   // which use of that slot it is: (t + DEPTH) / R
@@ -239,8 +235,10 @@ k_stencil_tma(OpDev op, StencilParams mp)
         }
         am = ac; ac = an; bm = bc; bc = bn;
         hl_c = hl_n; hr_c = hr_n;
-      }
-    }
+    };
+    int t0 = 0;
+    for (; t0 + R <= g.nsteps; t0 += R) run_trip(step, t0, t0 / R, std::make_integer_sequence<int, R>{});
+    for (int t = t0; t < g.nsteps; t++) step(t, t0 / R, t - t0);
     if (EPI == EPI_K2R) {
         if (grid_sum<NT, 2>(acc, part_base(mp.w, rhs), mp.w.pstride, &mp.w.tickets[rhs * 4 + 2], sm.red) && threadIdx.x == 0)
             reduction_done<ROLE_K2, 2>(mp.w, rhs, acc, mp.cond, mp.use_cond);

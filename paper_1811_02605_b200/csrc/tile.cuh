@@ -10,6 +10,7 @@
 // neighbour slabs and are read through `VecHalo` pointers (peer mappings on a real node); coefficient planes are GLOBAL
 // and indexed by op.i_lo + local plane.
 #pragma once
+#include <utility>
 #include "common.cuh"
 
 namespace mas {
@@ -311,6 +312,20 @@ __device__ __forceinline__ PhiNb phi_neighbours(double2 ac, double2 bc, int lane
     n.mA = __shfl_sync(0xffffffffu, ac.y, lm); n.mB = __shfl_sync(0xffffffffu, bc.y, lm);
     n.pA = __shfl_sync(0xffffffffu, ac.x, lp); n.pB = __shfl_sync(0xffffffffu, bc.x, lp);
     return n;
+}
+
+// One trip of a plane loop unrolled by N: calls step(t0 + I, trip, SlotC<I>) for I = 0..N-1 with NO branch
+// between the steps, so that inside a trip ring slots are compile-time and the compiler renames the plane registers
+// (u_{i-1}, u_i, u_{i+1}) instead of moving them; the remaining (< N) steps of a block run the same step body with a
+// run-time slot.
+template <int V>
+struct SlotC {                               // a compile-time slot index that converts to int in device code
+    __host__ __device__ constexpr operator int() const { return V; }
+};
+template <class F, int... I>
+__device__ __forceinline__ void run_trip(F &step, int t0, int trip, std::integer_sequence<int, I...>)
+{
+    (step(t0 + I, trip, SlotC<I>{}), ...);
 }
 
 // r-chunk length of a marching kernel: minimise rounds x (planes per block + halo planes + start-up), ties ->
