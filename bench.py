@@ -646,6 +646,25 @@ def main():
         }
         if nrhs > 1:
             line["iteration"]["note"] = "per right-hand-side iteration"
+        if world == 1 and nrhs == 1 and args.workload == "c4":
+            # context beside the headline: the same system solved to rtol 1e-9 with the paper's two preconditioners
+            # (PAPER.md:65, 80, 98-100); one warm-up solve and one timed solve each, CUDA events on the launching stream
+            tts = {}
+            for pc in (1, 2):
+                gpu.set_preconditioner(pc)
+                for timed in (False, True):
+                    x.zero_()
+                    torch.cuda.synchronize()
+                    e0.record(stream)
+                    st_p, k_p, _ = gpu.solve(b, x, 1e-9, 5000, want_hist=False)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                tts[f"pc{pc}"] = {"ms": e0.elapsed_time(e1), "iterations": k_p, "status": st_p}
+            gpu.set_preconditioner(args.precond)
+            tts["pc2_speedup"] = tts["pc1"]["ms"] / tts["pc2"]["ms"]
+            tts["what"] = ("the same system solved to rtol 1e-9 from x0 = 0: PC1 point Jacobi vs PC2 block-Jacobi ILU(0) "
+                           "over phi-line domains (not part of `value`)")
+            line["time_to_solution_rtol_1e-9"] = tts
         if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
             from oracle import ref                      # config 3 = the oracle's FULL solve
             op = ref.RefOperator(prob.mesh, dt, prob.nu_kind, prob.nu, prob.bc)

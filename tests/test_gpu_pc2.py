@@ -118,11 +118,12 @@ def test_pc2_config4_full_size_first_40_iterations():
     _check(gpu, oref, b, None, 0.0, 40, "pc2 c4/40")
 
 
-def test_pc2_config5_chain_first_3_solves_set_dt_refactors():
+@pytest.mark.parametrize("full", [False, True])
+def test_pc2_config5_chain_first_3_solves_set_dt_refactors(full):
+    """config 5's chain (dt varies per step, warm start) with PC2, at a reduced size and at 192 x 256 x 384"""
     import torch
-    prob = configs.make("c5", shape=(48, 64, 96))
-    s1 = H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
-    dt0 = 100.0 / s1
+    prob = configs.make("c5") if full else configs.make("c5", shape=(48, 64, 96))
+    dt0 = prob.dt_for(100.0) if full else 100.0 / H.oracle_s1(prob.mesh, prob.nu_kind, prob.nu)
     oref, gpu = H.both_ops(prob.mesh, dt0, prob.nu_kind, prob.nu)
     gpu.set_preconditioner(2)
     chain = configs.Chain(prob, 100)
