@@ -53,20 +53,21 @@ __global__ void k_pc2_factor(OpDev op, double *dinvT, int M)
     double *out = dinvT + (size_t)line * 32 * M;
     const int np = op.np;
     auto diag = [&](int k) { return fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k)); };
-    const double piv0 = diag(0);
-    double piv = piv0;
-    out[pc2_slot(0, M)] = 1.0 / piv;
-    for (int k = 1; k < np; k++) {
+    double inv = 1.0 / diag(0);                             // 1 / piv_{k-1}; ONE division per cell: l_k = c / piv is formed as c * (1 / piv),
+    const double inv0 = inv;                                // the product the line kernel uses as well
+    double even = inv;                                      // 1/piv of the last even cell: cells (k, k + 1), k even, are
+    for (int k = 1; k < np; k++) {                          // adjacent in the chunk order and stored as one 16-byte pair
         double a = diag(k);
-        if (k == np - 1) {                              // lower entries in ascending column order: the wrap (column 0) first
+        if (k == np - 1) {                                  // lower entries in ascending column order: the wrap (column 0) first
             const double w = -F * __ldg(op.ip + np - 1);
-            a -= (w / piv0) * w;
+            a -= (w * inv0) * w;
         }
         const double c = -F * __ldg(op.ip + k - 1);
-        piv = a - (c / piv) * c;
-        out[pc2_slot(k, M)] = 1.0 / piv;
+        inv = 1.0 / (a - (c * inv) * c);
+        if (k & 1) *reinterpret_cast<double2 *>(out + pc2_slot(k - 1, M)) = make_double2(even, inv);
+        else even = inv;
     }
-    for (int k = np; k < 32 * M; k++) out[pc2_slot(k, M)] = 0.0;
+    for (int k = np; k < 32 * M; k += 2) *reinterpret_cast<double2 *>(out + pc2_slot(k, M)) = make_double2(0.0, 0.0);
 }
 
 // ---------------------------------------------------------------------------------------------
