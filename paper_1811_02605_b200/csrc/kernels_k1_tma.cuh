@@ -235,8 +235,7 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
 struct K1TmaTile {
     int tj, depth, minb;
 };
-static const K1TmaTile kK1TmaTiles[] = {{14, 2, 1}, {8, 2, 2}, {6, 2, 2}, {8, 3, 1}, {10, 2, 1}, {16, 2, 1}, {12, 2, 1},
-                                          {8, 4, 1}, {6, 3, 2}, {10, 3, 1}, {12, 3, 1}};
+static const K1TmaTile kK1TmaTiles[] = {{14, 2, 1}, {8, 2, 2}, {6, 2, 2}, {8, 3, 1}, {10, 2, 1}, {16, 2, 1}, {12, 2, 1}};
 inline int k1_tma_num_tiles() { return (int)(sizeof(kK1TmaTiles) / sizeof(kK1TmaTiles[0])); }
 
 template <int TJ, int DEPTH, int MINB>
@@ -262,11 +261,7 @@ inline void k1_tma_configure(int nr, int nt, int np, int uniform, bool noq, int 
         case 3: k1_tma_pick<8, 3, 1>(uniform, noq, func, block, smem); break;
         case 4: k1_tma_pick<10, 2, 1>(uniform, noq, func, block, smem); break;
         case 5: k1_tma_pick<16, 2, 1>(uniform, noq, func, block, smem); break;
-        case 6: k1_tma_pick<12, 2, 1>(uniform, noq, func, block, smem); break;
-        case 7: k1_tma_pick<8, 4, 1>(uniform, noq, func, block, smem); break;
-        case 8: k1_tma_pick<6, 3, 2>(uniform, noq, func, block, smem); break;
-        case 9: k1_tma_pick<10, 3, 1>(uniform, noq, func, block, smem); break;
-        default: k1_tma_pick<12, 3, 1>(uniform, noq, func, block, smem); break;
+        default: k1_tma_pick<12, 2, 1>(uniform, noq, func, block, smem); break;
     }
     mp->nkt = (np + TILE_TK - 1) / TILE_TK;
     mp->njt = (nt + T.tj - 1) / T.tj;

@@ -268,10 +268,9 @@ inline void stencil_tma_pick(bool uniform, int epi, const void **func, dim3 *blo
     cudaFuncSetAttribute(*func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem);
 }
 
-inline int stencil_num_tiles() { return 11; }
+inline int stencil_num_tiles() { return 6; }
 
-// tile ids -> (TJ, DEPTH, min blocks/SM): 0 (6,2,2), 1 (8,2,2), 2 (14,2,1), 3 (10,2,1), 4 (8,3,1), 5 (12,3,1), 6 (8,4,2), 7 (8,3,2),
-// 8 (6,4,2), 9 (10,4,1), 10 (14,4,1)
+// tile ids -> (TJ, DEPTH, min blocks/SM): 0 (6,2,2), 1 (8,2,2), 2 (14,2,1), 3 (10,2,1), 4 (8,3,1), 5 (12,3,1)
 inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int tile, int num_sms, int ci_force, int ny,
                               StencilParams *mp, const void **func, dim3 *grid, dim3 *block, size_t *smem)
 {
@@ -282,12 +281,7 @@ inline void stencil_configure(int nr, int nt, int np, int uniform, int epi, int 
         case 2: tj = 14; stencil_tma_pick<14, 2, 1>(uniform, epi, func, block, smem); break;
         case 3: tj = 10; stencil_tma_pick<10, 2, 1>(uniform, epi, func, block, smem); break;
         case 4: tj = 8; stencil_tma_pick<8, 3, 1>(uniform, epi, func, block, smem); break;
-        case 5: tj = 12; stencil_tma_pick<12, 3, 1>(uniform, epi, func, block, smem); break;
-        case 6: tj = 8; stencil_tma_pick<8, 4, 2>(uniform, epi, func, block, smem); break;
-        case 7: tj = 8; stencil_tma_pick<8, 3, 2>(uniform, epi, func, block, smem); break;
-        case 8: tj = 6; stencil_tma_pick<6, 4, 2>(uniform, epi, func, block, smem); break;
-        case 9: tj = 10; stencil_tma_pick<10, 4, 1>(uniform, epi, func, block, smem); break;
-        default: tj = 14; stencil_tma_pick<14, 4, 1>(uniform, epi, func, block, smem); break;
+        default: tj = 12; stencil_tma_pick<12, 3, 1>(uniform, epi, func, block, smem); break;
     }
     mp->t.nkt = (np + TILE_TK - 1) / TILE_TK;
     mp->t.njt = (nt + tj - 1) / tj;
