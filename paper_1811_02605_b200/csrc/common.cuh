@@ -144,22 +144,4 @@ __device__ __forceinline__ bool grid_sum(double (&v)[NP], double *partials, int 
     return true;
 }
 
-// Thread -> (row, vector) mapping without per-element division: a block of NT threads covers
-// RB = NT/nvc rows of nvc = min(nv, NT) vectors at a time; longer rows are walked in steps of nvc.
-struct RowMap {
-    int rl, kv0, nvc, rb;
-    bool idle;
-};
-template <int NT>
-__device__ __forceinline__ RowMap row_map(int nv)
-{
-    RowMap m;
-    m.nvc = nv < NT ? nv : NT;
-    m.rb = NT / m.nvc;
-    m.rl = threadIdx.x / m.nvc;
-    m.kv0 = threadIdx.x - m.rl * m.nvc;
-    m.idle = m.rl >= m.rb;
-    return m;
-}
-
 }  // namespace mas

@@ -186,34 +186,28 @@ __global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditio
     double *rv = w.r + rhs * w.vstride, *p0 = w.p0 + rhs * w.vstride;
     const double *qv0 = w.q + rhs * w.vstride;
     const int crow0 = op.i_lo * op.nt;
-    const RowMap m = row_map<NT>(op.nv);
     double acc[3] = {0.0, 0.0, 0.0};   // bb, rr, rho
-    if (!m.idle)
-        for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
-            const int row = rowbase + m.rl;
-            if (row >= op.nrows) break;
-            const int crow = row + crow0;
-            const double E = __ldg(op.E + crow), F = __ldg(op.F + crow), V2 = __ldg(op.V2 + crow);
-            const double dinv = __ldg(op.Dinv + crow);
-            const size_t base = (size_t)row * op.np;
-            for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
-                const int k = 2 * kv;
-                const double vp0 = __ldg(op.vp + k), vp1 = __ldg(op.vp + k + 1);
-                const double d0 = fma(vp0, E, F * __ldg(op.wp + k)), d1 = fma(vp1, E, F * __ldg(op.wp + k + 1));
-                const size_t cell = base + k;
-                const double2 bv = ld2(b, cell), qv = ld2(qv0, cell);
-                const double bs0 = V2 * vp0 * bv.x, bs1 = V2 * vp1 * bv.y;
-                double2 r;
-                r.x = bs0 - qv.x;
-                r.y = bs1 - qv.y;
-                st2(rv, cell, r);
-                st2(p0, cell, make_double2(0.0, 0.0));
-                acc[0] += bs0 * bs0 + bs1 * bs1;
-                acc[1] += r.x * r.x + r.y * r.y;
-                acc[2] += UNIFORM ? r.x * (r.x * dinv) + r.y * (r.y * dinv)      // same z as K1/K2 use
-                                  : r.x * (r.x / d0) + r.y * (r.y / d1);
-            }
-        }
+    const int total = op.nrows * op.nv;                     // flat sweep over 16-byte vectors (see k2_vec)
+    for (int v = blockIdx.x * NT + threadIdx.x; v < total; v += gridDim.x * NT) {
+        const int row = v / op.nv, k = 2 * (v - row * op.nv);
+        const int crow = row + crow0;
+        const double E = __ldg(op.E + crow), F = __ldg(op.F + crow), V2 = __ldg(op.V2 + crow);
+        const double dinv = __ldg(op.Dinv + crow);
+        const double vp0 = __ldg(op.vp + k), vp1 = __ldg(op.vp + k + 1);
+        const double d0 = fma(vp0, E, F * __ldg(op.wp + k)), d1 = fma(vp1, E, F * __ldg(op.wp + k + 1));
+        const size_t cell = 2 * (size_t)v;
+        const double2 bv = ld2(b, cell), qv = ld2(qv0, cell);
+        const double bs0 = V2 * vp0 * bv.x, bs1 = V2 * vp1 * bv.y;
+        double2 r;
+        r.x = bs0 - qv.x;
+        r.y = bs1 - qv.y;
+        st2(rv, cell, r);
+        st2(p0, cell, make_double2(0.0, 0.0));
+        acc[0] += bs0 * bs0 + bs1 * bs1;
+        acc[1] += r.x * r.x + r.y * r.y;
+        acc[2] += UNIFORM ? r.x * (r.x * dinv) + r.y * (r.y * dinv)      // same z as K1/K2 use
+                          : r.x * (r.x / d0) + r.y * (r.y / d1);
+    }
     if (grid_sum<NT, 3>(acc, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 0], sh) && threadIdx.x == 0)
         reduction_done<ROLE_INIT, 3>(w, rhs, acc, cond, use_cond);
 }
@@ -241,47 +235,40 @@ OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond,
     double *rvec = w.r + rhs * w.vstride;
     const double *qvec = w.q + rhs * w.vstride;
     const int crow0 = op.i_lo * op.nt;
-    const RowMap m = row_map<NT>(op.nv);
     double acc[2] = {0.0, 0.0};   // rho', rr
-    // Two row groups per trip (A and B, one grid stride apart): their loads are issued together, which
-    // doubles the bytes in flight per thread -- K2 has no other latency hiding than memory parallelism.
-    auto body = [&](int row, int kv, double2 rv, double2 qv, double E, double F, double dinv) {
-        const size_t cell = (size_t)row * op.np + 2 * kv;
+    // Flat sweep over the 16-byte vectors of the whole array (vector v = cells 2v, 2v+1; its row is v / nv), so that
+    // every thread works whatever the row length is (a row-wise mapping idles a quarter of the block at np = 384).
+    // Two vectors per trip (A and B, one grid stride apart): their loads are issued together, which doubles the
+    // bytes in flight per thread -- K2 has no other latency hiding than memory parallelism.
+    auto body = [&](int v, double2 rv, double2 qv) {
+        const int row = v / op.nv;
         rv.x = fma(-alpha, qv.x, rv.x);
         rv.y = fma(-alpha, qv.y, rv.y);
-        st2(rvec, cell, rv);
+        st2(rvec, 2 * (size_t)v, rv);
         double z0, z1;
-        if (UNIFORM) { z0 = rv.x * dinv; z1 = rv.y * dinv; }
-        else {
-            const int k = 2 * kv;
+        if (UNIFORM) {
+            const double dinv = __ldg(op.Dinv + crow0 + row);
+            z0 = rv.x * dinv; z1 = rv.y * dinv;
+        } else {
+            const int k = 2 * (v - row * op.nv);
+            const double E = __ldg(op.E + crow0 + row), F = __ldg(op.F + crow0 + row);
             z0 = rv.x / fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k));
             z1 = rv.y / fma(__ldg(op.vp + k + 1), E, F * __ldg(op.wp + k + 1));
         }
         acc[0] += rv.x * z0 + rv.y * z1;
         acc[1] += rv.x * rv.x + rv.y * rv.y;
     };
-    if (!m.idle) {
-        const int stride = gridDim.x * m.rb;
+    {
+        const int total = op.nrows * op.nv, stride = gridDim.x * NT;     // N < 2^31 cells => total < 2^30
         const double2 zero = make_double2(0.0, 0.0);
-        for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += 2 * stride) {
-            int rowA = rowbase + m.rl, rowB = rowA + stride;
-            const bool okA = rowA < op.nrows, okB = rowB < op.nrows;
-            if (!okA) break;
-            if (reverse) { rowA = op.nrows - 1 - rowA; rowB = op.nrows - 1 - rowB; }
-            double EA = 0, FA = 0, dA = 0, EB = 0, FB = 0, dB = 0;
-            if (UNIFORM) { dA = __ldg(op.Dinv + crow0 + rowA); if (okB) dB = __ldg(op.Dinv + crow0 + rowB); }
-            else {
-                EA = __ldg(op.E + crow0 + rowA); FA = __ldg(op.F + crow0 + rowA);
-                if (okB) { EB = __ldg(op.E + crow0 + rowB); FB = __ldg(op.F + crow0 + rowB); }
-            }
-            const size_t baseA = (size_t)rowA * op.np, baseB = okB ? (size_t)rowB * op.np : 0;
-            for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
-                const size_t cA = baseA + 2 * kv, cB = baseB + 2 * kv;
-                const double2 rA = ld2(rvec, cA), qA = ld2(qvec, cA);
-                const double2 rB = okB ? ld2(rvec, cB) : zero, qB = okB ? ld2(qvec, cB) : zero;
-                body(rowA, kv, rA, qA, EA, FA, dA);
-                if (okB) body(rowB, kv, rB, qB, EB, FB, dB);
-            }
+        for (int v0 = blockIdx.x * NT + threadIdx.x; v0 < total; v0 += 2 * stride) {
+            int vA = v0, vB = v0 + stride;
+            const bool okB = vB < total;
+            if (reverse) { vA = total - 1 - vA; vB = total - 1 - vB; }
+            const double2 rA = ld2(rvec, 2 * (size_t)vA), qA = ld2(qvec, 2 * (size_t)vA);
+            const double2 rB = okB ? ld2(rvec, 2 * (size_t)vB) : zero, qB = okB ? ld2(qvec, 2 * (size_t)vB) : zero;
+            body(vA, rA, qA);
+            if (okB) body(vB, rB, qB);
         }
     }
     if (grid_sum<NT, 2>(acc, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 2], sh) && threadIdx.x == 0)
@@ -299,20 +286,14 @@ __global__ void __launch_bounds__(NT) k_xtail(OpDev op, Work w)
     if (alpha == 0.0) return;
     const double *p = ((st->k & 1) ? w.p1 : w.p0) + rhs * w.vstride;
     double *x = w.args->x[rhs];
-    const RowMap m = row_map<NT>(op.nv);
-    if (m.idle) return;
-    for (int rowbase = blockIdx.x * m.rb; rowbase < op.nrows; rowbase += gridDim.x * m.rb) {
-        const int row = rowbase + m.rl;
-        if (row >= op.nrows) break;
-        const size_t base = (size_t)row * op.np;
-        for (int kv = m.kv0; kv < op.nv; kv += m.nvc) {
-            const size_t cell = base + 2 * kv;
-            double2 xv = ld2(x, cell);
-            const double2 pv = ld2(p, cell);
-            xv.x = fma(alpha, pv.x, xv.x);
-            xv.y = fma(alpha, pv.y, xv.y);
-            st2(x, cell, xv);
-        }
+    const int total = op.nrows * op.nv;
+    for (int v = blockIdx.x * NT + threadIdx.x; v < total; v += gridDim.x * NT) {
+        const size_t cell = 2 * (size_t)v;
+        double2 xv = ld2(x, cell);
+        const double2 pv = ld2(p, cell);
+        xv.x = fma(alpha, pv.x, xv.x);
+        xv.y = fma(alpha, pv.y, xv.y);
+        st2(x, cell, xv);
     }
 }
 

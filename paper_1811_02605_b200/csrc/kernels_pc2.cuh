@@ -32,7 +32,7 @@ struct Pc2Dev {
     const double *dinvT;        // [rows][32 * M]  1 / piv, chunk order (pc2_slot)
     const double *ipT;          // [32 * M]        ip[k] in chunk order, 0 beyond np (non-uniform phi only)
     double ip0;                 // uniform phi: 1 / dph_f
-    int M;                      // cells per lane: the smallest of 2, 4, 8, 16, 32 with 32 M >= np
+    int M;                      // cells per lane: the smallest of 4, 8, 12, 16, 24, 32 with 32 M >= np
 };
 
 // where cell k of a line lives in the chunk-ordered arrays: lane l = k / M, slot u = k % M; pairs (u, u + 1) adjacent
@@ -77,11 +77,11 @@ constexpr int PC2_NT = 256, PC2_NWARP = PC2_NT / 32;
 inline size_t pc2_smem(int M) { return (size_t)PC2_NWARP * 32 * (M + 2) * sizeof(double); }
 
 template <int M, bool UNIFORM, bool INIT>
-__global__ void __launch_bounds__(PC2_NT, M >= 32 ? 1 : 2)
+__global__ void __launch_bounds__(PC2_NT, M >= 24 ? 1 : 2)
 k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use_cond, int reverse)
 {
-    constexpr int S = M + 2;                            // chunk stride in the staging buffer (doubles): S/2 is odd for
-    constexpr int H = M / 2;                            // M = 4, 8, 16, 32 => conflict-free 16-byte accesses both ways
+    constexpr int S = M + 2;                            // chunk stride in the staging buffer (doubles): S/2 is odd for every
+    constexpr int H = M / 2;                            // supported M (multiples of 4) => conflict-free 16-byte accesses both ways
     extern __shared__ __align__(16) double pc2_buf[];
     __shared__ double sh[32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -260,16 +260,18 @@ inline const void *pc2_line_pick(int M, bool uniform, bool init)
     switch (M) {
         case 4: return pc2_line_func<4>(uniform, init);
         case 8: return pc2_line_func<8>(uniform, init);
+        case 12: return pc2_line_func<12>(uniform, init);
         case 16: return pc2_line_func<16>(uniform, init);
+        case 24: return pc2_line_func<24>(uniform, init);
         default: return pc2_line_func<32>(uniform, init);
     }
 }
 inline int pc2_chunk(int np)            // 0: unsupported
 {
     if (np < 4 || np > 1024) return 0;
-    int M = 4;
-    while (32 * M < np) M *= 2;
-    return M;
+    for (int M : {4, 8, 12, 16, 24, 32})     // the smallest chunk that covers the line: idle lanes cost bandwidth (np = 384 -> 12)
+        if (32 * M >= np) return M;
+    return 0;
 }
 
 }  // namespace mas

@@ -415,9 +415,7 @@ struct Plan {                        // storage that kernel argument pointers re
 
 int base_grid(const mas_pcg *h, const OpDev &op, const void *func, int nt_block)
 {
-    const int nvc = op.nv < nt_block ? op.nv : nt_block;
-    const int rb = nt_block / nvc;
-    const long long groups = ((long long)op.nrows + rb - 1) / rb;
+    const long long groups = ((long long)op.nrows * op.nv + nt_block - 1) / nt_block;   // blocks of 16-byte vectors
     int occ = 1;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, func, nt_block, 0) != cudaSuccess || occ < 1) {
         cudaGetLastError();
