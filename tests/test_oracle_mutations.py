@@ -1,7 +1,7 @@
 """Mutation check of the oracle's pins (What's weak #3): each single-token mutation of
 oracle/mas_pcg_ref.c -- a dropped factor, a wrong index, a sign, a transposed operand -- is built in a temp
 directory and the mathematical pin tests are run against it; at least one pin must fail.  The pins are the
-ones in tests/test_oracle_pins.py, tests/test_oracle_sts_pins.py and tests/test_oracle_pc2_pins.py; stored oracle outputs (golden files,
+ones in tests/test_oracle_pins.py, test_oracle_sts_pins.py, test_oracle_pc2_pins.py and test_oracle_random_pins.py; stored oracle outputs (golden files,
 the dt calibration file) do NOT count as pins and are excluded (-k / --deselect below).
 
 One mutation is expected to SURVIVE the mathematical pins and is listed as such: the face-nu mean (reading Q3).
@@ -71,7 +71,8 @@ NOT_PINS = ["--deselect", "tests/test_oracle_pins.py::test_calibration_file_matc
 
 
 def _run_pins(repo, first=None):
-    files = ["tests/test_oracle_pins.py", "tests/test_oracle_sts_pins.py", "tests/test_oracle_pc2_pins.py"]
+    files = ["tests/test_oracle_pins.py", "tests/test_oracle_sts_pins.py", "tests/test_oracle_pc2_pins.py",
+             "tests/test_oracle_random_pins.py"]
     if first:
         files = [first] + [f for f in files if f != first]
     cmd = [sys.executable, "-m", "pytest", *files, "-x", "-q",
@@ -87,7 +88,8 @@ def sandbox(tmp_path_factory):
     for d in ("oracle", "mas_inputs"):
         shutil.copytree(os.path.join(ROOT, d), repo / d, ignore=shutil.ignore_patterns("*.so", "__pycache__", "*.tmp"))
     os.makedirs(repo / "tests")
-    for f in ("__init__.py", "helpers.py", "test_oracle_pins.py", "test_oracle_sts_pins.py", "test_oracle_pc2_pins.py"):
+    for f in ("__init__.py", "helpers.py", "test_oracle_pins.py", "test_oracle_sts_pins.py", "test_oracle_pc2_pins.py",
+              "test_oracle_random_pins.py"):
         shutil.copy(os.path.join(ROOT, "tests", f), repo / "tests" / f)
     open(repo / "tests" / "conftest.py", "w").write(
         "import os, sys\nsys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))\n")
