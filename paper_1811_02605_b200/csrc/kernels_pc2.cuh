@@ -74,7 +74,8 @@ __global__ void k_pc2_factor(OpDev op, double *dinvT, int M)
 // the line kernel
 // ---------------------------------------------------------------------------------------------
 constexpr int PC2_NT = 256, PC2_NWARP = PC2_NT / 32;
-inline size_t pc2_smem(int M) { return (size_t)PC2_NWARP * 32 * (M + 2) * sizeof(double); }
+__device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+inline size_t pc2_smem(int M) { return (size_t)PC2_NWARP * (32 * (M + 2) + 2 * 32 * M) * sizeof(double); }   // chunk-order buffer + q, r stage
 
 template <int M, bool UNIFORM, bool INIT>
 __global__ void __launch_bounds__(PC2_NT, M >= 24 ? 1 : 2)
@@ -85,7 +86,10 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
     extern __shared__ __align__(16) double pc2_buf[];
     __shared__ double sh[32];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double2 *buf = reinterpret_cast<double2 *>(pc2_buf + (size_t)warp * 32 * S);   // [lane][S/2] double2
+    double2 *buf = reinterpret_cast<double2 *>(pc2_buf + (size_t)warp * (32 * S + 64 * M));   // [lane][S/2] double2
+    // stage of the NEXT line's q and r (or b): [h][lane] double2 each, filled by cp.async (LDGSTS); a thread reads back
+    // only the slots it copied itself, so cp.async.wait_group is the only synchronisation the stage needs
+    double2 *stq = buf + 16 * S, *str = stq + 32 * H;
     const int rhs = blockIdx.y;
     State *st = w.st + rhs;
     double alpha = 0.0;
@@ -113,23 +117,40 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
     const double ipw = UNIFORM ? pc.ip0 : __ldg(op.ip + np - 1);
     double acc[3] = {0.0, 0.0, 0.0};                            // rho', rr, (init) bb
 
-    for (int ln = blockIdx.x * PC2_NWARP + warp; ln < op.nrows; ln += gridDim.x * PC2_NWARP) {
+    const double *rsrc = INIT ? bvec : rvec;
+    auto prefetch = [&](int ln) {                               // this lane's q and r vectors of line ln -> the stage
+        if (ln < op.nrows) {
+            const size_t b2 = (size_t)(reverse ? op.nrows - 1 - ln : ln) * np;
+#pragma unroll
+            for (int h = 0; h < H; h++) {
+                const int v = lane + 32 * h;
+                if (v < nv) {
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr(stq + h * 32 + lane)), "l"(qvec + b2 + 2 * v) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr(str + h * 32 + lane)), "l"(rsrc + b2 + 2 * v) : "memory");
+                }
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    const int ln0 = blockIdx.x * PC2_NWARP + warp, lstep = gridDim.x * PC2_NWARP;
+    prefetch(ln0);
+    for (int ln = ln0; ln < op.nrows; ln += lstep) {
         const int row = reverse ? op.nrows - 1 - ln : ln;
         const size_t base = (size_t)row * np;
         const double F = __ldg(op.F + row);
-        // ---- all loads of the line first (q, r or b in the natural order, 1/piv in the chunk order): the stores
-        // below may alias them as far as the compiler knows, so loads left between stores would be serialised ----
+        // ---- the line's q and r (or b) were copied into the stage while the previous line was being solved; they
+        // are read into registers and the NEXT line's copies are issued at once, so that its memory latency hides
+        // behind this line's recurrences (a warp has one line in flight, 16 warps share an SM) ----
         double2 qn[H], rn[H];
         double dv[M], e[M], yd[M];
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll
         for (int h = 0; h < H; h++) {
             const int v = lane + 32 * h;
             qn[h] = rn[h] = make_double2(0.0, 0.0);
-            if (v < nv) {
-                qn[h] = ld2(qvec, base + 2 * v);
-                rn[h] = ld2(INIT ? bvec : rvec, base + 2 * v);
-            }
+            if (v < nv) { qn[h] = stq[h * 32 + lane]; rn[h] = str[h * 32 + lane]; }
         }
+        prefetch(ln + lstep);
         const double2 *dT = reinterpret_cast<const double2 *>(pc.dinvT + (size_t)(op.i_lo * op.nt + row) * 32 * M);
 #pragma unroll
         for (int h = 0; h < H; h++) {
