@@ -132,7 +132,7 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
  * On the GPU the boxes are the phi lines: bi = bj = 1 and bk = 0 (or >= np) = the whole periodic line, wrap coupling
  * included; any other box shape returns MAS_EINVAL (the oracle covers general boxes and shows the line boxes within
  * 2 iterations of the undivided factorisation on the synthetic meshes).  4 <= np <= 1024.  The factors follow dt:
- * mas_pcg_set_dt refactors.  Not available for slab groups; mas_pcg_solve_multi works.  Synchronous. */
+ * mas_pcg_set_dt refactors.  mas_pcg_solve_multi and slab groups (mas_pcg_slabs_set_preconditioner) work.  Synchronous. */
 enum { MAS_PC1 = 1, MAS_PC2 = 2 };
 int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj, int bk);
 
@@ -191,6 +191,9 @@ typedef struct mas_pcg_slabs mas_pcg_slabs_t;
 int mas_pcg_slabs_create(const mas_grid_t *grid, const mas_metric_t *metric, double dt, const mas_nu_t *nu,
                          const mas_bc_t *bc, int nslab, const int *i_split, mas_pcg_slabs_t **out);
 int mas_pcg_slabs_set_dt(mas_pcg_slabs_t *g, double dt, void *stream);
+/* as mas_pcg_set_preconditioner: with PC2 every slab preconditions its own phi lines (they have no radial coupling) and
+ * K1 reads the neighbours' adjacent planes of z = M^-1 r through pointers, as it reads their planes of r with PC1 */
+int mas_pcg_slabs_set_preconditioner(mas_pcg_slabs_t *g, int kind, int bi, int bj, int bk);
 /* same names as mas_pcg_set_option (except "persistent") */
 int mas_pcg_slabs_set_option(mas_pcg_slabs_t *g, const char *name, int value);
 /* b_dev, x_dev: HOST arrays of nslab DEVICE pointers; slab s's vectors hold its own planes only,

@@ -64,6 +64,7 @@ def _prototypes(L):
         "mas_pcg_slabs_create": (ci, create_args + [ci, _ip, _vpp]),
         "mas_pcg_slabs_set_dt": (ci, [vp, cd, vp]),
         "mas_pcg_slabs_set_option": (ci, [vp, ctypes.c_char_p, ci]),
+        "mas_pcg_slabs_set_preconditioner": (ci, [vp, ci, ci, ci, ci]),
         "mas_pcg_slabs_solve": (ci, [vp, _vpp, _vpp, cd, ci, vp, _ip, _dp]),
         "mas_pcg_slabs_stats": (ci, [vp, ctypes.POINTER(ctypes.c_longlong)]),
         "mas_pcg_slabs_destroy": (None, [vp]),
@@ -271,6 +272,12 @@ def mas_pcg_slabs_set_dt(handle, dt, stream=0):
     st = lib().mas_pcg_slabs_set_dt(handle, float(dt), stream)
     if st != MAS_OK:
         raise MasError(st, "mas_pcg_slabs_set_dt")
+
+
+def mas_pcg_slabs_set_preconditioner(handle, kind: int, boxes=(1, 1, 0)):
+    st = lib().mas_pcg_slabs_set_preconditioner(handle, int(kind), int(boxes[0]), int(boxes[1]), int(boxes[2]))
+    if st != MAS_OK:
+        raise MasError(st, f"mas_pcg_slabs_set_preconditioner({kind}, {tuple(boxes)})")
 
 
 def mas_pcg_slabs_set_option(handle, name: str, value: int):

@@ -76,6 +76,7 @@ struct Work {                    // handle-owned vectors; right-hand side j at +
     // slab mode (null / 0 otherwise): the adjacent planes of the neighbour slabs, and where a slab's kernel
     // leaves its partial sums for the combine step instead of finishing the scalar step itself
     const double *lo_r, *lo_p0, *lo_p1, *hi_r, *hi_p0, *hi_p1;
+    const double *lo_z, *hi_z;   // PC2: the neighbours' adjacent planes of z
     double *slab_sums;           // [3][MAX_SLABS]
     int slab;
 };

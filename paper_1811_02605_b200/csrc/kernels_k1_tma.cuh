@@ -88,7 +88,7 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     const long long voff = rhs * w.vstride;
     const VecHalo pV = {(par ? w.p1 : w.p0) + voff, par ? w.lo_p1 : w.lo_p0, par ? w.hi_p1 : w.hi_p0};
     const bool zin = mp.zin != 0;               // PC2: "r" below is z = M^-1 r, already preconditioned
-    const VecHalo rV = zin ? VecHalo{w.z + voff, nullptr, nullptr} : VecHalo{w.r + voff, w.lo_r, w.hi_r};
+    const VecHalo rV = zin ? VecHalo{w.z + voff, w.lo_z, w.hi_z} : VecHalo{w.r + voff, w.lo_r, w.hi_r};
     double *__restrict__ pout = (par ? w.p0 : w.p1) + voff;
     double *__restrict__ qout = w.q + voff;
     const double alpha_prev = st->alpha;        // x += alpha_{k-1} p_{k-1}: the deferred x-update (xfuse)

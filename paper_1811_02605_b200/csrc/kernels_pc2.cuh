@@ -95,7 +95,7 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
     double alpha = 0.0;
     if (!INIT) {
         if (!st->active) {                              // this right-hand side is done: report, nothing else
-            if (blockIdx.x == 0 && threadIdx.x == 0) loop_vote(w, 0, gridDim.y, cond, use_cond);
+            if (blockIdx.x == 0 && threadIdx.x == 0 && !w.slab_sums) loop_vote(w, 0, gridDim.y, cond, use_cond);
             return;
         }
         alpha = st->alpha;
@@ -137,7 +137,8 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
     for (int ln = ln0; ln < op.nrows; ln += lstep) {
         const int row = reverse ? op.nrows - 1 - ln : ln;
         const size_t base = (size_t)row * np;
-        const double F = __ldg(op.F + row);
+        const int crow = op.i_lo * op.nt + row;             // the coefficient planes are the global ones (slabs)
+        const double F = __ldg(op.F + crow);
         // ---- the line's q and r (or b) were copied into the stage while the previous line was being solved; they
         // are read into registers and the NEXT line's copies are issued at once, so that its memory latency hides
         // behind this line's recurrences (a warp has one line in flight, 16 warps share an SM) ----
@@ -151,7 +152,7 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
             if (v < nv) { qn[h] = stq[h * 32 + lane]; rn[h] = str[h * 32 + lane]; }
         }
         prefetch(ln + lstep);
-        const double2 *dT = reinterpret_cast<const double2 *>(pc.dinvT + (size_t)(op.i_lo * op.nt + row) * 32 * M);
+        const double2 *dT = reinterpret_cast<const double2 *>(pc.dinvT + (size_t)crow * 32 * M);
 #pragma unroll
         for (int h = 0; h < H; h++) {
             const double2 t = __ldg(dT + h * 32 + lane);
@@ -159,7 +160,7 @@ k_pc2_line(OpDev op, Work w, Pc2Dev pc, cudaGraphConditionalHandle cond, int use
         }
         // ---- natural order: r' = r - alpha q (init: V.b - A x0), stored; staged for the chunk order ----
         double V2 = 0.0;
-        if (INIT) V2 = __ldg(op.V2 + row);
+        if (INIT) V2 = __ldg(op.V2 + crow);
 #pragma unroll
         for (int h = 0; h < H; h++) {
             const int v = lane + 32 * h;

@@ -784,11 +784,12 @@ extern "C" int mas_pcg_apply(mas_pcg_t *h, const double *x_dev, double *y_dev, v
     return MAS_OK;
 }
 
-extern "C" int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj, int bk)
+namespace {
+
+// Switch the operator's preconditioner.  own_z: allocate the handle's own z vectors (a slab group keeps one per slab).
+int set_precond(mas_pcg *h, int kind, int bi, int bj, int bk, bool own_z)
 {
-    if (!h || (kind != MAS_PC1 && kind != MAS_PC2)) return MAS_EINVAL;
-    DeviceGuard dg(h->device);
-    if (!dg.ok) return MAS_ECUDA;
+    if (kind != MAS_PC1 && kind != MAS_PC2) return MAS_EINVAL;
     if (kind == MAS_PC1) {
         if (h->precond != MAS_PC1) drop_graphs(h);
         h->precond = MAS_PC1;
@@ -808,7 +809,7 @@ extern "C" int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj
         const int rc = upload(h->ipT, ipT);
         if (rc != MAS_OK) return rc;
     }
-    if (!h->z.p || h->z.n < h->n * (size_t)h->nrhs_cap) {
+    if (own_z && (!h->z.p || h->z.n < h->n * (size_t)h->nrhs_cap)) {
         if (h->z.alloc(h->n * (size_t)(h->nrhs_cap > 0 ? h->nrhs_cap : 1)) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
     }
     h->pc2_M = M;
@@ -819,6 +820,16 @@ extern "C" int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj
     CK(cudaGetLastError());
     CK(cudaDeviceSynchronize());
     return MAS_OK;
+}
+
+}  // namespace
+
+extern "C" int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj, int bk)
+{
+    if (!h) return MAS_EINVAL;
+    DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
+    return set_precond(h, kind, bi, bj, bk, true);
 }
 
 extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)

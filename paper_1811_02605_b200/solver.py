@@ -118,6 +118,9 @@ class MasPcgSlabs:
     def set_option(self, name, value):
         B.mas_pcg_slabs_set_option(self._h, name, value)
 
+    def set_preconditioner(self, kind: int, boxes=(1, 1, 0)):
+        B.mas_pcg_slabs_set_preconditioner(self._h, kind, boxes)
+
     def _slab_ptrs(self, t: torch.Tensor):
         plane = self.shape[1] * self.shape[2]
         _dev_ptr(t, self.shape[0] * plane)

@@ -193,3 +193,38 @@ def test_pc2_breakdown_zero_rhs_and_argument_errors():
     _, gpu2 = H.both_ops(mesh2, 1e-3, 0, np.array([1.0]))
     with pytest.raises(MasError):
         gpu2.set_preconditioner(2)                               # np < 4
+
+
+@pytest.mark.parametrize("loop_mode", [1, 0])
+@pytest.mark.parametrize("split", [[0, 10, 21], [0, 1, 2, 20, 21], [0, 5, 11, 16, 21]])
+def test_pc2_slab_groups_parity_and_bits(split, loop_mode):
+    """PC2 on an r-slab group (NEXT-3 x NEXT-4): every slab preconditions its own phi lines, K1 reads the neighbours'
+    adjacent planes of z through pointers; the oracle is the undivided PC2 solve."""
+    from paper_1811_02605_b200 import MasPcgSlabs
+    bc = (0, 1)
+    mesh, dt, nu_kind, nu = H.general_case(21, 19, 134, s=500.0, bc=bc)
+    oref = ref.RefOperator(mesh, dt, nu_kind, nu, bc)
+    g = MasPcgSlabs(mesh, dt, nu_kind, nu, bc, split)
+    g.set_option("loop_mode", loop_mode)
+    g.set_preconditioner(2)
+    rng = np.random.default_rng(3)
+    b, x0 = rng.uniform(-1, 1, mesh.shape), rng.standard_normal(mesh.shape)
+    pc = oref.pc2(LINES)
+    st_r, k_r, x_r, h_r = oref.pcg_pc2(pc, b, x0, 1e-10, 2000)
+    runs = []
+    for _ in range(2):
+        xd = _t(x0)
+        st_g, k_g, h_g = g.solve(_t(b), xd, 1e-10, 2000)
+        runs.append((k_g, h_g.tobytes(), xd.cpu().numpy().tobytes()))
+    assert runs[0] == runs[1]
+    assert st_g == st_r and abs(k_g - k_r) <= 1
+    m = min(H.HIST_ITERS, k_r, k_g) + 1
+    rel = np.maximum(np.abs(h_g[:m] - h_r[:m]) - H.HIST_FLOOR, 0.0) / h_r[:m]
+    assert rel.max() <= H.HIST_RTOL
+    if k_g == k_r:
+        assert np.linalg.norm(xd.cpu().numpy() - x_r) / np.linalg.norm(x_r) <= H.X_RTOL
+    s = g.stats()
+    assert s["bytes_per_cell_iter"] == 88 and s["persistent_grid_or_slabs"] == len(split) - 1
+    g.set_preconditioner(1)                                      # back to PC1 on the same group
+    st1, k1, _ = g.solve(_t(b), _t(x0), 1e-10, 2000)
+    assert st1 == 0 and k1 > k_g
