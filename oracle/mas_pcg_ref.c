@@ -33,10 +33,14 @@
  *
  * The system solved (R2): the caller's A_phys x = b with A_phys = diag(V)^-1 A_sym;
  * internally A_sym x = b_s, b_s = V.b; residuals, norms and the stopping test live in the
- * symmetric system.  Parity status: pinned by tests/test_oracle_*.py (dense LU, manufactured
- * solution, symmetry/SPD, Krylov optimality, closed forms, continuum consistency).  What is
- * tied to the paper's own run (its mesh, nu, RHS, its 70/550 iteration counts) is
- * "parity unpinned": the data are not available.
+ * symmetric system.  Further down: the RKL2 super time stepping of the viscosity term (NEXT-1) and
+ * the paper's second preconditioner PC2, block-Jacobi ILU(0) (NEXT-4), each with its own header.
+ * Parity status: pinned by tests/test_oracle_*.py (dense LU, manufactured
+ * solution, symmetry/SPD, Krylov optimality, closed forms, continuum consistency, Legendre stability
+ * polynomial, the ILU(0) defining property, exactness on tridiagonal operators, randomised meshes;
+ * 22 committed source mutations).  "Parity unpinned": the face-nu mean (Q3: a declared reading; the
+ * harmonic mean survives every mathematical pin) and what is tied to the paper's own run (its mesh,
+ * nu, RHS, its 70/550 and 100-200 iteration counts, its PC2 domains): the data are not available.
  *
  * Sums are plain index-order loops with a long double accumulator (Q22).  No blocking, no
  * fusion, no reordering.  Layout: [nr][nt][np], phi fastest.
