@@ -142,7 +142,7 @@ int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj, int bk);
  *                 cooperative kernel, whatever loop_mode says; 0: always the streaming loop;
  *   "qrecompute"  0 (default): 72 B/cell/iteration, q stored by K1 and streamed by K2; 1: 64 B -- K1 does not store q,
  *                 K2 recomputes it with the stencil kernel (fewer bytes, more instructions: measured slower);
- *   "tile"        K1 tile configuration (0..6), "k2r_tile" / "stencil_tile" (0..5) the stencil kernel's tile for
+ *   "tile"        K1 tile configuration (0..6; -1 = automatic, the default), "k2r_tile" / "stencil_tile" (0..5) the stencil kernel's tile for
  *                 K2R / for apply and RKL2 stages, "ci" r-chunk length of the marching kernels (0 = automatic, else 2..32);
  *   "serpentine"  1 (default): K2 sweeps the mesh backward (L2 reuse across K1 -> K2 -> K1);
  *   "unroll"      PCG iterations per WHILE trip of the graph loop (1..16, default 4);

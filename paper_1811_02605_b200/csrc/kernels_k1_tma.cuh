@@ -238,6 +238,17 @@ struct K1TmaTile {
 static const K1TmaTile kK1TmaTiles[] = {{14, 2, 1}, {8, 2, 2}, {6, 2, 2}, {8, 3, 1}, {10, 2, 1}, {16, 2, 1}, {12, 2, 1}};
 inline int k1_tma_num_tiles() { return (int)(sizeof(kK1TmaTiles) / sizeof(kK1TmaTiles[0])); }
 
+// Automatic tile: the 14-row tile with one 512-thread block per SM is the fastest when the mesh gives every SM several
+// blocks in turn (configs 4, 5); when all of its tiles fit in ONE round (mid-size meshes such as config 3: 140 blocks on
+// 148 SMs) nothing overlaps a block's start-up and reduction tail, and the 6-row tile with two blocks per SM is faster
+// (measured on config 3: 0.0591 vs 0.0619 ms).
+inline int k1_auto_tile(int nr, int nt, int np, int num_sms)
+{
+    const long long cols = (long long)((np + TILE_TK - 1) / TILE_TK) * ((nt + 13) / 14);
+    const int ci = tile_pick_ci(nr, cols, num_sms, 0);
+    return cols * ((nr + ci - 1) / ci) <= num_sms ? 2 : 0;
+}
+
 template <int TJ, int DEPTH, int MINB>
 inline void k1_tma_pick(bool uniform, bool noq, const void **func, dim3 *block, size_t *smem)
 {

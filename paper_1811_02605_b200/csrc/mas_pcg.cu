@@ -101,7 +101,7 @@ struct mas_pcg {
     size_t hist_cap = 0;
     // options
     int loop_mode = 1;               // requested: 1 graph-while, 0 host chunks
-    int tile = 0;                    // K1 tile configuration id
+    int tile = -1;                   // K1 tile configuration id; -1 = automatic (k1_auto_tile)
     int ci_force = 0;                // >0: override the r-chunk length (tuning)
     int stencil_tile = 1;            // k_stencil_tma tile for apply / STS
     int k2r_tile = 1;                // k_stencil_tma tile for K2R
@@ -476,7 +476,8 @@ int make_plan(const mas_pcg *h, const OpDev &op, const Work &work, int nrhs, int
     }
     // K1
     memset(&c.k1p, 0, sizeof(c.k1p));
-    k1_tma_configure(op.nr, op.nt, op.np, uni, h->qrecompute != 0 && !pc2, h->tile, h->num_sms, h->ci_force, nrhs, &c.k1p,
+    const int k1_tile = h->tile >= 0 ? h->tile : k1_auto_tile(op.nr, op.nt, op.np, h->num_sms);
+    k1_tma_configure(op.nr, op.nt, op.np, uni, h->qrecompute != 0 && !pc2, k1_tile, h->num_sms, h->ci_force, nrhs, &c.k1p,
                      &c.k1.func, &c.k1.grid, &c.k1.block, &c.k1.smem);
     c.k1p.vp = h->vp0; c.k1p.wp = h->wp0; c.k1p.ip = h->ip0;
     c.k1p.l2 = h->l2;
@@ -840,7 +841,7 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->loop_mode = value;
     } else if (!strcmp(name, "tile")) {
-        if (value < 0 || value >= k1_tma_num_tiles()) return MAS_EINVAL;
+        if (value < -1 || value >= k1_tma_num_tiles()) return MAS_EINVAL;
         h->tile = value;
     } else if (!strcmp(name, "stencil_tile")) {
         if (value < 0 || value >= stencil_num_tiles()) return MAS_EINVAL;
