@@ -63,10 +63,11 @@ enum {
     MAS_ENOMEM = -2,     /* host or device allocation failed                                            */
     MAS_ECUDA = -3,      /* a CUDA runtime call failed (no device, launch error, ...), or a kernel
                             reported a protocol fault (an mbarrier wait that timed out)                 */
-    MAS_EBREAKDOWN = -4  /* p.Ap <= 0, or a non-finite scalar (||V.b||^2, ||r||^2, r.z, p.Ap): the
+    MAS_EBREAKDOWN = -4, /* p.Ap <= 0, or a non-finite scalar (||V.b||^2, ||r||^2, r.z, p.Ap): the
                             operator is not SPD for these inputs, or b / x0 hold NaN / Inf.  x is the
                             last iterate (x0 if no iteration completed); iters_out and the history
                             are valid                                                                   */
+    MAS_ETOOBIG = -5     /* mas_pcg_residual_static only: the mesh has more than MAS_PCG_STATIC_MAX_CELLS cells  */
 };
 
 /* Build the operator for (grid, metric, dt, nu, boundary kinds) and allocate all workspaces
@@ -170,6 +171,44 @@ int mas_sts_stages(const mas_pcg_t *h, double tau, int *s_out);
  * s kernel launches on `stream`, asynchronous.  Uses the handle's PCG workspaces as stage buffers, so it
  * must not overlap a solve on the same handle. */
 int mas_sts_advance(mas_pcg_t *h, double *u_dev, double tau, int s, void *stream);
+
+/* ---- Residual check for callers that must not allocate device memory. ----
+ *
+ * Some users of this library cannot call cudaMalloc once their set-up is over: a time-stepping code that keeps every
+ * field resident on the GPU (as the paper's does) and has sized its arrays or its own pool to fill
+ * the card, so a later request simply fails; a process held to a fixed device-memory limit; or the inside of a step
+ * loop where cudaMalloc / cudaFree are unaffordable because they stall the whole device and with it every other
+ * stream.  mas_pcg_solve does not suit them: it may allocate on the way (a longer history, more right-hand sides, a
+ * graph for a shape it has not seen).  This call never allocates -- no cudaMalloc, no cudaFree, no library routine
+ * that allocates -- and it needs no workspace from the handle.  The handle itself must of course have been created
+ * earlier, while allocating was still possible.
+ *
+ * What it computes (one kernel, the init step S1 of the solve applied to the caller's vectors):
+ *     r = V.b - ax                 with ax = A_sym x from mas_pcg_apply (which needs no scratch memory either),
+ *     sums[0] = ||V.b||^2,  sums[1] = ||r||^2,  sums[2] = r.D^-1 r     (D = diag(A_sym), whatever preconditioner is set),
+ * so sqrt(sums[1] / sums[0]) is the TRUE relative residual of x, the quantity hist[] of mas_pcg_solve tracks through
+ * the recurrence.  The sums are the deterministic two-stage reduction of the solve: the same
+ * inputs give the same bits on every run.
+ *   b_dev, ax_dev : DEVICE, N doubles each, 16-byte aligned, not written.
+ *   r_dev         : DEVICE, N doubles, 16-byte aligned; may be the same buffer as ax_dev (in place), not b_dev.
+ *   sums_dev      : DEVICE, 3 doubles, written by the kernel; read them after synchronising `stream`.
+ *   stream        : everything is enqueued on it (one 256-byte memset node and one kernel); nothing synchronises.
+ *
+ * The scratch the reduction needs (per-block partial sums, an arrival counter) lives in a fixed 98 560-byte array
+ * inside the library image.  Consequences:
+ *   - Limit: N <= MAS_PCG_STATIC_MAX_CELLS (2^25 = 256 x 256 x 512, BASELINE.json config 4).  A larger mesh returns
+ *     MAS_ETOOBIG and nothing is launched.
+ *   - Every GPU that loads this library holds those 98 560 bytes until the process exits.
+ *   - All calls on one device -- from any handle, any thread, any stream -- share the one array.  Two calls whose
+ *     kernels may overlap on the GPU race on it and return garbage: keep calls on one stream, or order them with
+ *     events.  The array keeps the previous call's contents; the call clears the part that has to start at zero.
+ *   - The first call on each device looks up the array's device address (and may make the driver load the module
+ *     there).  Make that first call during set-up, before any stream capture is begun; later calls on that device
+ *     only enqueue the memset and the kernel.
+ * Returns MAS_OK once enqueued; MAS_EINVAL (null / misaligned / overlapping pointers), MAS_ETOOBIG, MAS_ECUDA. */
+#define MAS_PCG_STATIC_MAX_CELLS 33554432LL
+int mas_pcg_residual_static(mas_pcg_t *h, const double *b_dev, const double *ax_dev, double *r_dev,
+                            double *sums_dev, void *stream);
 
 void mas_pcg_destroy(mas_pcg_t *h);            /* NULL is allowed                                 */
 

@@ -15,6 +15,8 @@ import numpy as np
 from . import build as _build
 
 MAS_OK, MAS_MAXIT, MAS_EINVAL, MAS_ENOMEM, MAS_ECUDA, MAS_EBREAKDOWN = 0, 1, -1, -2, -3, -4
+MAS_ETOOBIG = -5
+MAS_PCG_STATIC_MAX_CELLS = 1 << 25   # include/mas_pcg.h: the largest mesh mas_pcg_residual_static serves
 MAS_BC_DIRICHLET, MAS_BC_NEUMANN = 0, 1
 MAX_RHS = 3
 
@@ -52,6 +54,7 @@ def _prototypes(L):
         "mas_pcg_solve_host": (ci, [vp, vp, vp, cd, ci, vp, _ip, _dp]),
         "mas_pcg_solve_multi": (ci, [vp, ci, _vpp, _vpp, cd, ci, vp, _ip, _ip, _dp]),
         "mas_pcg_apply": (ci, [vp, vp, vp, vp]),
+        "mas_pcg_residual_static": (ci, [vp, vp, vp, vp, vp, vp]),
         "mas_pcg_lop": (ci, [vp, vp, vp, vp]),
         "mas_pcg_lambda_max": (ci, [vp, _dp]),
         "mas_sts_stages": (ci, [vp, cd, _ip]),
@@ -162,6 +165,16 @@ def mas_pcg_apply(handle, x_ptr, y_ptr, stream=0):
     st = lib().mas_pcg_apply(handle, x_ptr, y_ptr, stream)
     if st != MAS_OK:
         raise MasError(st, "mas_pcg_apply")
+
+
+def mas_pcg_residual_static(handle, b_ptr, ax_ptr, r_ptr, sums_ptr, stream=0):
+    """r = V.b - ax and the three sums (||V.b||^2, ||r||^2, r.D^-1 r) into the DEVICE array at sums_ptr, for callers
+    that must not allocate device memory (include/mas_pcg.h has the full contract: the scratch is a fixed array in
+    the library, N <= MAS_PCG_STATIC_MAX_CELLS, calls that overlap on the GPU race, make the first call on a device
+    before any stream capture).  Enqueues only; raises MasError on a non-zero status (MAS_ETOOBIG past the limit)."""
+    st = lib().mas_pcg_residual_static(handle, b_ptr, ax_ptr, r_ptr, sums_ptr, stream)
+    if st != MAS_OK:
+        raise MasError(st, "mas_pcg_residual_static")
 
 
 def _raise(st, where, iters=None, hist=None):

@@ -238,6 +238,7 @@ extern "C" const char *mas_pcg_strerror(int status)
         case MAS_ENOMEM: return "out of memory";
         case MAS_ECUDA: return "CUDA runtime error (no device, a launch failed, or a kernel reported a protocol fault)";
         case MAS_EBREAKDOWN: return "PCG breakdown: p.Ap <= 0 or a non-finite scalar";
+        case MAS_ETOOBIG: return "mesh has more cells than the fixed scratch array of the allocation-free entry point can serve (MAS_PCG_STATIC_MAX_CELLS)";
         default: return "unknown status";
     }
 }
@@ -929,6 +930,7 @@ extern "C" int mas_pcg_solve_host(mas_pcg_t *h, const double *b_host, double *x_
 
 #include "host_sts.inc"
 #include "host_slabs.inc"
+#include "noalloc_residual.inc"
 #ifdef MAS_PCG_DEBUG_PROBES
 #include "host_debug.inc"
 #endif

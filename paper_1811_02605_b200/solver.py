@@ -51,6 +51,12 @@ class MasPcg:
         B.mas_pcg_apply(self._h, _dev_ptr(x, self.n), _dev_ptr(y, self.n), _stream_ptr(stream))
         return y
 
+    def residual_static(self, b: torch.Tensor, ax: torch.Tensor, r: torch.Tensor, sums: torch.Tensor, stream=None):
+        """r = V.b - ax; sums (a CUDA float64 tensor of 3) = ||V.b||^2, ||r||^2, r.D^-1 r.  The allocation-free
+        entry point (mas_pcg_residual_static): every tensor is the caller's, nothing is allocated here or below."""
+        B.mas_pcg_residual_static(self._h, _dev_ptr(b, self.n), _dev_ptr(ax, self.n), _dev_ptr(r, self.n),
+                                  _dev_ptr(sums, 3), _stream_ptr(stream))
+
     def solve(self, b: torch.Tensor, x: torch.Tensor, rtol: float, maxit: int, stream=None, want_hist=True):
         """Solves A_phys x = b in place in x (x holds x0 on entry).  Returns (status, iters, hist)."""
         return B.mas_pcg_solve(self._h, _dev_ptr(b, self.n), _dev_ptr(x, self.n), rtol, maxit,

@@ -51,7 +51,7 @@ def test_python_binding_has_the_same_names():
 
 
 def test_strerror_covers_every_status():
-    for st in (0, 1, -1, -2, -3, -4):
+    for st in (0, 1, -1, -2, -3, -4, -5):
         s = B.mas_pcg_strerror(st)
         assert s and s != "unknown status"
     assert B.mas_pcg_strerror(77) == "unknown status"
