@@ -302,7 +302,7 @@ int mas_ref_pcg(const ref_op *op, const double *b_phys, double *x, double rtol, 
 
 /*
  * NEXT-2: several right-hand sides that share one operator -- the three components of v in
- * PAPER.md:50 eq. (1) "share one coefficient set".  By definition this is nrhs INDEPENDENT textbook solves,
+ * PAPER.md:50 eq. (1), which share one coefficient set (SURVEY 8(f)'s observation, not a quotation).  By definition this is nrhs INDEPENDENT textbook solves,
  * each with its own alpha, beta, iteration count, status and history: nothing is coupled across right-hand
  * sides.  b, x: nrhs vectors stored back to back (nrhs * N doubles); hist: NULL or nrhs * (maxit + 1) doubles,
  * right-hand side j's history starting at hist + j * (maxit + 1); iters, status: nrhs ints.
@@ -412,8 +412,9 @@ done:
 }
 
 /* ==============================================================================================
- * NEXT-4: the paper's second preconditioner -- "The second (PC2) uses a
- * non-overlapping domain decomposition with zero-fill incomplete LU factorization" (Sec. 2.2;
+ * NEXT-4: the paper's second preconditioner -- "the second (PC2) is a block-Jacobi
+ * using a zero-fill incomplete LU factorization [22]" (Sec. 2.2; that the blocks are
+ * non-overlapping boxes of cells is this oracle's reading, R8, not the paper's words;
  * 100-200 iterations against ~550 with PC1; its triangular solves are what the authors call
  * "not vectorizable" and leave on the CPU).
  *

@@ -1,5 +1,5 @@
-// kernels_pc2.cuh -- PC2 on the GPU (Sec. 2.2: "The second (PC2) uses a
-// non-overlapping domain decomposition with zero-fill incomplete LU factorization"; its triangular
+// kernels_pc2.cuh -- PC2 on the GPU (Sec. 2.2: "the second (PC2) is a
+// block-Jacobi using a zero-fill incomplete LU factorization [22]"; blocks = non-overlapping boxes: DESIGN.md R8; its triangular
 // solves are what the authors call not vectorizable and leave on the CPU).
 //
 // B200 design (R8, section 5 "PC2"): the domains of the block-Jacobi decomposition are free to choose, so

@@ -1,5 +1,5 @@
-"""GPU parity for PC2 ("non-overlapping domain decomposition with zero-fill incomplete
-LU factorization"): mas_pcg_set_preconditioner(MAS_PC2) + mas_pcg_solve against the oracle's mas_ref_pcg_pc2 with the
+"""GPU parity for PC2 ("the second (PC2) is a block-Jacobi using a zero-fill incomplete LU
+factorization [22]"; blocks = non-overlapping boxes is the reading DESIGN.md R8): mas_pcg_set_preconditioner(MAS_PC2) + mas_pcg_solve against the oracle's mas_ref_pcg_pc2 with the
 same boxes (the phi lines: 1 x 1 x np), under the north_star gates.  Run on the B200 box:  pytest tests -m gpu"""
 import numpy as np
 import pytest

@@ -1,5 +1,5 @@
-"""Pins for the ORACLE's PC2 (oracle/mas_pcg_ref.c, NEXT-4: "non-overlapping domain decomposition with zero-fill
-incomplete LU factorization"): checked against what the mathematics fixes, never against itself and
+"""Pins for the ORACLE's PC2 (oracle/mas_pcg_ref.c, NEXT-4: "the second (PC2) is a block-Jacobi using a zero-fill
+incomplete LU factorization [22]"; blocks = non-overlapping boxes is the reading DESIGN.md R8): checked against what the mathematics fixes, never against itself and
 never against the CUDA path.  CPU only.
 
   * the defining property of ILU(0) (Saad [22]): L unit lower, U upper, both confined to the pattern of A_blk, and
