@@ -100,9 +100,13 @@ int mas_pcg_solve_host(mas_pcg_t *h, const double *b_host, double *x_host, doubl
 
 /* Batched solve: nrhs <= 3 right-hand sides that share the operator -- PAPER.md:50 eq. (1):
  * the implicit terms act on the vector v, whose three components share one coefficient set.  By definition these
- * are nrhs INDEPENDENT textbook solves (own alpha, beta, iteration count, status and history each; bit-identical to
- * nrhs calls of mas_pcg_solve), run by ONE set of kernel launches per iteration: the right-hand side is the second
- * grid dimension, a right-hand side that has converged drops out, the loop ends when all have.
+ * are nrhs INDEPENDENT textbook solves (own alpha, beta, iteration count, status and history each), run by ONE set
+ * of kernel launches per iteration: the right-hand side is the second grid dimension, a right-hand side that has
+ * converged drops out, the loop ends when all have.  A batched solve always runs the streaming K1 / K2 kernels, and
+ * its results are bit-identical to nrhs calls of mas_pcg_solve THAT RUN THE SAME KERNELS: option "persistent" = 0, or
+ * a mesh too large for the one-kernel solve, or PC2.  With the default "persistent" = 1 a single solve of a small
+ * mesh runs in the cooperative kernel, whose reductions add in another order: the two then agree to rounding (the
+ * history within 1e-10 relative, x within 1e-9, as against the oracle), not bit for bit.
  *   b_dev, x_dev  : HOST arrays of nrhs DEVICE pointers (N doubles each; all distinct).
  *   iters_out     : HOST, nrhs ints (may be NULL);  status_out: HOST, nrhs ints (MAS_OK / MAS_MAXIT /
  *                   MAS_EBREAKDOWN per right-hand side; may be NULL).
@@ -126,9 +130,9 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
 
 /* The paper's two "communication-free preconditioning options" (Sec. 2.2):
  *   MAS_PC1  point-Jacobi, "the inverse diagonal of the matrix" (the default);
- *   MAS_PC2  "a non-overlapping domain decomposition with zero-fill incomplete LU factorization" (SURVEY 8(f)
- *            NEXT-4): block Jacobi over boxes of bi x bj x bk cells, ILU(0) of A_sym restricted to each box, natural
- *            ordering (R8).  PAPER.md:80: 100-200 iterations against ~550 with PC1; the
+ *   MAS_PC2  "a block-Jacobi using a zero-fill incomplete LU factorization [22]".  Reading
+ *            (R8, not the paper's words): block Jacobi over non-overlapping boxes of bi x bj x bk cells,
+ *            ILU(0) of A_sym restricted to each box, natural ordering.  PAPER.md:80: 100-200 iterations against ~550 with PC1; the
  *            authors kept it on the CPU because its triangular solves do not vectorise.
  * On the GPU the boxes are the phi lines: bi = bj = 1 and bk = 0 (or >= np) = the whole periodic line, wrap coupling
  * included; any other box shape returns MAS_EINVAL (the oracle covers general boxes and shows the line boxes within
