@@ -32,7 +32,7 @@ METRIC = "fp64_pcg_iterations_per_s_256x256x512"
 UNIT = "iterations/s"
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
 REF_ITERS_PER_STEP = 4             # oracle iterations per step of --impl reference (bounded sample)
-CPU_BASELINE_ITERS = 12            # oracle iterations timed for cpu_baseline (about 10-30 s)
+CPU_BASELINE_ITERS = 20            # oracle iterations timed for cpu_baseline (BASELINE.md sec. 5 / SURVEY 8(d): 20; about 20-30 s)
 
 
 def parse():
@@ -44,6 +44,10 @@ def parse():
     ap.add_argument("--workload", default="c4", choices=["c1", "c2", "c3", "c4", "c5", "sts", "visc", "precond"])
     ap.add_argument("--precond", type=int, default=1, choices=[1, 2],
                     help="1 = PC1 point Jacobi (default), 2 = PC2 block-Jacobi ILU(0) over phi lines (NEXT-4)")
+    ap.add_argument("--mesh", default="config", choices=["config", "nonuniform", "clustered"],
+                    help="configs 3-5, sts, precond: BASELINE.json's mesh (uniform theta / phi), the same shape with r, theta and "
+                         "phi widths varying by +-30 %% (the kernels' general instantiations), or a paper-like mesh packed in "
+                         "r and theta with a uniform nu (mas_inputs.configs.make)")
     ap.add_argument("--opt", action="append", default=[], help="name=value passed to mas_pcg_set_option (tuning)")
     ap.add_argument("--nrhs", type=int, default=1, help="right-hand sides per batched solve (1..3; NEXT-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -62,11 +66,11 @@ def workload_rhs(name, prob):
     return configs.rhs_blob(prob)
 
 
-def workload(name, rank=0):
+def workload(name, rank=0, mesh_kind="config"):
     """(problem, dt, b, rtol, maxit, description).  Seeds are offset by the rank for replicas."""
     from mas_inputs import configs
     import numpy as np
-    prob = configs.make(name)
+    prob = configs.make(name, mesh_kind=mesh_kind)
     prob.seed += 1000 * rank
     s = prob.stiffness[-1]
     dt = prob.dt_for(s)
@@ -75,6 +79,9 @@ def workload(name, rank=0):
     rtol, maxit = (0.0, 500) if name == "c4" else (prob.rtol, prob.maxit)
     desc = (f"{name}: {nr}x{nt}x{np_} fp64, stiffness s={s:g}, rtol={rtol:g}, maxit={maxit}, "
             f"{'500 fixed PCG iterations' if name == 'c4' else 'solve to rtol'}")
+    if mesh_kind != "config":
+        desc += {"nonuniform": "; mesh: r, theta and phi widths varying by +-30 % (grids.random_mesh), dt from the oracle-written S1",
+                 "clustered": "; mesh: packed in r and theta (grids.clustered_mesh), uniform nu, phi uniform"}[mesh_kind]
     return prob, dt, np.ascontiguousarray(b), rtol, maxit, desc
 
 
@@ -328,7 +335,7 @@ def run_sts(args):
     from mas_inputs import configs
     from paper_1811_02605_b200 import MasPcg
     torch.cuda.set_device(0)
-    prob = configs.make("c4")
+    prob = configs.make("c4", mesh_kind=args.mesh)
     S = 200
     gpu = MasPcg(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
     for kv in args.opt:
@@ -360,7 +367,7 @@ def run_sts(args):
     alg = (5.0 * (S - 1) + 3.0) / S * 8 * n            # bytes per stage, averaged (stage 1 moves 3N)
     peak, peak_src = hbm_peak()
     gbs = alg / (stage_ms * 1e-3) / 1e9
-    line = {"metric": "rkl2_sts_stages_per_s_256x256x512", "value": 1e3 / stage_ms, "unit": "stages/s", "n_gpus": 1,
+    line = {"metric": "rkl2_sts_stages_per_s_256x256x512" + ("" if args.mesh == "config" else f"_{args.mesh}_mesh"), "value": 1e3 / stage_ms, "unit": "stages/s", "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "sts: 256x256x512 fp64, nu(r) of config 4, one RKL2 super-step of 200 stages, "
@@ -437,7 +444,7 @@ def run_precond(args):
     stream = torch.cuda.current_stream()
     out = {}
     for name in ("c3", "c4"):
-        prob = configs.make(name)
+        prob = configs.make(name, mesh_kind=args.mesh)
         dt = prob.dt_for(1e4)
         b = torch.from_numpy(workload_rhs(name, prob)).cuda()
         x = torch.zeros_like(b)
@@ -467,11 +474,14 @@ def run_precond(args):
         res["iteration_ratio"] = res["pc1"]["iterations"] / res["pc2"]["iterations"]
         out[name] = res
         gpu.close()
-    line = {"metric": "viscosity_solve_ms_pc2_256x256x512", "value": out["c4"]["pc2"]["ms"], "unit": "ms", "n_gpus": 1,
+    line = {"metric": "viscosity_solve_ms_pc2_256x256x512" + ("" if args.mesh == "config" else f"_{args.mesh}_mesh"), "value": out["c4"]["pc2"]["ms"], "unit": "ms", "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 1), "ms_per_step": out["c4"]["pc2"]["ms"],
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "precond: configs 3 (128x192x256) and 4 (256x256x512) at stiffness 1e4, solved to "
-                                   "rtol 1e-9 from x0 = 0 with PC1 (point Jacobi) and PC2 (block-Jacobi ILU(0), phi-line domains)"},
+                                   "rtol 1e-9 from x0 = 0 with PC1 (point Jacobi) and PC2 (block-Jacobi ILU(0), phi-line domains)"
+                                   + ("" if args.mesh == "config" else f"; mesh kind: {args.mesh} (mas_inputs.configs.make)"),
+                       "note": "the PC2 / PC1 ratio depends on where the mesh puts its stiffness: the phi-line domains "
+                               "contain the phi couplings only (DESIGN.md R8)"},
             "c3": out["c3"], "c4": out["c4"]}
     print(json.dumps(line), flush=True)
 
@@ -513,7 +523,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    prob, dt, b_np, rtol, maxit, desc = workload(args.workload, rank)
+    prob, dt, b_np, rtol, maxit, desc = workload(args.workload, rank, args.mesh)
     n = prob.mesh.ncells
     nrhs = max(1, min(3, args.nrhs))
     opts = [(kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt]
@@ -610,11 +620,13 @@ def main():
                    ("k_pc2_line" if args.precond == 2 else "k2_vec"))
         dom = k1_name if prof["k1_ms"] >= prof["k2_ms"] else k2_name
         dom_gbs = k1_gbs if dom == k1_name else k2_gbs
-        traffic, traffic_src = ncu_traffic(dom)
+        # the committed capture is of the uniform-phi instantiations on BASELINE.json's mesh; other meshes: not captured
+        traffic, traffic_src = ncu_traffic(dom) if args.mesh == "config" else (None, None)
         it_ms = ms / (iters_all / world) if iters_all else float("nan")
         nr_, nt_, np__ = prob.mesh.shape
         line = {
-            "metric": METRIC if args.workload == "c4" else f"fp64_pcg_iterations_per_s_{nr_}x{nt_}x{np__}",
+            "metric": (METRIC if args.workload == "c4" else f"fp64_pcg_iterations_per_s_{nr_}x{nt_}x{np__}")
+                      + ("" if args.mesh == "config" else f"_{args.mesh}_mesh"),
             "value": value, "unit": UNIT if nrhs == 1 else "rhs-iterations/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",

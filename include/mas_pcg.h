@@ -85,8 +85,10 @@ int mas_pcg_set_dt(mas_pcg_t *h, double dt, void *stream);
  *   x_dev   : DEVICE, N doubles; in = initial guess x0, out = last iterate.
  *   rtol    : stop when ||r_k||_2 / ||V.b||_2 <= rtol (recurrence residual of the symmetric system).
  *   maxit   : iteration cap; with rtol = 0 exactly maxit iterations run.
- *   stream  : all work is enqueued on it; the call synchronises it ONCE, at the end, to return
- *             the count and history.  The iteration loop itself never returns to the host.
+ *   stream  : all work is enqueued on it; the call synchronises it at the end, to return the count
+ *             and history (once; a second time only when ||V.b|| = 0 and x has to be zeroed, and
+ *             mas_pcg_solve_host once more after copying x back).  The iteration loop itself never
+ *             returns to the host.
  *   iters_out    : HOST, number of iterations k performed (may be NULL).
  *   reshist_host : HOST, NULL or >= maxit+1 doubles; receives hist[0..k], hist[j] = ||r_j||/||V.b||.
  * One solve in flight per handle. */
@@ -137,7 +139,10 @@ int mas_pcg_stats(const mas_pcg_t *h, long long *out);
  * On the GPU the boxes are the phi lines: bi = bj = 1 and bk = 0 (or >= np) = the whole periodic line, wrap coupling
  * included; any other box shape returns MAS_EINVAL (the oracle covers general boxes and shows the line boxes within
  * 2 iterations of the undivided factorisation on the synthetic meshes).  4 <= np <= 1024.  The factors follow dt:
- * mas_pcg_set_dt refactors.  mas_pcg_solve_multi and slab groups (mas_pcg_slabs_set_preconditioner) work.  Synchronous. */
+ * mas_pcg_set_dt refactors.  mas_pcg_solve_multi and slab groups (mas_pcg_slabs_set_preconditioner) work.
+ * Synchronous: the factorisation runs on the default stream and the call returns after cudaDeviceSynchronize, so it is
+ * ordered against work on every stream, blocking or not (a set-up call, not one for the step loop; mas_pcg_set_dt is
+ * the in-loop way to refactor, on the caller's stream). */
 enum { MAS_PC1 = 1, MAS_PC2 = 2 };
 int mas_pcg_set_preconditioner(mas_pcg_t *h, int kind, int bi, int bj, int bk);
 

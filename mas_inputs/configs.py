@@ -76,9 +76,31 @@ def nu_profile(mesh: grids.Mesh, nu0: float = 1.0) -> np.ndarray:
     return np.ascontiguousarray(np.broadcast_to(prof[:, None], (mesh.nr, mesh.nt)))
 
 
-def make(name: str, shape: tuple | None = None) -> Problem:
-    """Problem `name` in {"c1".."c5"}; `shape` overrides the grid size (reduced test cases)."""
+MESH_KINDS = ("config", "nonuniform", "clustered")
+
+
+def make(name: str, shape: tuple | None = None, mesh_kind: str = "config") -> Problem:
+    """Problem `name` in {"c1".."c5"}; `shape` overrides the grid size (reduced test cases).
+    mesh_kind (configs 3-5 only; the problem is then called name + "n" / name + "k"):
+      "config"      BASELINE.json's mesh: packed in r, uniform in theta and phi;
+      "nonuniform"  the same shape, nu profile, stiffness and right-hand side on grids.random_mesh: r, theta AND phi
+                    widths varying by +-30 % ("non-uniform logically-rectangular", "extremely
+                    non-uniform grid"): the kernels' general (non-uniform phi) instantiations;
+      "clustered"   grids.clustered_mesh: cells packed in r AND theta around an "erupting region" at the inner boundary
+                    near the equator, phi uniform, with a large UNIFORM nu: the stiffness then sits
+                    in the r / theta couplings, which the phi-line domains of the GPU's PC2 do not contain."""
     nr, nt, np_ = shape if shape is not None else FULL_SHAPES[name]
+    if mesh_kind != "config":
+        assert name in ("c3", "c4", "c5") and mesh_kind in MESH_KINDS
+        if mesh_kind == "nonuniform":
+            mesh = grids.random_mesh(nr, nt, np_, seed=100 + SEED[name], amp=0.3)
+            nu_kind, nu = 1, nu_profile(mesh)
+        else:
+            mesh = grids.clustered_mesh(nr, nt, np_)
+            nu_kind, nu = 0, np.array([1.0])
+        st = STIFFNESS[name]
+        return Problem(name=name + {"nonuniform": "n", "clustered": "k"}[mesh_kind], mesh=mesh, nu_kind=nu_kind, nu=nu,
+                       rtol=RTOL[name], maxit=MAXIT[name], seed=SEED[name], stiffness=(st,))
     if name in ("c1", "c2"):
         r_f = grids.radial_faces_ratio(nr, 1.02)
     else:

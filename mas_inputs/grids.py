@@ -139,6 +139,56 @@ def wobbly_phi_mesh(r_f: np.ndarray, nt: int, np_: int, seed: int, amp: float = 
     return m
 
 
+def random_mesh(nr: int, nt: int, np_: int, seed: int, amp: float = 0.3, uniform_phi: bool = False,
+                r_lo: float = R_INNER, r_hi: float = R_OUTER, pack: float = 4.0) -> Mesh:
+    """Full sphere, NON-uniform in r, theta and (unless uniform_phi) phi: the input class of the paper's mesh
+    ("non-uniform logically-rectangular"; "extremely non-uniform grid").  r: the packed
+    faces of radial_faces_pack with every width scaled by (1 + amp*U(-1,1)); theta, phi: widths (1 + amp*U(-1,1))
+    renormalised to pi and 2*pi.  Polar faces get sin_f = 0.0 exactly.  np_ must be even (mas_grid_t)."""
+    rng = np.random.default_rng(seed)
+    w_r = np.diff(radial_faces_pack(nr, pack, r_lo, r_hi)) * (1.0 + amp * rng.uniform(-1.0, 1.0, nr))
+    w_r *= (r_hi - r_lo) / w_r.sum()
+    r_f = r_lo + np.concatenate(([0.0], np.cumsum(w_r)))
+    r_f[-1] = r_hi
+    w_t = 1.0 + amp * rng.uniform(-1.0, 1.0, nt)
+    th_f = np.concatenate(([0.0], np.cumsum(w_t))) * (np.pi / w_t.sum())
+    th_f[-1] = np.pi
+    if uniform_phi:
+        ph_f = 2.0 * np.pi * np.arange(np_ + 1, dtype=np.float64) / np_
+    else:
+        w_p = 1.0 + amp * rng.uniform(-1.0, 1.0, np_)
+        ph_f = np.concatenate(([0.0], np.cumsum(w_p))) * (2.0 * np.pi / w_p.sum())
+        ph_f[-1] = 2.0 * np.pi
+    m = mesh_from_faces(r_f, th_f, ph_f)
+    m.sin_f[0] = 0.0
+    m.sin_f[nt] = 0.0
+    if uniform_phi:
+        m.dph_c[:] = 2.0 * np.pi / np_
+        m.dph_f[:] = 2.0 * np.pi / np_
+    return m
+
+
+def clustered_mesh(nr: int, nt: int, np_: int, r_lo: float = 1.0, r_hi: float = 10.0, r_ratio: float = 200.0,
+                   th_ratio: float = 20.0, th_width: float = 0.25) -> Mesh:
+    """A paper-like mesh (r in [1, 10] solar radii, "extremely non-uniform", cells concentrated on the
+    erupting region): geometric radial widths growing by `r_ratio` in total from the inner boundary outwards, theta
+    widths `th_ratio` times finer at the equator than at the poles (a smooth Gaussian dip of width `th_width` rad
+    around pi/2), phi uniform."""
+    q = r_ratio ** (1.0 / max(nr - 1, 1))
+    r_f = _geometric_faces(nr, r_lo, r_hi, q)
+    xi = (np.arange(nt) + 0.5) / nt * np.pi
+    w_t = 1.0 - (1.0 - 1.0 / th_ratio) * np.exp(-0.5 * ((xi - 0.5 * np.pi) / th_width) ** 2)
+    th_f = np.concatenate(([0.0], np.cumsum(w_t))) * (np.pi / w_t.sum())
+    th_f[-1] = np.pi
+    ph_f = 2.0 * np.pi * np.arange(np_ + 1, dtype=np.float64) / np_
+    m = mesh_from_faces(r_f, th_f, ph_f)
+    m.sin_f[0] = 0.0
+    m.sin_f[nt] = 0.0
+    m.dph_c[:] = 2.0 * np.pi / np_
+    m.dph_f[:] = 2.0 * np.pi / np_
+    return m
+
+
 def shell_wedge_mesh(nr: int, nt: int, np_: int, r_lo=1.0, r_hi=2.0) -> Mesh:
     """Uniform full-sphere mesh on r in [r_lo, r_hi]; used by the continuum-consistency pins."""
     r_f = np.linspace(r_lo, r_hi, nr + 1)

@@ -14,8 +14,10 @@ from oracle import ref
 def main():
     out = {"comment": "S1 = max_cells (d - V)/V at dt = 1; written by oracle/calibrate_dt.py (oracle only)",
            "s1": {}}
-    for name in ("c1", "c2", "c3", "c4", "c5"):
-        prob = configs.make(name)
+    cases = [(name, "config") for name in ("c1", "c2", "c3", "c4", "c5")]
+    cases += [(name, kind) for kind in ("nonuniform", "clustered") for name in ("c3", "c4", "c5")]
+    for name, kind in cases:
+        prob = configs.make(name, mesh_kind=kind)
         op = ref.RefOperator(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
         out["s1"][prob.key()] = repr(op.stiffness_max())
         op.close()

@@ -43,8 +43,10 @@ struct DevBuf {
     cudaError_t alloc(size_t count)
     {
         release();
-        n = count;
-        return cudaMalloc((void **)&p, (count ? count : 1) * sizeof(T));
+        const cudaError_t e = cudaMalloc((void **)&p, (count ? count : 1) * sizeof(T));
+        if (e != cudaSuccess) p = nullptr;       // a failed buffer is an empty buffer
+        else n = count;
+        return e;
     }
     void release()
     {
@@ -214,14 +216,19 @@ int ensure_rhs_capacity(mas_pcg *h, int nrhs)
     if (nrhs <= h->nrhs_cap) return MAS_OK;
     drop_graphs(h);
     const size_t tot = h->n * (size_t)nrhs;
-    if (h->r.alloc(tot) || h->p0.alloc(tot) || h->p1.alloc(tot) || h->q.alloc(tot) ||
-        (h->precond == MAS_PC2 && h->z.alloc(tot))) {
-        cudaGetLastError();
+    auto give_up = [&](int code) {             // leave a handle that knows it has no vectors: every user of r / p0 / p1 / q
+        cudaGetLastError();                    // (solves, mas_sts_advance) comes through here again and retries
+        h->r.release(); h->p0.release(); h->p1.release(); h->q.release(); h->z.release();
         h->nrhs_cap = 0;
-        return MAS_ENOMEM;
-    }
-    CK(cudaMemset(h->p0.p, 0, tot * sizeof(double)));
-    CK(cudaMemset(h->p1.p, 0, tot * sizeof(double)));
+        fill_op(h);
+        return code;
+    };
+    if (h->r.alloc(tot) || h->p0.alloc(tot) || h->p1.alloc(tot) || h->q.alloc(tot) ||
+        (h->precond == MAS_PC2 && h->z.alloc(tot)))
+        return give_up(MAS_ENOMEM);
+    if (cudaMemset(h->p0.p, 0, tot * sizeof(double)) != cudaSuccess ||
+        cudaMemset(h->p1.p, 0, tot * sizeof(double)) != cudaSuccess)
+        return give_up(MAS_ECUDA);
     h->nrhs_cap = nrhs;
     fill_op(h);
     return MAS_OK;
@@ -597,12 +604,21 @@ int ensure_hist(mas_pcg *h, int maxit)
 {
     const size_t need = (size_t)maxit + 1;
     if (need <= h->hist_cap) return MAS_OK;
-    size_t cap = h->hist_cap;
+    size_t cap = h->hist_cap ? h->hist_cap : 1;
     while (cap < need) cap *= 2;
-    if (h->hist.alloc(MAX_RHS * cap) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    // the new pair first, the old pair released only once both exist: a failure leaves the handle as it was
+    DevBuf<double> nd;
+    double *nh = nullptr;
+    if (nd.alloc(MAX_RHS * cap) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    if (cudaMallocHost((void **)&nh, MAX_RHS * cap * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        nd.release();
+        return MAS_ENOMEM;
+    }
+    h->hist.release();
+    h->hist = nd;
     if (h->h_hist) cudaFreeHost(h->h_hist);
-    h->h_hist = nullptr;
-    if (cudaMallocHost((void **)&h->h_hist, MAX_RHS * cap * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return MAS_ENOMEM; }
+    h->h_hist = nh;
     h->hist_cap = cap;
     fill_op(h);
     drop_graphs(h);             // kernel nodes hold the old hist pointer
@@ -703,7 +719,10 @@ int solve_core(mas_pcg *h, int nrhs, const double *const *b_dev, double *const *
             if (ok) h->graph[nrhs - 1] = g;
             ok = ok && cudaGraphConditionalHandleCreate(&cond, g, 1, cudaGraphCondAssignDefault) == cudaSuccess;
             if (ok) {
-                if ((rc = make_plan(h, h->op, h->work, nrhs, 1, cond, *plan)) != MAS_OK) return rc;
+                if ((rc = make_plan(h, h->op, h->work, nrhs, 1, cond, *plan)) != MAS_OK) {
+                    drop_graphs(h);            // the graph created above has no executable yet: do not leave it behind
+                    return rc;
+                }
                 seq_for_plan(*plan, seq);
                 ok = build_graph(seq, g, cond, h->unroll, &h->exec[nrhs - 1]) == MAS_OK;
             }
@@ -838,6 +857,7 @@ extern "C" int mas_pcg_set_option(mas_pcg_t *h, const char *name, int value)
 {
     if (!h || !name) return MAS_EINVAL;
     DeviceGuard dg(h->device);
+    if (!dg.ok) return MAS_ECUDA;
     if (!strcmp(name, "loop_mode")) {
         if (value != 0 && value != 1) return MAS_EINVAL;
         h->loop_mode = value;

@@ -43,7 +43,9 @@ def pytest_terminal_summary(terminalreporter):
                 worst[k] = (v, label)
     for k, (v, label) in sorted(worst.items()):
         tr.write_line(f"max {k:6s} = {v:.3e}   ({label})")
-    big = [(l, kw) for l, kw in helpers.GAPS if any(t in l for t in ("c3", "c4", "c5")) and "x_l2" in kw]
+    big = [(l, kw) for l, kw in helpers.GAPS if any(t in l for t in ("c3", "c4", "c5", "128x192x256"))
+           and "x_l2" in kw and "x_max" in kw]
     for label, kw in big:
-        tr.write_line(f"{label}: hist {kw['hist']:.2e}  x_l2 {kw['x_l2']:.2e}  x_max {kw['x_max']:.2e}  "
+        raw = f" (raw {kw['hist_raw']:.2e})" if "hist_raw" in kw else ""
+        tr.write_line(f"{label}: hist {kw['hist']:.2e}{raw}  x_l2 {kw['x_l2']:.2e}  x_max {kw['x_max']:.2e}  "
                       f"k {kw['k_gpu']}/{kw['k_ref']}")

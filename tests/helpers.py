@@ -10,7 +10,10 @@ from oracle import ref
 # --- the gates (BASELINE.json north_star; readings Q9, Q10 of SURVEY.md 8(c)) ---
 HIST_RTOL = 1e-10      # per-iteration relative residual: |h_gpu - h_ref| / h_ref, first 50 iterations
 HIST_ITERS = 50
-HIST_FLOOR = 1e-15     # entries at the fp64 rounding floor (h ~ eps) carry no digits: absolute slack there
+HIST_FLOOR = 1e-15     # absolute slack, applied ONLY to entries at the rounding floor of the solve: h_ref[j] <
+                       # 1e3 * eps * h_ref[0] (such entries carry no digits); every other entry is gated on the raw
+                       # relative gap (round 3; before, the slack applied to every entry -- DESIGN.md R5)
+HIST_FLOOR_BELOW = 1e3 * np.finfo(np.float64).eps
 X_RTOL = 1e-9          # final x, relative L2, compared at EQUAL iteration counts
 APPLY_RTOL = 1e-14     # single matvec, relative to max |A u| (pure rounding-order difference; SURVEY 7 step 4.
                        # Observed on the B200, round 2: <= 3.7e-16 including config 3 at stiffness 1e4)
@@ -29,6 +32,18 @@ def apply_gap(y, y_ref, label):
     g = float(np.abs(y - y_ref).max() / max(np.abs(y_ref).max(), 1e-300))
     record_gap(label, apply=g)
     return g
+
+
+def hist_gaps(h_g, h_r, m):
+    """(gated, raw) largest relative gap over the first m history entries.  `raw` is |h_gpu - h_ref| / h_ref as it
+    stands; `gated` is the same except that entries below HIST_FLOOR_BELOW * h_ref[0] get HIST_FLOOR of absolute
+    slack (R5) -- it is what the gate tests.  Both are recorded so that the summary shows an observation,
+    not the floor (parity hygiene)."""
+    h_r = np.asarray(h_r[:m], dtype=np.float64)
+    d = np.abs(np.asarray(h_g[:m]) - h_r)
+    den = np.maximum(h_r, 1e-300)
+    slack = np.where(h_r < HIST_FLOOR_BELOW * h_r[0], HIST_FLOOR, 0.0)
+    return float((np.maximum(d - slack, 0.0) / den).max()), float((d / den).max())
 
 
 def oracle_s1(mesh, nu_kind, nu, bc=(0, 0)) -> float:
@@ -62,8 +77,8 @@ def check_parity(gpu, oref, b, x0, rtol, maxit, *, label=""):
     assert st_g == st_r, f"{label}: status gpu {st_g} vs oracle {st_r}"
     assert abs(k_g - k_r) <= 1, f"{label}: iterations gpu {k_g} vs oracle {k_r}"
     m = min(HIST_ITERS, k_r, k_g) + 1
-    rel = np.maximum(np.abs(h_g[:m] - h_r[:m]) - HIST_FLOOR, 0.0) / h_r[:m]
-    assert rel.max() <= HIST_RTOL, f"{label}: history gap {rel.max():.3e} at it {rel.argmax()}"
+    hist_gated, hist_raw = hist_gaps(h_g, h_r, m)
+    assert hist_gated <= HIST_RTOL, f"{label}: history gap {hist_gated:.3e} (raw {hist_raw:.3e})"
     if k_g != k_r:      # Q10: compare x at equal iteration counts
         xd = torch.zeros_like(bd) if x0 is None else torch.from_numpy(np.ascontiguousarray(x0)).cuda()
         _, k_g2, _ = gpu.solve(bd, xd, 0.0, k_r)
@@ -73,7 +88,7 @@ def check_parity(gpu, oref, b, x0, rtol, maxit, *, label=""):
     # element-wise: the largest single-cell gap relative to max |x| (a localised error in a few boundary
     # rows would hide under the L2 gate on a large mesh); reported, and gated at 100x the L2 tolerance
     emax = float(np.abs(xg - x_r).max() / np.abs(x_r).max())
-    record_gap(label, hist=float(rel.max()), x_l2=float(err), x_max=emax, k_ref=k_r, k_gpu=k_g)
+    record_gap(label, hist=hist_gated, hist_raw=hist_raw, x_l2=float(err), x_max=emax, k_ref=k_r, k_gpu=k_g)
     assert err <= X_RTOL, f"{label}: x gap {err:.3e}"
     assert emax <= 100 * X_RTOL, f"{label}: element-wise x gap {emax:.3e}"
     return k_r, k_g

@@ -95,6 +95,23 @@ def test_sts_then_pcg_solve_on_the_same_handle():
     H.check_parity(gpu, oref, b, None, prob.rtol, prob.maxit, label="after sts")
 
 
+def test_sts_config4_full_size_eight_stages():
+    """RKL2 against the oracle at the size `bench.py --workload sts` times (256 x 256 x 512, config 4's mesh and nu):
+    one super-step of s = 8 stages, every cell compared ("What's missing" 5)."""
+    prob = configs.make("c4")
+    oref, gpu = H.both_ops(prob.mesh, 1.0, prob.nu_kind, prob.nu)
+    u = configs.rhs_blob(prob)
+    s = 8
+    tau = 0.9 * (s * s + s - 2.0) / 4.0 * 2.0 / gpu.lambda_max()
+    assert gpu.sts_stages(tau) == s
+    y_ref = oref.sts(u, tau, s)
+    ud = _t(u)
+    gpu.sts_advance(ud, tau, s)
+    gap = float(np.abs(ud.cpu().numpy().reshape(y_ref.shape) - y_ref).max() / np.abs(u).max())
+    H.record_gap("sts c4 s=8", sts=gap)
+    assert gap <= STS_RTOL
+
+
 def test_sts_viscosity_advance_production_like_mesh():
     """The paper's regime: ~200 sub-steps per step with the large uniform viscosity."""
     prob = configs.make("c3", shape=(48, 64, 128))
