@@ -86,6 +86,22 @@ constexpr int ST_OK = 0, ST_MAXIT = 1, ST_BREAKDOWN = -4;
 
 __device__ __forceinline__ double *part_base(const Work &w, int rhs) { return w.partials + (size_t)rhs * PART_REGIONS * w.pstride; }
 
+// 1/d for the point-Jacobi step z = r/d on meshes that are non-uniform in phi, where d = vp[k] E + F wp[k] differs from
+// cell to cell and no reciprocal plane exists (uniform phi: the Dinv plane).  rcp.approx.ftz.f64 gives 20 good bits;
+// two Newton steps x <- x + x (1 - d x) square the error twice: < 1 ulp of 1/d, so r * rcp_nr(d) is within ~1.5 ulp of
+// the IEEE quotient -- the same class of difference as r * Dinv on uniform meshes (R6) -- at 5 DFMA-class
+// instructions instead of the ~20 plus a slow-path branch of the IEEE division.  d is a diagonal entry of an SPD
+// operator: positive, normal range.  Every kernel that forms z uses this one function, so K1's prologue, K2's sums
+// and the init step see the same z bit for bit.
+__device__ __forceinline__ double rcp_nr(double d)
+{
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+    x = fma(x, fma(-d, x, 1.0), x);
+    x = fma(x, fma(-d, x, 1.0), x);
+    return x;
+}
+
 __device__ __forceinline__ double warp_sum(double v)
 {
 #pragma unroll

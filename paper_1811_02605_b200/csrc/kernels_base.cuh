@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(NT) k_init(OpDev op, Work w, cudaGraphConditio
         acc[0] += bs0 * bs0 + bs1 * bs1;
         acc[1] += r.x * r.x + r.y * r.y;
         acc[2] += UNIFORM ? r.x * (r.x * dinv) + r.y * (r.y * dinv)      // same z as K1/K2 use
-                          : r.x * (r.x / d0) + r.y * (r.y / d1);
+                          : r.x * (r.x * rcp_nr(d0)) + r.y * (r.y * rcp_nr(d1));
     }
     if (grid_sum<NT, 3>(acc, part_base(w, rhs), w.pstride, &w.tickets[rhs * 4 + 0], sh) && threadIdx.x == 0)
         reduction_done<ROLE_INIT, 3>(w, rhs, acc, cond, use_cond);
@@ -252,8 +252,8 @@ OpDev op, Work w, cudaGraphConditionalHandle cond, int use_cond,
         } else {
             const int k = 2 * (v - row * op.nv);
             const double E = __ldg(op.E + crow0 + row), F = __ldg(op.F + crow0 + row);
-            z0 = rv.x / fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k));
-            z1 = rv.y / fma(__ldg(op.vp + k + 1), E, F * __ldg(op.wp + k + 1));
+            z0 = rv.x * rcp_nr(fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k)));
+            z1 = rv.y * rcp_nr(fma(__ldg(op.vp + k + 1), E, F * __ldg(op.wp + k + 1)));
         }
         acc[0] += rv.x * z0 + rv.y * z1;
         acc[1] += rv.x * rv.x + rv.y * rv.y;

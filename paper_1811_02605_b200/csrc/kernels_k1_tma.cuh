@@ -98,7 +98,14 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
     const PhiFac<UNIFORM, TileCoefs<NW, UNIFORM>> ph = {sm.c, mp.vp, mp.wp, mp.ip};
     const int ea = 2 * lane + 1, eb = 2 * lane + 65;
     auto zval = [&](double r, double E, double F, double dinv, int e) {
-        return zin ? r : (UNIFORM ? r * dinv : r / fma(ph.VP(e), E, F * ph.WP(e)));
+        return zin ? r : (UNIFORM ? r * dinv : r * rcp_nr(fma(ph.VP(e), E, F * ph.WP(e))));
+    };
+
+    auto zval2 = [&](double2 r, double E, double F, double dinv, int e) {       // the two cells (e, e + 1) of a vector
+        if (zin) return r;
+        if (UNIFORM) return make_double2(r.x * dinv, r.y * dinv);
+        const double2 v = ph.VP2(e), wv = ph.WP2(e);
+        return make_double2(r.x * rcp_nr(fma(v.x, E, F * wv.x)), r.y * rcp_nr(fma(v.y, E, F * wv.y)));
     };
 
     const long long plane = (long long)op.nt * op.np;
@@ -166,12 +173,14 @@ k1_tma(OpDev op, Work w, TileParams mp, cudaGraphConditionalHandle cond, int use
             const double2 ra = fr[1 + lane], rb = fr[33 + lane];
             const double2 pa = fp[1 + lane], pb = fp[33 + lane];
             if (UNIFORM || g.vA) {
-                an.x = fma(beta, pa.x, zval(ra.x, En, Fn, dinv, ea));
-                an.y = fma(beta, pa.y, zval(ra.y, En, Fn, dinv, ea + 1));
+                const double2 z = zval2(ra, En, Fn, dinv, ea);
+                an.x = fma(beta, pa.x, z.x);
+                an.y = fma(beta, pa.y, z.y);
             }
             if (UNIFORM || g.vB) {
-                bn.x = fma(beta, pb.x, zval(rb.x, En, Fn, dinv, eb));
-                bn.y = fma(beta, pb.y, zval(rb.y, En, Fn, dinv, eb + 1));
+                const double2 z = zval2(rb, En, Fn, dinv, eb);
+                bn.x = fma(beta, pb.x, z.x);
+                bn.y = fma(beta, pb.y, z.y);
             }
             if (g.left_edge) hl_n = fma(beta, fp[0].y, zval(fr[0].y, En, Fn, dinv, 0));
             if (g.right_edge) hr_n = fma(beta, fp[g.hr].x, zval(fr[g.hr].x, En, Fn, dinv, g.tkeff + 1));

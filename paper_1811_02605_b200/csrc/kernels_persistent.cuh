@@ -176,8 +176,8 @@ __global__ void __launch_bounds__(PNT, 1) k_pcg_persistent(OpDev op, PersistPara
             return make_double2(rv.x * dinv, rv.y * dinv);
         }
         const double E = __ldg(op.E + rw), F = __ldg(op.F + rw);
-        return make_double2(rv.x / fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k)),
-                            rv.y / fma(__ldg(op.vp + k + 1), E, F * __ldg(op.wp + k + 1)));
+        return make_double2(rv.x * rcp_nr(fma(__ldg(op.vp + k), E, F * __ldg(op.wp + k))),
+                            rv.y * rcp_nr(fma(__ldg(op.vp + k + 1), E, F * __ldg(op.wp + k + 1))));
     };
 
     // ---- init: b_s = V b, r = b_s - A x0, z_0 -> Z, P[1] = 0 (p_{-1}), sums bb, rr, rho ----

@@ -193,13 +193,17 @@ k_stencil_tma(OpDev op, StencilParams mp)
                     o.y = fma(-alpha, s.y, rv.y);
                     double z0, z1;
                     if (UNIFORM) { z0 = o.x * dsc; z1 = o.y * dsc; }
-                    else { z0 = o.x / fma(ph.VP(e), rc.Ec, rc.Fc * ph.WP(e)); z1 = o.y / fma(ph.VP(e + 1), rc.Ec, rc.Fc * ph.WP(e + 1)); }
+                    else {
+                        const double2 v = ph.VP2(e), wv = ph.WP2(e);
+                        z0 = o.x * rcp_nr(fma(v.x, rc.Ec, rc.Fc * wv.x)); z1 = o.y * rcp_nr(fma(v.y, rc.Ec, rc.Fc * wv.y));
+                    }
                     acc[0] += o.x * z0 + o.y * z1;
                     acc[1] += o.x * o.x + o.y * o.y;
                 } else {
                     double2 mu;                                  // M u = -S u / (V2 vp)
-                    mu.x = UNIFORM ? -(s.x * dsc) * (1.0 / mp.t.vp) : -(s.x * dsc) / ph.VP(e);
-                    mu.y = UNIFORM ? -(s.y * dsc) * (1.0 / mp.t.vp) : -(s.y * dsc) / ph.VP(e + 1);
+                    const double2 rvp = ph.RVP2(e);
+                    mu.x = -(s.x * dsc) * rvp.x;
+                    mu.y = -(s.y * dsc) * rvp.y;
                     if (mp.out2) st2g(mp.out2, orow + kcell, mu);
                     o.x = mp.c_u * uc.x + mp.c_L * mu.x;
                     o.y = mp.c_u * uc.y + mp.c_L * mu.y;

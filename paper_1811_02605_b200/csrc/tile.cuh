@@ -217,6 +217,14 @@ template <int NW, bool UNIFORM>
 struct TileCoefs {
     double cE[TILE_NPL][NW], cF[TILE_NPL][NW], cD[TILE_NPL][NW], cAR[TILE_NPL][NW], cAT[TILE_NPL][NW];
     double phv[UNIFORM ? 1 : TILE_TK + 2], phw[UNIFORM ? 1 : TILE_TK + 2], phi[UNIFORM ? 1 : TILE_TK + 2];
+    double phr[UNIFORM ? 1 : TILE_TK + 2];   // 1/vp: the M u = -S u / V epilogue multiplies instead of dividing per cell
+    // The same factors once more as PAIRS, for the two cells (2l+1, 2l+2) of half-row vector l (l = lane, lane + 32): a
+    // lane then fetches what its vector needs with one 16-byte load per array, lanes 16 bytes apart -- conflict-free --
+    // instead of two 8-byte loads 16 bytes apart (2-way bank conflicts: ncu counted 16.7 M conflicts per K1 launch on
+    // the non-uniform 256x256x512 mesh against 2.1 M on the uniform one).  ipm[l] = ip of cell 2l (face 2l + 1/2).
+    alignas(16) double2 pv2[UNIFORM ? 1 : TILE_TK / 2], pw2[UNIFORM ? 1 : TILE_TK / 2], pi2[UNIFORM ? 1 : TILE_TK / 2],
+        pr2[UNIFORM ? 1 : TILE_TK / 2];
+    double ipm[UNIFORM ? 1 : TILE_TK / 2];
 };
 
 struct PlaneSetDev {                         // which planes the stencil uses (dt-scaled: A_sym; base: L_sym)
@@ -252,7 +260,15 @@ __device__ __forceinline__ void stage_coefs(C &sm, const TileGeom &g, const OpDe
             int kk = g.k0 - 1 + e;                                // wrap once in either direction
             kk = kk < 0 ? kk + op.np : (kk >= op.np ? kk - op.np : kk);
             kk = kk >= op.np ? kk % op.np : kk;                   // tiny meshes (np < 130)
-            sm.phv[e] = __ldg(op.vp + kk); sm.phw[e] = __ldg(op.wp + kk); sm.phi[e] = __ldg(op.ip + kk);
+            const double v = __ldg(op.vp + kk), wv = __ldg(op.wp + kk), iv = __ldg(op.ip + kk), rv = 1.0 / v;
+            sm.phv[e] = v; sm.phw[e] = wv; sm.phi[e] = iv; sm.phr[e] = rv;
+            if (e >= 1 && e <= TILE_TK) {                         // cell e of the tile = component (e-1)&1 of pair (e-1)>>1
+                const int l = (e - 1) >> 1;
+                double *pv = reinterpret_cast<double *>(&sm.pv2[l]), *pw = reinterpret_cast<double *>(&sm.pw2[l]);
+                double *pi = reinterpret_cast<double *>(&sm.pi2[l]), *pr = reinterpret_cast<double *>(&sm.pr2[l]);
+                pv[(e - 1) & 1] = v; pw[(e - 1) & 1] = wv; pi[(e - 1) & 1] = iv; pr[(e - 1) & 1] = rv;
+            }
+            if (!(e & 1) && e < TILE_TK) sm.ipm[e >> 1] = iv;   // ip of cell e = 2l
         }
 }
 
@@ -265,6 +281,13 @@ struct PhiFac {
     __device__ __forceinline__ double VP(int e) const { return UNIFORM ? vp : sm.phv[e]; }
     __device__ __forceinline__ double WP(int e) const { return UNIFORM ? wp : sm.phw[e]; }
     __device__ __forceinline__ double IP(int e) const { return UNIFORM ? ip : sm.phi[e]; }   // face e+1/2
+    __device__ __forceinline__ double RVP(int e) const { return UNIFORM ? 1.0 / vp : sm.phr[e]; }
+    // pairs for the vector whose first cell is e (odd): (X(e), X(e+1)); IPM = IP(e-1)
+    __device__ __forceinline__ double2 VP2(int e) const { return UNIFORM ? make_double2(vp, vp) : sm.pv2[(e - 1) >> 1]; }
+    __device__ __forceinline__ double2 WP2(int e) const { return UNIFORM ? make_double2(wp, wp) : sm.pw2[(e - 1) >> 1]; }
+    __device__ __forceinline__ double2 IP2(int e) const { return UNIFORM ? make_double2(ip, ip) : sm.pi2[(e - 1) >> 1]; }
+    __device__ __forceinline__ double2 RVP2(int e) const { return UNIFORM ? make_double2(1.0 / vp, 1.0 / vp) : sm.pr2[(e - 1) >> 1]; }
+    __device__ __forceinline__ double IPM(int e) const { return UNIFORM ? ip : sm.ipm[(e - 1) >> 1]; }
 };
 
 struct RowCoefs {                            // coefficients of the row whose stencil is being formed (plane t-1)
@@ -294,9 +317,11 @@ __device__ __forceinline__ double2 stencil_half(const PF &ph, int e, const RowCo
         s.y = fma(-c.Fc, ukp + uc.x, c.Ec * uc.y - sy);
         return s;
     }
-    const double d0 = fma(ph.VP(e), c.Ec, c.Fc * ph.WP(e)), d1 = fma(ph.VP(e + 1), c.Ec, c.Fc * ph.WP(e + 1));
-    s.x = d0 * uc.x - ph.VP(e) * sx - c.Fc * (ph.IP(e) * uc.y + ph.IP(e - 1) * ukm);
-    s.y = d1 * uc.y - ph.VP(e + 1) * sy - c.Fc * (ph.IP(e + 1) * ukp + ph.IP(e) * uc.x);
+    const double2 v = ph.VP2(e), wv = ph.WP2(e), iv = ph.IP2(e);     // same arithmetic as with the scalar factors, in
+    const double im = ph.IPM(e);                                     // the same order: results are bit-identical
+    const double d0 = fma(v.x, c.Ec, c.Fc * wv.x), d1 = fma(v.y, c.Ec, c.Fc * wv.y);
+    s.x = d0 * uc.x - v.x * sx - c.Fc * (iv.x * uc.y + im * ukm);
+    s.y = d1 * uc.y - v.y * sy - c.Fc * (iv.y * ukp + iv.x * uc.x);
     return s;
 }
 

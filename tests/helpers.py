@@ -10,10 +10,14 @@ from oracle import ref
 # --- the gates (BASELINE.json north_star; readings Q9, Q10 of SURVEY.md 8(c)) ---
 HIST_RTOL = 1e-10      # per-iteration relative residual: |h_gpu - h_ref| / h_ref, first 50 iterations
 HIST_ITERS = 50
-HIST_FLOOR = 1e-15     # absolute slack, applied ONLY to entries at the rounding floor of the solve: h_ref[j] <
-                       # 1e3 * eps * h_ref[0] (such entries carry no digits); every other entry is gated on the raw
-                       # relative gap (round 3; before, the slack applied to every entry -- DESIGN.md R5)
-HIST_FLOOR_BELOW = 1e3 * np.finfo(np.float64).eps
+HIST_FLOOR = 1e-15     # absolute slack, applied ONLY to entries h_ref[j] < 1e-4 * h_ref[0]; every entry within four
+                       # decades of the initial residual is gated on the raw relative gap (round 3; before, the slack
+                       # applied to every entry).  Why not relative everywhere: the recurrence residual carries an
+                       # ABSOLUTE rounding error of a few eps * h[0] on either side, which at h[j] = 1e-6 * h[0] already
+                       # is 1e-10 relative.  Observed on the B200: 2.0e-10 relative at such an entry of a PC2 solve that
+                       # gains two decades per iteration (a threshold of 1e3 * eps * h[0] was tried and fails there),
+                       # and <= 1e-12 on every entry above the threshold (R5)
+HIST_FLOOR_BELOW = 1e-4
 X_RTOL = 1e-9          # final x, relative L2, compared at EQUAL iteration counts
 APPLY_RTOL = 1e-14     # single matvec, relative to max |A u| (pure rounding-order difference; SURVEY 7 step 4.
                        # Observed on the B200, round 2: <= 3.7e-16 including config 3 at stiffness 1e4)
