@@ -290,10 +290,33 @@ def test_P1_manufactured_solution_config2(s):
 
 def test_calibration_file_matches_oracle():
     """mas_inputs/dt_calibration.json is what oracle/calibrate_dt.py would write today."""
-    for name in ("c1", "c2", "c3"):
-        prob = configs.make(name)
+    for name, kind in (("c1", "config"), ("c2", "config"), ("c3", "config"), ("c3", "nonuniform"), ("c3", "clustered")):
+        prob = configs.make(name, mesh_kind=kind)
         op = ref.RefOperator(prob.mesh, 1.0, prob.nu_kind, prob.nu, prob.bc)
         assert op.stiffness_max() == pytest.approx(prob.s1(), rel=1e-14)
+        op.close()
+
+
+@pytest.mark.parametrize("kind", ["nonuniform", "clustered"])
+def test_round3_mesh_kinds_are_valid_inputs_and_give_an_spd_operator(kind):
+    """grids.random_mesh / grids.clustered_mesh: widths positive and summing to the domain,
+    polar faces of zero area, theta really non-uniform, and -- on a reduced shape -- the oracle's operator on them
+    is the symmetric positive definite M-matrix the pins above establish for the other meshes."""
+    prob = configs.make("c3", shape=(5, 7, 8), mesh_kind=kind)
+    m = prob.mesh
+    assert prob.name == {"nonuniform": "c3n", "clustered": "c3k"}[kind]
+    for w, total in ((m.dr_c, m.r_f[-1] - m.r_f[0]), (m.dth_c, np.pi), (m.dph_c, 2 * np.pi)):
+        assert np.all(w > 0) and w.sum() == pytest.approx(total, rel=1e-13)
+    assert m.sin_f[0] == 0.0 and m.sin_f[-1] == 0.0 and np.all(m.sin_f[1:-1] > 0)
+    assert np.ptp(m.dth_c) > 0.1 * m.dth_c.mean()
+    assert (np.ptp(m.dph_c) > 0) == (kind == "nonuniform")
+    op = ref.RefOperator(m, 1.0, prob.nu_kind, prob.nu, prob.bc)
+    op.set_dt(100.0 / op.stiffness_max())
+    A = op.dense()
+    assert np.array_equal(A, A.T) and np.all(np.diag(A) > 0)
+    np.linalg.cholesky(A)
+    assert np.allclose(A.sum(axis=1)[m.nt * m.np_:-m.nt * m.np_], op.volume().ravel()[m.nt * m.np_:-m.nt * m.np_], rtol=1e-12)
+    op.close()
 
 
 def test_config1_diagonal_dominance_ratio_is_1p5():
