@@ -226,7 +226,7 @@ def run_chain(args):
     from mas_inputs import configs
     from paper_1811_02605_b200 import MasPcg
     torch.cuda.set_device(0)
-    prob = configs.make("c5")
+    prob = configs.make("c5", mesh_kind=args.mesh)
     nsteps = max(args.chain_steps, 1)
     dt0 = prob.dt_for(prob.stiffness[-1])
     chain = configs.Chain(prob, 100)
@@ -282,7 +282,7 @@ def run_chain(args):
     peak, peak_src = hbm_peak()
     its = float(np.sum(iters))
     gbs = bpc * n * its / (total_ms * 1e-3) / 1e9
-    line = {"metric": "pcg_solves_per_s_192x256x384_timestep_proxy", "value": nsteps / (total_ms * 1e-3),
+    line = {"metric": "pcg_solves_per_s_192x256x384_timestep_proxy" + ("" if args.mesh == "config" else f"_{args.mesh}_mesh"), "value": nsteps / (total_ms * 1e-3),
             "unit": "solves/s", "n_gpus": 1, "steps": nsteps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / nsteps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",

@@ -251,11 +251,16 @@ inline int k1_tma_num_tiles() { return (int)(sizeof(kK1TmaTiles) / sizeof(kK1Tma
 // blocks in turn (configs 4, 5); when all of its tiles fit in ONE round (mid-size meshes such as config 3: 140 blocks on
 // 148 SMs) nothing overlaps a block's start-up and reduction tail, and the 6-row tile with two blocks per SM is faster
 // (measured on config 3: 0.0591 vs 0.0619 ms).
-inline int k1_auto_tile(int nr, int nt, int np, int num_sms)
+// Non-uniform phi (round 3): the general kernel issues ~30 % more instructions per cell and is latency- rather than
+// DRAM-bound, so the 16-row tile (18 warps per block at 96 registers instead of 16 at 120) wins on multi-round meshes:
+// 256x256x512 with +-30 % widths, K1 per tile id 0..6 = 0.2992, 0.4209, 0.3397, 0.3635, 0.3207, 0.2863, 0.3040 ms
+// (profiles/r3_k1_tile_sweep_nonuniform.md).
+inline int k1_auto_tile(int nr, int nt, int np, int num_sms, bool uniform_phi)
 {
     const long long cols = (long long)((np + TILE_TK - 1) / TILE_TK) * ((nt + 13) / 14);
     const int ci = tile_pick_ci(nr, cols, num_sms, 0);
-    return cols * ((nr + ci - 1) / ci) <= num_sms ? 2 : 0;
+    if (cols * ((nr + ci - 1) / ci) <= num_sms) return 2;
+    return uniform_phi ? 0 : 5;
 }
 
 template <int TJ, int DEPTH, int MINB>

@@ -484,7 +484,7 @@ int make_plan(const mas_pcg *h, const OpDev &op, const Work &work, int nrhs, int
     }
     // K1
     memset(&c.k1p, 0, sizeof(c.k1p));
-    const int k1_tile = h->tile >= 0 ? h->tile : k1_auto_tile(op.nr, op.nt, op.np, h->num_sms);
+    const int k1_tile = h->tile >= 0 ? h->tile : k1_auto_tile(op.nr, op.nt, op.np, h->num_sms, h->uniform_phi != 0);
     k1_tma_configure(op.nr, op.nt, op.np, uni, h->qrecompute != 0 && !pc2, k1_tile, h->num_sms, h->ci_force, nrhs, &c.k1p,
                      &c.k1.func, &c.k1.grid, &c.k1.block, &c.k1.smem);
     c.k1p.vp = h->vp0; c.k1p.wp = h->wp0; c.k1p.ip = h->ip0;
